@@ -1,0 +1,142 @@
+/*
+ * heal.h -- C ABI of the B200-native HEAL compensated GEMM library (libheal.so).
+ *
+ * The operation (Section 3 "Mitigating GEMM Truncation via FP16 Promotion and
+ * Algebraic Compensation"): an FP32 activation matrix h is decomposed into two FP16 matrices,
+ *      h = h_hi + h_lo / 2^s            hi = r16(h),  lo = r16((h - hi) * 2^s)
+ * (r16 = round-to-nearest-even to IEEE binary16) and the GEMM is expanded into FP16 tensor-core
+ * products accumulated in FP32 into an FP32 output (Eq. 10, 563, 571):
+ *      2 products:  C = h_hi.W + h_lo.W                         W already FP16      (Eq. 10)
+ *      3 products:  C = A_hi.B_hi + A_hi.B_lo + A_lo.B_hi       both operands FP32  (Eq. 9 expansion,
+ *                                                               PAPER.md:195; lo.lo dropped)
+ *      1 product :  C = h_hi.W                                  the "skipped layer" / HEAL-Base GEMM
+ *
+ * This build uses s = 0 (BASELINE.json north_star: lo = r16(x - hi), all products into one
+ * accumulator); reading A1 discusses the paper's s = 10.
+ *
+ * Reduction order (fixed; a function of K and mode only, never of M, N, tile shape or launch):
+ *   K is cut into segments of HEAL_K_SEGMENT = 512 consecutive k.  Within a segment the tensor core
+ *   accumulates in FP32, k ascending in slices of 16, the products of one slice issued in the order
+ *   listed above.  Segment partial sums are added in FP32 (round-to-nearest) in ascending segment
+ *   order.  No split-K atomics.  Results are bit-identical run to run, across M and across row
+ *   position.
+ *
+ * All matrices are row-major.  Unless a function says "host", pointers are DEVICE pointers, and
+ * the call is asynchronous on `stream` (a cudaStream_t passed as void*; NULL = the legacy default
+ * stream).  The library never prints and never aborts; every entry point returns a heal_status.
+ * There is no CPU fallback: without an sm_100 device every compute call returns HEAL_ERR_CUDA /
+ * HEAL_ERR_UNSUPPORTED_DEVICE.
+ */
+#ifndef HEAL_H_
+#define HEAL_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    HEAL_OK = 0,
+    HEAL_ERR_INVALID_VALUE = 1,      /* negative dimension, leading dimension too small            */
+    HEAL_ERR_NULL_POINTER = 2,       /* NULL matrix pointer with a non-empty problem               */
+    HEAL_ERR_MISALIGNED = 3,         /* pointer not 16-byte aligned / leading dimension not a
+                                        multiple of 16 bytes (TMA and 128-bit loads need both)     */
+    HEAL_ERR_UNSUPPORTED_MODE = 4,   /* unknown mode bits, or B dtype/mode mismatch                */
+    HEAL_ERR_CUDA = 5,               /* a CUDA call failed; see heal_last_cuda_error()             */
+    HEAL_ERR_WORKSPACE = 6,          /* caller-supplied workspace too small                        */
+    HEAL_ERR_UNSUPPORTED_DEVICE = 7  /* current device is not sm_100                               */
+} heal_status;
+
+#define HEAL_K_SEGMENT 512
+
+/* mode word ------------------------------------------------------------------------------------ */
+#define HEAL_MODE_PRODUCTS_MASK 0x0fu
+#define HEAL_MODE_1P 1u        /* hi.W                      B is FP16                              */
+#define HEAL_MODE_2P 2u        /* hi.W + lo.W               B is FP16   (Eq. 10)     */
+#define HEAL_MODE_3P 3u        /* hi.hi + hi.lo + lo.hi     B is FP32   (Eq. 9)      */
+#define HEAL_MODE_4P 4u        /* 3P + lo.lo (diagnostic)   B is FP32                              */
+#define HEAL_B_NK 0x10u        /* B is stored N x K (K contiguous) -- the paper's W^T /
+                                  nn.Linear layout; default is K x N (N contiguous) */
+
+/*
+ * C[M x N] (FP32) = A[M x K] (FP32) . B          one pass of the whole path: split, MMAs, epilogue.
+ *   A    FP32, lda >= K elements; 16-byte aligned, lda % 4 == 0.  Read-only.
+ *   B    FP16 (modes 1P, 2P) or FP32 (modes 3P, 4P).  K x N with ldb >= N, or N x K with ldb >= K
+ *        if HEAL_B_NK.  16-byte aligned; ldb % 8 == 0 (FP16) / ldb % 4 == 0 (FP32).  Read-only.
+ *   C    FP32, ldc >= N, 16-byte aligned, ldc % 4 == 0.  Overwritten (no beta).  Must not alias A/B.
+ *   M == 0 or N == 0: no-op, HEAL_OK.  K == 0: C is zero-filled.
+ * Ownership: the caller owns A, B, C and keeps them alive until `stream` has passed the call.  The
+ * hi/lo planes live in a library-owned workspace (see heal_set_workspace) which this call may
+ * grow with stream-ordered allocation; calls that share a workspace must be issued on one stream
+ * at a time.  Numerical contract: finite inputs with |x| <= 65504 (activations
+ * observed < 1024); anything larger, Inf or NaN propagates to Inf/NaN in the affected rows/columns.
+ */
+int heal_gemm(int64_t M, int64_t N, int64_t K,
+              const void *A, int64_t lda,
+              const void *B, int64_t ldb,
+              void *C, int64_t ldc,
+              uint32_t mode, void *stream);
+
+/*
+ * Step S alone: hi[r][c] = r16(X[r][c]), lo[r][c] = r16(X[r][c] - hi[r][c]).
+ *   X      FP32 rows x cols, ldx >= cols
+ *   hi,lo  FP16 rows x cols, leading dimension ld >= cols (elements)
+ * All pointers 16-byte aligned; ldx % 4 == 0 and ld % 8 == 0.  Used by tests and to pre-split
+ * static FP32 weights once (three-product mode).
+ */
+int heal_split(int64_t rows, int64_t cols, const void *X, int64_t ldx,
+               void *hi, void *lo, int64_t ld, void *stream);
+
+/*
+ * Steps G + E on pre-split planes: C = sum of the products `mode` keeps.
+ *   A_hi, A_lo   FP16 M x K, leading dimension lda (elements, % 8 == 0).  A_lo may be NULL for 1P.
+ *   B_hi, B_lo   FP16 K x N (or N x K with HEAL_B_NK), leading dimension ldb (% 8 == 0).
+ *                B_lo is ignored (may be NULL) for 1P/2P.
+ * Same alignment, aliasing and asynchrony rules as heal_gemm.  Never allocates.
+ */
+int heal_gemm_presplit(int64_t M, int64_t N, int64_t K,
+                       const void *A_hi, const void *A_lo, int64_t lda,
+                       const void *B_hi, const void *B_lo, int64_t ldb,
+                       void *C, int64_t ldc,
+                       uint32_t mode, void *stream);
+
+/*
+ * HOST-buffer variant of heal_gemm: A, B, C are HOST pointers (ideally pinned).  Copies A and B to
+ * the device, runs the path, copies C back and synchronises `stream` before returning.  Same
+ * layout rules as heal_gemm except that alignment applies to the internal device copies only.
+ * Staging buffers are library-owned and reused between calls.
+ */
+int heal_gemm_host(int64_t M, int64_t N, int64_t K,
+                   const void *A_host, int64_t lda,
+                   const void *B_host, int64_t ldb,
+                   void *C_host, int64_t ldc,
+                   uint32_t mode, void *stream);
+
+/* Bytes of workspace heal_gemm needs for this problem (hi/lo planes of A, and of B in 3P/4P). */
+size_t heal_workspace_size(int64_t M, int64_t N, int64_t K, uint32_t mode);
+
+/*
+ * Hand the library a caller-owned device workspace (256-byte aligned) so that heal_gemm never
+ * allocates; it must stay valid until replaced.  (NULL, 0) returns to the library-owned,
+ * lazily-grown workspace.  heal_gemm returns HEAL_ERR_WORKSPACE if a supplied one is too small.
+ */
+int heal_set_workspace(void *ptr, size_t bytes);
+
+/* Number of kernels heal_* calls have launched in this process (split + GEMM), for accounting. */
+uint64_t heal_launch_count(void);
+
+/* Library version: major * 10000 + minor * 100 + patch. */
+int heal_version(void);
+
+/* The cudaError_t (as int) of the most recent failing CUDA call made by this library, 0 if none. */
+int heal_last_cuda_error(void);
+
+/* Static, NUL-terminated description of a heal_status. */
+const char *heal_status_string(int status);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* HEAL_H_ */

@@ -1,0 +1,433 @@
+// heal_api.cu -- the C ABI of libheal.so (include/heal.h): argument validation, workspace,
+// TMA tensor-map encoding, kernel dispatch.  Every step of the path runs in the kernels of
+// heal_split.cuh / heal_gemm_umma.cuh; there is no CPU or library fallback.
+#include "../../include/heal.h"
+
+#include <cuda.h>
+#include <cudaTypedefs.h>
+#include <cuda_fp16.h>
+#include <cuda_runtime.h>
+
+#include <atomic>
+#include <mutex>
+
+#include "heal_gemm_umma.cuh"
+#include "heal_split.cuh"
+
+namespace {
+
+using namespace heal;
+
+std::atomic<int> g_last_cuda_error{0};
+std::atomic<uint64_t> g_launches{0};
+std::mutex g_mu;
+
+struct State {
+    bool init = false;
+    int init_status = HEAL_OK;
+    int device = -1;
+    int num_sms = 0;
+    int *diag = nullptr;
+    // workspace
+    void *user_ws = nullptr;
+    size_t user_ws_bytes = 0;
+    void *own_ws = nullptr;
+    size_t own_ws_bytes = 0;
+    // host-variant staging
+    void *stage = nullptr;
+    size_t stage_bytes = 0;
+    PFN_cuTensorMapEncodeTiled_v12000 encode = nullptr;
+};
+State g;
+
+inline int cuda_fail(cudaError_t e)
+{
+    g_last_cuda_error.store(static_cast<int>(e));
+    return HEAL_ERR_CUDA;
+}
+#define HEAL_CUDA(expr)                                  \
+    do {                                                 \
+        cudaError_t e__ = (expr);                        \
+        if (e__ != cudaSuccess) return cuda_fail(e__);   \
+    } while (0)
+
+int ensure_init()
+{
+    std::lock_guard<std::mutex> lk(g_mu);
+    if (g.init) return g.init_status;
+    g.init = true;
+    auto fail = [&](int st) { g.init_status = st; return st; };
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return fail(cuda_fail(e));
+    cudaDeviceProp prop;
+    e = cudaGetDeviceProperties(&prop, dev);
+    if (e != cudaSuccess) return fail(cuda_fail(e));
+    if (prop.major != 10) return fail(HEAL_ERR_UNSUPPORTED_DEVICE);
+    g.device = dev;
+    g.num_sms = prop.multiProcessorCount;
+    void *fn = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    e = cudaGetDriverEntryPointByVersion("cuTensorMapEncodeTiled", &fn, 12000, cudaEnableDefault, &qres);
+    if (e != cudaSuccess || qres != cudaDriverEntryPointSuccess || !fn)
+        return fail(cuda_fail(e != cudaSuccess ? e : cudaErrorUnknown));
+    g.encode = reinterpret_cast<PFN_cuTensorMapEncodeTiled_v12000>(fn);
+    e = cudaMalloc(&g.diag, 64);
+    if (e != cudaSuccess) return fail(cuda_fail(e));
+    e = cudaMemset(g.diag, 0, 64);
+    if (e != cudaSuccess) return fail(cuda_fail(e));
+    return HEAL_OK;
+}
+
+inline bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+inline int64_t round_up(int64_t x, int64_t m) { return (x + m - 1) / m * m; }
+
+// 2-D FP16 tensor map, 128-byte swizzle, out-of-bounds elements read as zero (K/M/N tails).
+//   inner/outer: extents in elements; ld: row pitch in elements; box: {inner, outer} elements.
+int encode_f16_2d(CUtensorMap *tm, const void *base, int64_t inner, int64_t outer, int64_t ld, uint32_t box_inner,
+                  uint32_t box_outer)
+{
+    cuuint64_t dims[2] = {static_cast<cuuint64_t>(inner), static_cast<cuuint64_t>(outer)};
+    cuuint64_t strides[1] = {static_cast<cuuint64_t>(ld) * 2};
+    cuuint32_t box[2] = {box_inner, box_outer};
+    cuuint32_t estr[2] = {1, 1};
+    CUresult r = g.encode(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 2, const_cast<void *>(base), dims, strides, box, estr,
+                          CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                          CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) {
+        g_last_cuda_error.store(static_cast<int>(cudaErrorInvalidValue));
+        return HEAL_ERR_CUDA;
+    }
+    return HEAL_OK;
+}
+
+}  // namespace
+
+namespace {
+
+// ---- step S launch --------------------------------------------------------------------------
+int launch_split(int64_t rows, int64_t cols, const float *X, int64_t ldx, __half *hi, __half *lo, int64_t ld,
+                 cudaStream_t stream)
+{
+    if (rows == 0 || cols == 0) return HEAL_OK;
+    const int64_t vecs = rows * ((cols + 7) / 8);
+    int64_t blocks = (vecs + 255) / 256;
+    const int64_t cap = static_cast<int64_t>(g.num_sms) * 16;      // grid-stride beyond 16 CTAs per SM
+    if (blocks > cap) blocks = cap;
+    heal_split_kernel<<<static_cast<unsigned>(blocks), 256, 0, stream>>>(X, ldx, rows, cols, hi, lo, ld);
+    g_launches.fetch_add(1);
+    HEAL_CUDA(cudaGetLastError());
+    return HEAL_OK;
+}
+
+// ---- steps G + E launch -----------------------------------------------------------------------
+template <class Cfg>
+int launch_gemm_cfg(int64_t M, int64_t N, int64_t K, const void *A_hi, const void *A_lo, int64_t lda, const void *B_hi,
+                    const void *B_lo, int64_t ldb, float *C, int64_t ldc, cudaStream_t stream)
+{
+    static bool attr_set = false;
+    auto kern = heal_gemm_umma_kernel<Cfg>;
+    if (!attr_set) {
+        HEAL_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::SMEM_BYTES));
+        attr_set = true;
+    }
+    CUtensorMap ta_hi, ta_lo, tb_hi, tb_lo;
+    int st = encode_f16_2d(&ta_hi, A_hi, K, M, lda, kBK, kBM);
+    if (st) return st;
+    if (Cfg::A_PLANES == 2) {
+        st = encode_f16_2d(&ta_lo, A_lo, K, M, lda, kBK, kBM);
+        if (st) return st;
+    } else {
+        ta_lo = ta_hi;
+    }
+    if (Cfg::B_MN) st = encode_f16_2d(&tb_hi, B_hi, N, K, ldb, 64, kBK);
+    else           st = encode_f16_2d(&tb_hi, B_hi, K, N, ldb, kBK, Cfg::BN);
+    if (st) return st;
+    if (Cfg::B_PLANES == 2) {
+        if (Cfg::B_MN) st = encode_f16_2d(&tb_lo, B_lo, N, K, ldb, 64, kBK);
+        else           st = encode_f16_2d(&tb_lo, B_lo, K, N, ldb, kBK, Cfg::BN);
+        if (st) return st;
+    } else {
+        tb_lo = tb_hi;
+    }
+    GemmArgs args;
+    args.C = C;
+    args.ldc = ldc;
+    args.M = static_cast<int>(M);
+    args.N = static_cast<int>(N);
+    args.K = static_cast<int>(K);
+    args.tiles_m = static_cast<int>((M + kBM - 1) / kBM);
+    args.tiles_n = static_cast<int>((N + Cfg::BN - 1) / Cfg::BN);
+    args.diag = g.diag;
+    const int64_t tiles = static_cast<int64_t>(args.tiles_m) * args.tiles_n;
+    const unsigned grid = static_cast<unsigned>(tiles < g.num_sms ? tiles : g.num_sms);
+    kern<<<grid, kGemmThreads, Cfg::SMEM_BYTES, stream>>>(ta_hi, ta_lo, tb_hi, tb_lo, args);
+    g_launches.fetch_add(1);
+    HEAL_CUDA(cudaGetLastError());
+    return HEAL_OK;
+}
+
+template <int BN, bool B_MN>
+int launch_gemm_np(int nprod, int64_t M, int64_t N, int64_t K, const void *A_hi, const void *A_lo, int64_t lda,
+                   const void *B_hi, const void *B_lo, int64_t ldb, float *C, int64_t ldc, cudaStream_t s)
+{
+    switch (nprod) {
+    case 1: return launch_gemm_cfg<GemmCfg<BN, 1, B_MN>>(M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, C, ldc, s);
+    case 2: return launch_gemm_cfg<GemmCfg<BN, 2, B_MN>>(M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, C, ldc, s);
+    case 3: return launch_gemm_cfg<GemmCfg<BN, 3, B_MN>>(M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, C, ldc, s);
+    case 4: return launch_gemm_cfg<GemmCfg<BN, 4, B_MN>>(M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, C, ldc, s);
+    }
+    return HEAL_ERR_UNSUPPORTED_MODE;
+}
+
+// Tile width: a function of N only (never of M), so the schedule cannot make results depend on M.
+template <bool B_MN>
+int launch_gemm_bn(int nprod, int64_t M, int64_t N, int64_t K, const void *A_hi, const void *A_lo, int64_t lda,
+                   const void *B_hi, const void *B_lo, int64_t ldb, float *C, int64_t ldc, cudaStream_t s)
+{
+    if (N <= 64) return launch_gemm_np<64, B_MN>(nprod, M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, C, ldc, s);
+    if (N <= 128) return launch_gemm_np<128, B_MN>(nprod, M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, C, ldc, s);
+    return launch_gemm_np<256, B_MN>(nprod, M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, C, ldc, s);
+}
+
+int validate_mode(uint32_t mode, int *nprod, bool *b_nk)
+{
+    if (mode & ~(HEAL_MODE_PRODUCTS_MASK | HEAL_B_NK)) return HEAL_ERR_UNSUPPORTED_MODE;
+    const uint32_t p = mode & HEAL_MODE_PRODUCTS_MASK;
+    if (p < 1 || p > 4) return HEAL_ERR_UNSUPPORTED_MODE;
+    *nprod = static_cast<int>(p);
+    *b_nk = (mode & HEAL_B_NK) != 0;
+    return HEAL_OK;
+}
+
+int presplit_impl(int64_t M, int64_t N, int64_t K, const void *A_hi, const void *A_lo, int64_t lda, const void *B_hi,
+                  const void *B_lo, int64_t ldb, void *C, int64_t ldc, int nprod, bool b_nk, cudaStream_t stream)
+{
+    if (K == 0) {
+        HEAL_CUDA(cudaMemset2DAsync(C, static_cast<size_t>(ldc) * 4, 0, static_cast<size_t>(N) * 4,
+                                    static_cast<size_t>(M), stream));
+        return HEAL_OK;
+    }
+    if (b_nk)
+        return launch_gemm_bn<false>(nprod, M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, static_cast<float *>(C), ldc, stream);
+    return launch_gemm_bn<true>(nprod, M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, static_cast<float *>(C), ldc, stream);
+}
+
+// workspace layout for heal_gemm: [A_hi][A_lo][B_hi][B_lo], each plane 256-byte aligned
+struct WsPlan {
+    int64_t lda_p, ldb_p;          // plane pitches (elements)
+    size_t a_plane, b_plane;       // bytes per plane (0 if not needed)
+    size_t total;
+};
+WsPlan plan_ws(int64_t M, int64_t N, int64_t K, int nprod, bool b_nk)
+{
+    WsPlan p;
+    p.lda_p = round_up(K, 8);
+    p.a_plane = static_cast<size_t>(round_up(M * p.lda_p * 2, 256));
+    if (nprod >= 3) {
+        const int64_t brows = b_nk ? N : K, bcols = b_nk ? K : N;
+        p.ldb_p = round_up(bcols, 8);
+        p.b_plane = static_cast<size_t>(round_up(brows * p.ldb_p * 2, 256));
+    } else {
+        p.ldb_p = 0;
+        p.b_plane = 0;
+    }
+    p.total = 2 * p.a_plane + 2 * p.b_plane;
+    return p;
+}
+
+int get_ws(size_t bytes, cudaStream_t stream, void **out)
+{
+    if (g.user_ws) {
+        if (bytes > g.user_ws_bytes) return HEAL_ERR_WORKSPACE;
+        *out = g.user_ws;
+        return HEAL_OK;
+    }
+    if (bytes > g.own_ws_bytes) {
+        if (g.own_ws) HEAL_CUDA(cudaFreeAsync(g.own_ws, stream));
+        g.own_ws = nullptr;
+        g.own_ws_bytes = 0;
+        HEAL_CUDA(cudaMallocAsync(&g.own_ws, bytes, stream));
+        g.own_ws_bytes = bytes;
+    }
+    *out = g.own_ws;
+    return HEAL_OK;
+}
+
+}  // namespace
+
+// =============================================== C ABI ===========================================
+extern "C" {
+
+int heal_version(void) { return 100; }
+
+int heal_last_cuda_error(void) { return g_last_cuda_error.load(); }
+
+uint64_t heal_launch_count(void) { return g_launches.load(); }
+
+const char *heal_status_string(int status)
+{
+    switch (status) {
+    case HEAL_OK: return "HEAL_OK";
+    case HEAL_ERR_INVALID_VALUE: return "HEAL_ERR_INVALID_VALUE: negative dimension or leading dimension too small";
+    case HEAL_ERR_NULL_POINTER: return "HEAL_ERR_NULL_POINTER: null matrix pointer for a non-empty problem";
+    case HEAL_ERR_MISALIGNED: return "HEAL_ERR_MISALIGNED: pointer or leading dimension not 16-byte aligned";
+    case HEAL_ERR_UNSUPPORTED_MODE: return "HEAL_ERR_UNSUPPORTED_MODE: unknown mode bits";
+    case HEAL_ERR_CUDA: return "HEAL_ERR_CUDA: a CUDA call failed (see heal_last_cuda_error)";
+    case HEAL_ERR_WORKSPACE: return "HEAL_ERR_WORKSPACE: supplied workspace too small";
+    case HEAL_ERR_UNSUPPORTED_DEVICE: return "HEAL_ERR_UNSUPPORTED_DEVICE: current device is not sm_100";
+    }
+    return "unknown heal_status";
+}
+
+size_t heal_workspace_size(int64_t M, int64_t N, int64_t K, uint32_t mode)
+{
+    int nprod;
+    bool b_nk;
+    if (validate_mode(mode, &nprod, &b_nk) || M < 0 || N < 0 || K < 0) return 0;
+    return plan_ws(M, N, K, nprod, b_nk).total;
+}
+
+int heal_set_workspace(void *ptr, size_t bytes)
+{
+    if (ptr && (reinterpret_cast<uintptr_t>(ptr) & 255u)) return HEAL_ERR_MISALIGNED;
+    std::lock_guard<std::mutex> lk(g_mu);
+    g.user_ws = ptr;
+    g.user_ws_bytes = ptr ? bytes : 0;
+    return HEAL_OK;
+}
+
+int heal_split(int64_t rows, int64_t cols, const void *X, int64_t ldx, void *hi, void *lo, int64_t ld, void *stream)
+{
+    if (rows < 0 || cols < 0 || ldx < cols || ld < cols) return HEAL_ERR_INVALID_VALUE;
+    if (rows == 0 || cols == 0) return HEAL_OK;
+    if (!X || !hi || !lo) return HEAL_ERR_NULL_POINTER;
+    if (!aligned16(X) || !aligned16(hi) || !aligned16(lo) || (ldx & 3) || (ld & 7)) return HEAL_ERR_MISALIGNED;
+    int st = ensure_init();
+    if (st) return st;
+    return launch_split(rows, cols, static_cast<const float *>(X), ldx, static_cast<__half *>(hi),
+                        static_cast<__half *>(lo), ld, static_cast<cudaStream_t>(stream));
+}
+
+int heal_gemm_presplit(int64_t M, int64_t N, int64_t K, const void *A_hi, const void *A_lo, int64_t lda,
+                       const void *B_hi, const void *B_lo, int64_t ldb, void *C, int64_t ldc, uint32_t mode,
+                       void *stream)
+{
+    int nprod;
+    bool b_nk;
+    int st = validate_mode(mode, &nprod, &b_nk);
+    if (st) return st;
+    if (M < 0 || N < 0 || K < 0) return HEAL_ERR_INVALID_VALUE;
+    if (M > 0x7fffff00 || N > 0x7fffff00 || K > 0x7fffff00) return HEAL_ERR_INVALID_VALUE;
+    if (lda < K || ldc < N || ldb < (b_nk ? K : N)) return HEAL_ERR_INVALID_VALUE;
+    if (M == 0 || N == 0) return HEAL_OK;
+    if (!C) return HEAL_ERR_NULL_POINTER;
+    if (K > 0) {
+        if (!A_hi || !B_hi) return HEAL_ERR_NULL_POINTER;
+        if (nprod >= 2 && !A_lo) return HEAL_ERR_NULL_POINTER;
+        if (nprod >= 3 && !B_lo) return HEAL_ERR_NULL_POINTER;
+        if (!aligned16(A_hi) || !aligned16(A_lo) || !aligned16(B_hi) || !aligned16(B_lo) || (lda & 7) || (ldb & 7))
+            return HEAL_ERR_MISALIGNED;
+    }
+    if (!aligned16(C) || (ldc & 3)) return HEAL_ERR_MISALIGNED;
+    st = ensure_init();
+    if (st) return st;
+    return presplit_impl(M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, C, ldc, nprod, b_nk,
+                         static_cast<cudaStream_t>(stream));
+}
+
+int heal_gemm(int64_t M, int64_t N, int64_t K, const void *A, int64_t lda, const void *B, int64_t ldb, void *C,
+              int64_t ldc, uint32_t mode, void *stream_)
+{
+    int nprod;
+    bool b_nk;
+    int st = validate_mode(mode, &nprod, &b_nk);
+    if (st) return st;
+    if (M < 0 || N < 0 || K < 0) return HEAL_ERR_INVALID_VALUE;
+    if (M > 0x7fffff00 || N > 0x7fffff00 || K > 0x7fffff00) return HEAL_ERR_INVALID_VALUE;
+    if (lda < K || ldc < N || ldb < (b_nk ? K : N)) return HEAL_ERR_INVALID_VALUE;
+    if (M == 0 || N == 0) return HEAL_OK;
+    if (!C) return HEAL_ERR_NULL_POINTER;
+    const bool b_f32 = nprod >= 3;
+    if (K > 0) {
+        if (!A || !B) return HEAL_ERR_NULL_POINTER;
+        if (!aligned16(A) || !aligned16(B) || (lda & 3) || (ldb & (b_f32 ? 3 : 7))) return HEAL_ERR_MISALIGNED;
+    }
+    if (!aligned16(C) || (ldc & 3)) return HEAL_ERR_MISALIGNED;
+    st = ensure_init();
+    if (st) return st;
+    cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+    if (K == 0) return presplit_impl(M, N, K, nullptr, nullptr, lda, nullptr, nullptr, ldb, C, ldc, nprod, b_nk, stream);
+
+    std::lock_guard<std::mutex> lk(g_mu);
+    const WsPlan p = plan_ws(M, N, K, nprod, b_nk);
+    void *ws = nullptr;
+    st = get_ws(p.total, stream, &ws);
+    if (st) return st;
+    char *w = static_cast<char *>(ws);
+    __half *a_hi = reinterpret_cast<__half *>(w);
+    __half *a_lo = reinterpret_cast<__half *>(w + p.a_plane);
+    // step S on the activations; in 1P only the hi plane is consumed
+    st = launch_split(M, K, static_cast<const float *>(A), lda, a_hi, a_lo, p.lda_p, stream);
+    if (st) return st;
+    const void *b_hi = B, *b_lo = nullptr;
+    int64_t ldb_eff = ldb;
+    if (b_f32) {
+        __half *bh = reinterpret_cast<__half *>(w + 2 * p.a_plane);
+        __half *bl = reinterpret_cast<__half *>(w + 2 * p.a_plane + p.b_plane);
+        const int64_t brows = b_nk ? N : K, bcols = b_nk ? K : N;
+        st = launch_split(brows, bcols, static_cast<const float *>(B), ldb, bh, bl, p.ldb_p, stream);
+        if (st) return st;
+        b_hi = bh;
+        b_lo = bl;
+        ldb_eff = p.ldb_p;
+    }
+    return presplit_impl(M, N, K, a_hi, a_lo, p.lda_p, b_hi, b_lo, ldb_eff, C, ldc, nprod, b_nk, stream);
+}
+
+int heal_gemm_host(int64_t M, int64_t N, int64_t K, const void *A_host, int64_t lda, const void *B_host, int64_t ldb,
+                   void *C_host, int64_t ldc, uint32_t mode, void *stream_)
+{
+    int nprod;
+    bool b_nk;
+    int st = validate_mode(mode, &nprod, &b_nk);
+    if (st) return st;
+    if (M < 0 || N < 0 || K < 0) return HEAL_ERR_INVALID_VALUE;
+    if (lda < K || ldc < N || ldb < (b_nk ? K : N)) return HEAL_ERR_INVALID_VALUE;
+    if (M == 0 || N == 0) return HEAL_OK;
+    if (!C_host || (K > 0 && (!A_host || !B_host))) return HEAL_ERR_NULL_POINTER;
+    st = ensure_init();
+    if (st) return st;
+    cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+    const size_t b_es = nprod >= 3 ? 4 : 2;
+    const int64_t brows = b_nk ? N : K, bcols = b_nk ? K : N;
+    // dense device copies with 16-byte-aligned pitches
+    const int64_t dlda = round_up(K > 0 ? K : 1, 8), dldb = round_up(bcols > 0 ? bcols : 1, 8), dldc = round_up(N, 4);
+    const size_t a_bytes = static_cast<size_t>(round_up(M * dlda * 4, 256));
+    const size_t b_bytes = static_cast<size_t>(round_up(brows * dldb * static_cast<int64_t>(b_es), 256));
+    const size_t c_bytes = static_cast<size_t>(round_up(M * dldc * 4, 256));
+    {
+        std::lock_guard<std::mutex> lk(g_mu);
+        const size_t need = a_bytes + b_bytes + c_bytes;
+        if (need > g.stage_bytes) {
+            if (g.stage) HEAL_CUDA(cudaFree(g.stage));
+            g.stage = nullptr;
+            g.stage_bytes = 0;
+            HEAL_CUDA(cudaMalloc(&g.stage, need));
+            g.stage_bytes = need;
+        }
+    }
+    char *dA = static_cast<char *>(g.stage), *dB = dA + a_bytes, *dC = dB + b_bytes;
+    if (K > 0) {
+        HEAL_CUDA(cudaMemcpy2DAsync(dA, dlda * 4, A_host, lda * 4, K * 4, M, cudaMemcpyHostToDevice, stream));
+        HEAL_CUDA(cudaMemcpy2DAsync(dB, dldb * b_es, B_host, ldb * b_es, bcols * b_es, brows, cudaMemcpyHostToDevice,
+                                    stream));
+    }
+    st = heal_gemm(M, N, K, dA, dlda, dB, dldb, dC, dldc, mode, stream_);
+    if (st) return st;
+    HEAL_CUDA(cudaMemcpy2DAsync(C_host, ldc * 4, dC, dldc * 4, N * 4, M, cudaMemcpyDeviceToHost, stream));
+    HEAL_CUDA(cudaStreamSynchronize(stream));
+    return HEAL_OK;
+}
+
+}  // extern "C"
