@@ -1,0 +1,65 @@
+"""CPU-only checks of the boundary: libheal.so builds for sm_100a without a GPU, loads, exports
+every symbol include/heal.h declares, and its host-side validation answers without a device."""
+import ctypes
+import os
+import re
+
+import numpy as np
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    from paper_2606_21023_b200 import build, binding
+    build.build()
+    return binding.lib()
+
+
+def test_exports_every_declared_symbol(lib):
+    hdr = open(os.path.join(ROOT, "include", "heal.h")).read()
+    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+    names = set(re.findall(r"\b(heal_[a-z_]+)\s*\(", hdr))
+    assert {"heal_gemm", "heal_split", "heal_gemm_presplit", "heal_gemm_host", "heal_workspace_size",
+            "heal_set_workspace", "heal_version", "heal_last_cuda_error", "heal_status_string",
+            "heal_launch_count"} <= names
+    for n in names:
+        assert hasattr(lib, n), n
+
+
+def test_host_side_validation_without_device(lib):
+    from paper_2606_21023_b200 import binding as hb
+    assert hb.version() >= 100
+    raw = hb.heal_gemm_raw
+    assert raw(-1, 1, 1, None, 1, None, 8, None, 4, 2) == 1          # negative dimension
+    assert raw(4, 4, 8, None, 4, None, 8, None, 4, 2) == 1           # lda < K
+    assert raw(0, 4, 8, None, 8, None, 8, None, 4, 2) == 0           # empty: no-op
+    assert raw(4, 4, 8, None, 8, None, 8, None, 4, 2) == 2           # null pointer
+    assert raw(4, 4, 8, 16, 8, 16, 8, 16, 4, 9) == 4                 # unknown product count
+    assert raw(4, 4, 8, 16, 8, 16, 8, 16, 4, 0x22) == 4              # unknown flag bit
+    assert raw(4, 4, 8, 20, 8, 16, 8, 16, 4, 2) == 3                 # misaligned A
+    assert "MISALIGNED" in hb.status_string(3) and hb.status_string(0) == "HEAL_OK"
+    # workspace = two FP16 planes of A (256-byte rounded); plus two planes of B in 3P
+    assert hb.workspace_size(2048, 14336, 4096, 2) == 2 * 2048 * 4096 * 2
+    assert hb.workspace_size(64, 256, 256, 3) == 2 * 64 * 256 * 2 + 2 * 256 * 256 * 2
+    assert hb.workspace_size(1, 8, 4, 2) == 2 * 256
+
+
+def test_no_cpu_fallback_when_library_missing(monkeypatch):
+    from paper_2606_21023_b200 import binding as hb
+    monkeypatch.setattr(hb, "_lib", None)
+    monkeypatch.setattr(hb, "LIB_PATH", "/nonexistent/libheal.so")
+    with pytest.raises(hb.HealError):
+        hb.lib()
+
+
+def test_product_does_not_import_oracle():
+    for dirpath, _, files in os.walk(os.path.join(ROOT, "paper_2606_21023_b200")):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".c", ".h")):
+                src = open(os.path.join(dirpath, f)).read()
+                assert "import oracle" not in src and "from oracle" not in src and "heal_oracle" not in src, f
+    osrc = open(os.path.join(ROOT, "oracle", "__init__.py")).read() + open(os.path.join(ROOT, "oracle", "heal_oracle.c")).read()
+    assert "import paper_2606_21023_b200" not in osrc and "from paper_2606_21023_b200" not in osrc
+    assert "#include <cuda" not in osrc and "import torch" not in osrc

@@ -1,0 +1,381 @@
+"""GPU parity tests (-m gpu): the CUDA path behind the C ABI (paper_2606_21023_b200.binding ->
+libheal.so) against the CPU oracle (oracle/), element by element on the same seeded inputs.
+
+Bars:
+  * step S (split) and the exact-regime GEMMs: bit-exact.
+  * rounded regime: normwise e = ||C-Cref||_F/(||A||_F ||B||_F) <= 2e-6 vs O1 (BASELINE.json
+    north_star), and element-wise |C - O3| <= (32 n_prod + n_seg + 1) 2^-23 sum_k |a||b| vs the exact
+    evaluation O3 of the products the mode keeps (one possible rounding per tensor-core accumulate,
+    32 n_prod of them per 512-long K segment, plus one per segment add and the final value).
+  * reproducibility: bit-identical across runs, M, row position, padding, streams.
+"""
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+GATE = 2e-6
+
+
+@pytest.fixture(scope="module")
+def hb():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_2606_21023_b200 import binding
+    binding.lib()
+    return binding
+
+
+def dev(x):
+    return torch.from_numpy(np.ascontiguousarray(x)).cuda()
+
+
+def padded(x, pad):
+    """Same matrix inside a buffer with a larger leading dimension."""
+    buf = np.zeros((x.shape[0], x.shape[1] + pad), x.dtype)
+    buf[:, :x.shape[1]] = x
+    return buf[:, :x.shape[1]]
+
+
+def dev_padded(x, pad):
+    buf = torch.zeros((x.shape[0], x.shape[1] + pad), dtype=torch.from_numpy(x[:1, :1].copy()).dtype, device="cuda")
+    buf[:, :x.shape[1]] = torch.from_numpy(np.ascontiguousarray(x)).cuda()
+    return buf[:, :x.shape[1]]
+
+
+def run(hb, A, B, mode, **kw):
+    C = hb.heal_gemm(dev(A), dev(B), mode, **kw)
+    torch.cuda.synchronize()
+    return C.cpu().numpy()
+
+
+def elementwise_bound(A, B, K, nprod, b_nk=False):
+    n_seg = (K + 511) // 512
+    Bd = np.abs(B.astype(np.float64))
+    absprod = np.abs(A.astype(np.float64)) @ (Bd.T if b_nk else Bd)
+    return (32 * nprod + n_seg + 1) * 2.0 ** -23 * absprod
+
+
+# --------------------------------------------------------------------------------- step S
+
+@pytest.mark.parametrize("rows,cols,pad", [(1, 8, 0), (3, 100, 4), (64, 256, 0), (257, 4096, 8), (5, 7, 1)])
+def test_split_bit_exact(hb, oracle, inputs, rows, cols, pad):
+    X = inputs.activations(rows, cols, seed=rows, outliers=cols >= 1000)
+    X[0, 0] = 0.0
+    if cols >= 8:
+        X[0, 1:8] = [-0.0, 65504.0, 2.0 ** -24, 2.0 ** -25, 1 + 2.0 ** -11, 1 + 3 * 2.0 ** -11, -3e-6]
+    ldx = (cols + pad + 3) // 4 * 4
+    Xd = torch.zeros((rows, ldx), device="cuda")
+    Xd[:, :cols] = dev(X)
+    hi, lo = hb.heal_split(Xd[:, :cols])
+    torch.cuda.synchronize()
+    ohi, olo = oracle.split(X)
+    assert np.array_equal(hi.cpu().numpy().view(np.uint16), ohi)
+    assert np.array_equal(lo.cpu().numpy().view(np.uint16), olo)
+
+
+def test_split_wide_range_bit_exact(hb, oracle):
+    rng = np.random.default_rng(3)
+    bits = rng.integers(0, 2 ** 32, size=1 << 20, dtype=np.uint64).astype(np.uint32).view(np.float32)
+    x = bits[np.isfinite(bits) & (np.abs(bits) <= 65504)]
+    x = np.ascontiguousarray(x[: x.size // 1024 * 1024].reshape(-1, 1024))
+    hi, lo = hb.heal_split(dev(x))
+    ohi, olo = oracle.split(x)
+    assert np.array_equal(hi.cpu().numpy().view(np.uint16), ohi)
+    assert np.array_equal(lo.cpu().numpy().view(np.uint16), olo)
+
+
+# --------------------------------------------------------------------------------- exact regime
+
+SHAPES_EXACT = [(1, 8, 16), (128, 64, 64), (127, 72, 72), (129, 264, 520), (64, 256, 256), (300, 520, 1032),
+                (256, 512, 1536), (130, 136, 2056)]
+
+
+@pytest.mark.parametrize("M,N,K", SHAPES_EXACT)
+@pytest.mark.parametrize("nprod", [1, 2, 3, 4])
+@pytest.mark.parametrize("b_nk", [False, True])
+def test_integer_exact(hb, inputs, M, N, K, nprod, b_nk):
+    """Entries in [-8, 8]: hi = x, lo = 0, every partial sum exact => C == integer GEMM bit for bit,
+    whatever the tensor core's accumulate rounding.  Sizes straddle tile edges (128 rows, 64/128/256
+    columns, 64-wide k-tiles, 512-long segments)."""
+    A = inputs.integers(M, K, -8, 8, seed=M + K)
+    B = inputs.integers(K, N, -8, 8, seed=N + K + 1)
+    want = (A.astype(np.int64) @ B.astype(np.int64)).astype(np.float32)
+    Bx = B if nprod >= 3 else B.astype(np.float16)
+    Bx = np.ascontiguousarray(Bx.T) if b_nk else Bx
+    got = run(hb, A, Bx, nprod | (hb.B_NK if b_nk else 0))
+    assert np.array_equal(got, want)
+
+
+@pytest.mark.parametrize("b_nk", [False, True])
+def test_lo_plane_exact(hb, inputs, b_nk):
+    """Integers in [2049, 8191] are not FP16 numbers: lo != 0 and hi + lo = a exactly; with B in
+    {-1,0,1} and K <= 1024 every partial sum is exact, so 2P/3P must equal the integer GEMM."""
+    M, N, K = 200, 264, 1024
+    A = (inputs.integers(M, K, 2049, 8191, seed=3) * (inputs.integers(M, K, 0, 1, seed=4) * 2 - 1)).astype(np.float32)
+    B = inputs.integers(K, N, -1, 1, seed=5)
+    want = (A.astype(np.int64) @ B.astype(np.int64)).astype(np.float32)
+    flag = hb.B_NK if b_nk else 0
+    lay = (lambda x: np.ascontiguousarray(x.T)) if b_nk else (lambda x: x)
+    assert np.array_equal(run(hb, A, lay(B.astype(np.float16)), 2 | flag), want)
+    assert np.array_equal(run(hb, A, lay(B), 3 | flag), want)                     # lo only in A
+    assert not np.array_equal(run(hb, A, lay(B.astype(np.float16)), 1 | flag), want)
+    # lo only in B: swap roles
+    A2 = np.ascontiguousarray(B.T[:N])            # (N, K) small ints
+    B2 = np.ascontiguousarray(A.T)                # (K, M) big ints
+    got = run(hb, A2, lay(B2), 3 | flag)
+    assert np.array_equal(got, want.T)
+
+
+def test_dropped_lo_lo_term_exact(hb, inputs):
+    M, N, K = 130, 72, 512
+    vals = np.array([2049, -2049, 4098, -4098, 0], np.float32)
+    A = vals[inputs.integers(M, K, 0, 4, seed=6).astype(np.int64)]
+    B = vals[inputs.integers(K, N, 0, 4, seed=7).astype(np.int64)]
+    full = A.astype(np.int64) @ B.astype(np.int64)
+    lo = lambda X: np.sign(X) * np.where(np.abs(X) == 2049, 1, np.where(np.abs(X) == 4098, 2, 0))
+    dropped = lo(A).astype(np.int64) @ lo(B).astype(np.int64)
+    # every partial sum of the kept products has the form 2^22 n1 + 2^11 n2 and fits 24 bits: exact.
+    # (With the lo.lo term added -- mode 4P -- sums like 2^24 + 1 are no longer FP32 numbers.)
+    assert np.array_equal(run(hb, A, B, 3), (full - dropped).astype(np.float32))
+
+
+@pytest.mark.parametrize("b_nk", [False, True])
+def test_one_hot_indexing(hb, b_nk):
+    """A = one-hot rows selecting k = f(i): C[i,:] must be row f(i) of B -- every (tile, k-slice) index."""
+    M, N, K = 260, 328, 1160
+    A = np.zeros((M, K), np.float32)
+    sel = (np.arange(M) * 37 + 11) % K
+    A[np.arange(M), sel] = 1.0
+    B = ((np.arange(K)[:, None] * 3 + np.arange(N)[None, :]) % 2039).astype(np.float16)   # < 2048: exact in FP16
+    Bx = np.ascontiguousarray(B.T) if b_nk else B
+    got = run(hb, A, Bx, 2 | (hb.B_NK if b_nk else 0))
+    assert np.array_equal(got, B[sel].astype(np.float32))
+
+
+# --------------------------------------------------------------------------------- rounded regime
+
+def test_config0_single_gemm(hb, oracle, inputs):
+    """BASELINE.json configs[0]: M=64 N=256 K=256, A and B FP32 N(0,1) seed 0, three products."""
+    A = inputs.activations(64, 256, seed=0)
+    B = inputs.weights_f32(256, 256, seed=0, dist="normal")
+    got = run(hb, A, B, 3)
+    ref = oracle.gemm_f64(A, B)
+    assert oracle.normwise_error(got, ref, A, B) <= GATE
+    assert np.all(np.abs(got - oracle.gemm_split(A, B, 3)) <= elementwise_bound(A, B, 256, 3))
+    # sampled values stored by tests/golden/make_golden.py (oracle only)
+    gold = np.loadtxt(__import__("os").path.join(__import__("os").path.dirname(__file__), "golden", "config0_oracle_samples.txt"))
+    for i, j, v in gold:
+        assert abs(got[int(i), int(j)] - v) <= 1e-5 * max(1.0, abs(v))
+    # contrast: one product (plain FP16 cast) is far worse, four products no better than three
+    e1 = oracle.normwise_error(run(hb, A, B.astype(np.float16), 1), ref, A, B)
+    e3 = oracle.normwise_error(got, ref, A, B)
+    assert e1 > 20 * e3
+
+
+@pytest.mark.parametrize("M,N,K,nprod,b_nk", [(300, 520, 4096, 2, False), (300, 520, 4096, 3, False),
+                                              (77, 264, 4096, 2, True), (77, 264, 1000, 3, True),
+                                              (200, 1032, 8192, 3, False), (130, 136, 14336, 2, False)])
+def test_rounded_regime(hb, oracle, inputs, M, N, K, nprod, b_nk):
+    A = inputs.activations(M, K, seed=1, outliers=True)
+    B = inputs.weights_f32(K, N, seed=1, nk=b_nk) if nprod >= 3 else inputs.weights_f16(K, N, seed=1, nk=b_nk)
+    B = np.ascontiguousarray(B)
+    got = run(hb, A, B, nprod | (hb.B_NK if b_nk else 0))
+    ref = oracle.gemm_f64(A, B, b_nk=b_nk)
+    e = oracle.normwise_error(got, ref, A, B)
+    assert e <= GATE and e <= 2e-7, e
+    o3 = oracle.gemm_split(A, B, nprod, b_nk=b_nk)
+    assert np.all(np.abs(got - o3) <= elementwise_bound(A, B, K, nprod, b_nk))
+
+
+def test_config1_decode(hb, oracle, inputs):
+    """configs[1]: M in {1, 8, 32} x K=4096 with outlier channels, FP16 W 4096x4096, two products.
+    Shared rows must be bit-identical across M (activations are row prefixes of one another)."""
+    W = inputs.weights_f16(4096, 4096, seed=0)
+    Wd = dev(W)
+    outs = {}
+    for M in (1, 8, 32):
+        A = inputs.activations(M, 4096, seed=0, outliers=True)
+        C = hb.heal_gemm(dev(A), Wd, 2).cpu().numpy()
+        ref = oracle.gemm_f64(A, W)
+        assert oracle.normwise_error(C, ref, A, W) <= GATE
+        assert np.all(np.abs(C - oracle.gemm_split(A, W, 2)) <= elementwise_bound(A, W, 4096, 2))
+        outs[M] = C
+    assert np.array_equal(outs[1], outs[32][:1]) and np.array_equal(outs[8], outs[32][:8])
+
+
+@pytest.mark.parametrize("K,N", [(4096, 14336), (14336, 4096)])
+def test_config2_mlp_sampled(hb, oracle, inputs, K, N):
+    """configs[2] at full size, in the launch configuration bench.py times; oracle on sampled rows."""
+    M = 2048
+    A = inputs.activations(M, K, seed=0, outliers=True)
+    W = inputs.weights_f16(K, N, seed=0)
+    C = hb.heal_gemm(dev(A), dev(W), 2).cpu().numpy()
+    rows = [0, 1, 127, 128, 1000, 1023, 1024, 2047]
+    ref = oracle.gemm_f64(A, W, rows=rows)
+    e = oracle.normwise_error(C, ref, A, W, rows=rows)
+    assert e <= GATE, e
+    o3 = oracle.gemm_split(A, W, 2, rows=rows)
+    assert np.all(np.abs(C[rows] - o3) <= elementwise_bound(A[rows], W, K, 2))
+    # the same rows submitted as a small-M problem give the same bits
+    small = hb.heal_gemm(dev(A[rows]), dev(W), 2).cpu().numpy()
+    assert np.array_equal(small, C[rows])
+
+
+@pytest.mark.parametrize("n", [1024, 2048, 8192])
+def test_config3_square_sampled(hb, oracle, inputs, n):
+    A = inputs.activations(n, n, seed=0, dist="uniform")
+    B = inputs.weights_f32(n, n, seed=0, dist="uniform")
+    C = hb.heal_gemm(dev(A), dev(B), 3).cpu().numpy()
+    rows = sorted({0, 127, 128, n - 1} | set(np.random.default_rng(0).integers(0, n, 12).tolist()))
+    ref = oracle.gemm_f64(A, B, rows=rows)
+    e = oracle.normwise_error(C, ref, A, B, rows=rows)
+    assert e <= GATE, e
+    # compensation must beat the plain FP16 GEMM on the same inputs by > 4x (A13)
+    C1 = hb.heal_gemm(dev(A), dev(B.astype(np.float16)), 1).cpu().numpy()
+    e1 = oracle.normwise_error(C1, ref, A, B, rows=rows)
+    assert e <= 0.25 * e1, (e, e1)
+
+
+def test_config4_lm_head(hb, oracle, inputs):
+    """configs[4]: hidden M in {1, 64, 512} x 4096, FP16 W 4096x128256; top-1 per row equals the
+    oracle's (rule A8 for near ties) and shared rows are bit-identical across M."""
+    K, N = 4096, 128256
+    W = inputs.weights_f16(K, N, seed=0)
+    Wd = dev(W)
+    A = inputs.activations(512, K, seed=0)
+    outs = {M: hb.heal_gemm(dev(A[:M]), Wd, 2).cpu().numpy() for M in (1, 64, 512)}
+    assert np.array_equal(outs[1], outs[512][:1]) and np.array_equal(outs[64], outs[512][:64])
+    rows = [0, 1, 63, 64, 300, 511]
+    ref = oracle.gemm_f64(A, W, rows=rows)
+    C = outs[512]
+    assert oracle.normwise_error(C, ref, A, W, rows=rows) <= GATE
+    for r, i in enumerate(rows):
+        top = int(np.argmax(ref[r]))
+        srt = np.sort(ref[r])
+        gap = srt[-1] - srt[-2]
+        err = np.abs(C[i] - ref[r]).max()
+        if gap > 4 * err:
+            assert int(np.argmax(C[i])) == top
+        else:                                      # ambiguous row: either of the two leaders
+            assert ref[r][int(np.argmax(C[i]))] >= srt[-2]
+
+
+# --------------------------------------------------------------------------------- reproducibility
+
+def test_bitwise_reproducible_runs_and_streams(hb, inputs):
+    A = dev(inputs.activations(300, 4096, seed=2, outliers=True))
+    W = dev(inputs.weights_f16(4096, 520, seed=2))
+    first = hb.heal_gemm(A, W, 2).clone()
+    for _ in range(20):
+        assert torch.equal(hb.heal_gemm(A, W, 2), first)
+    # interleave another shape (workspace reuse), then a side stream
+    hb.heal_gemm(dev(inputs.activations(64, 256, seed=0)), dev(inputs.weights_f32(256, 256, seed=0)), 3)
+    s = torch.cuda.Stream()
+    torch.cuda.synchronize()
+    with torch.cuda.stream(s):
+        again = hb.heal_gemm(A, W, 2)
+    s.synchronize()
+    assert torch.equal(again, first)
+
+
+def test_bitwise_across_m_row_position_and_padding(hb, inputs):
+    K, N = 4096, 520
+    A = inputs.activations(700, K, seed=3, outliers=True)
+    W = inputs.weights_f16(K, N, seed=3)
+    Wd = dev(W)
+    full = hb.heal_gemm(dev(A), Wd, 2).cpu().numpy()
+    for M in (1, 8, 32, 64, 129, 512):
+        assert np.array_equal(hb.heal_gemm(dev(A[:M]), Wd, 2).cpu().numpy(), full[:M])
+    # rows 300..363 submitted at row offset 0
+    assert np.array_equal(hb.heal_gemm(dev(A[300:364]), Wd, 2).cpu().numpy(), full[300:364])
+    # padded leading dimensions for A, W and C
+    Ap, Wp = dev_padded(A, 12), dev_padded(W, 24)
+    Cp = torch.full((700, N + 4), 7.0, device="cuda")
+    hb.heal_gemm(Ap, Wp, 2, C=Cp[:, :N])
+    assert np.array_equal(Cp[:, :N].cpu().numpy(), full)
+    assert torch.all(Cp[:, N:] == 7.0)                     # padding untouched
+    # the N x K storage of the same W gives the same bits
+    Wnk = dev(np.ascontiguousarray(W.T))
+    assert np.array_equal(hb.heal_gemm(dev(A), Wnk, 2 | hb.B_NK).cpu().numpy(), full)
+
+
+def test_presplit_and_host_variants_match(hb, inputs):
+    A = inputs.activations(150, 1024, seed=4)
+    B = inputs.weights_f32(1024, 264, seed=4)
+    Ad, Bd = dev(A), dev(B)
+    C = hb.heal_gemm(Ad, Bd, 3)
+    ah, al = hb.heal_split(Ad)
+    bh, bl = hb.heal_split(Bd)
+    assert torch.equal(hb.heal_gemm_presplit(ah, al, bh, bl, 3), C)
+    Ch = hb.heal_gemm_host(torch.from_numpy(A).pin_memory(), torch.from_numpy(B).pin_memory(), 3)
+    assert torch.equal(Ch, C.cpu())
+
+
+# --------------------------------------------------------------------------------- edges / contract
+
+def test_empty_and_k0(hb):
+    A = torch.zeros((0, 64), device="cuda")
+    W = torch.zeros((64, 16), dtype=torch.float16, device="cuda")
+    assert hb.heal_gemm(A, W, 2).shape == (0, 16)
+    C = torch.full((5, 16), 3.0, device="cuda")
+    hb.heal_gemm(torch.zeros((5, 0), device="cuda"), torch.zeros((0, 16), dtype=torch.float16, device="cuda"), 2, C=C)
+    assert torch.all(C == 0)
+
+
+def test_error_codes(hb):
+    A = torch.zeros((8, 64), device="cuda")
+    W = torch.zeros((64, 16), dtype=torch.float16, device="cuda")
+    C = torch.zeros((8, 16), device="cuda")
+    a, w, c = A.data_ptr(), W.data_ptr(), C.data_ptr()
+    raw = hb.heal_gemm_raw
+    assert raw(-1, 16, 64, a, 64, w, 16, c, 16, 2) == 1
+    assert raw(8, 16, 64, a, 32, w, 16, c, 16, 2) == 1                 # lda < K
+    assert raw(8, 16, 64, None, 64, w, 16, c, 16, 2) == 2
+    assert raw(8, 16, 64, a + 4, 64, w, 16, c, 16, 2) == 3
+    assert raw(8, 16, 64, a, 66, w, 16, c, 16, 2) == 3                 # lda % 4
+    assert raw(8, 16, 64, a, 64, w, 20, c, 16, 2) == 3                 # ldb % 8 (FP16)
+    assert raw(8, 16, 64, a, 64, w, 16, c, 16, 0) == 4
+    assert raw(8, 16, 64, a, 64, w, 16, c, 16, 0x102) == 4
+    assert raw(8, 16, 64, a, 64, w, 16, c, 16, 2) == 0
+    ws = torch.zeros(256, dtype=torch.uint8, device="cuda")
+    hb.set_workspace(ws)
+    assert raw(8, 16, 64, a, 64, w, 16, c, 16, 2) == 6                 # supplied workspace too small
+    big = torch.zeros(hb.workspace_size(8, 16, 64, 2), dtype=torch.uint8, device="cuda")
+    hb.set_workspace(big)
+    assert raw(8, 16, 64, a, 64, w, 16, c, 16, 2) == 0
+    hb.set_workspace(None)
+    torch.cuda.synchronize()
+
+
+def test_nonfinite_propagation_and_subnormals(hb):
+    A = torch.ones((4, 64), device="cuda")
+    A[1, 3] = float("nan")
+    A[2, 5] = 1e6                                       # > 65504: hi overflows to Inf
+    W = torch.ones((64, 16), dtype=torch.float16, device="cuda")
+    C = hb.heal_gemm(A, W, 2).cpu()
+    assert torch.all(C[0] == 64) and torch.all(C[3] == 64)
+    assert torch.all(torch.isnan(C[1])) and not torch.all(torch.isfinite(C[2]))
+    # FP16 subnormal operands are honoured by the tensor core: (2^-24) * 1024 = 2^-14
+    A = torch.zeros((1, 64), device="cuda")
+    A[0, 0] = 1024.0
+    W = torch.zeros((64, 8), dtype=torch.float16, device="cuda")
+    W[0, :] = 2.0 ** -24
+    assert torch.all(hb.heal_gemm(A, W, 2).cpu() == 2.0 ** -14)
+
+
+def test_segment_order_is_fp32_rn_ascending(hb):
+    """Segments of 512 are added in FP32 round-to-nearest, ascending: with per-segment sums
+    s0 = 2^24, s1 = 1, s2 = 1 the result is fl(fl(2^24 + 1) + 1) = 2^24 (a descending or pairwise
+    order would give 2^24 + 2)."""
+    K = 1536
+    A = torch.zeros((1, K), device="cuda")
+    W = torch.ones((K, 8), dtype=torch.float16, device="cuda")
+    A[0, 0] = 4096.0
+    W[0, :] = 4096.0
+    A[0, 512] = 1.0
+    A[0, 1024] = 1.0
+    assert torch.all(hb.heal_gemm(A, W, 2).cpu() == 2.0 ** 24)
+    A[0, 1025] = 1.0          # s2 = 2: fl(2^24 + 2) is exact
+    assert torch.all(hb.heal_gemm(A, W, 2).cpu() == 2.0 ** 24 + 2)
