@@ -20,11 +20,7 @@
 namespace heal {
 
 constexpr int kBM = 128;          // UMMA M (rows of A per tile)
-constexpr int kBK = 64;           // k-tile: 64 FP16 = 128 bytes = one 128B-swizzle row
-constexpr int kKSeg = 512;        // HEAL_K_SEGMENT
-constexpr int kTilesPerSeg = kKSeg / kBK;
 constexpr int kGemmThreads = 384;
-constexpr int kSmemLimit = 227 * 1024;
 
 template <int BN_, int NPROD_, bool B_MN_>
 struct GemmCfg {
@@ -163,10 +159,10 @@ heal_gemm_umma_kernel(const __grid_constant__ CUtensorMap tm_a_hi, const __grid_
                         mbar_wait(full_bar(stage), phase, args.diag, 200 + stage);
                         tc_fence_after();
                         const uint32_t sb = smem_base + stage * Cfg::STAGE_BYTES;
-                        const uint64_t a_hi = adesc0 | (sb >> 4);
-                        const uint64_t a_lo = adesc0 | ((sb + Cfg::A_TILE) >> 4);
-                        const uint64_t b_hi = bdesc0 | ((sb + Cfg::A_PLANES * Cfg::A_TILE) >> 4);
-                        const uint64_t b_lo = bdesc0 | ((sb + Cfg::A_PLANES * Cfg::A_TILE + Cfg::B_TILE) >> 4);
+                        const uint64_t a_hi = adesc0 | desc_addr(sb);
+                        const uint64_t a_lo = adesc0 | desc_addr(sb + Cfg::A_TILE);
+                        const uint64_t b_hi = bdesc0 | desc_addr(sb + Cfg::A_PLANES * Cfg::A_TILE);
+                        const uint64_t b_lo = bdesc0 | desc_addr(sb + Cfg::A_PLANES * Cfg::A_TILE + Cfg::B_TILE);
 #pragma unroll
                         for (int j = 0; j < kBK / 16; ++j) {
                             const uint64_t ao = static_cast<uint64_t>(j * a_step), bo = static_cast<uint64_t>(j * b_step);

@@ -7,6 +7,12 @@
 
 namespace heal {
 
+// ---- constants shared by the GEMM kernels ----------------------------------------------------
+constexpr int kBK = 64;                     // k-tile: 64 FP16 = 128 bytes = one 128B-swizzle row
+constexpr int kKSeg = 512;                  // HEAL_K_SEGMENT (include/heal.h): the reduction-order contract
+constexpr int kTilesPerSeg = kKSeg / kBK;
+constexpr int kSmemLimit = 227 * 1024;      // dynamic shared memory per CTA on sm_100
+
 __device__ __forceinline__ uint32_t smem_u32(const void *p)
 {
     return static_cast<uint32_t>(__cvta_generic_to_shared(p));
@@ -168,6 +174,12 @@ __host__ __device__ constexpr uint64_t umma_smem_desc_sw128(uint32_t saddr, uint
 {
     return static_cast<uint64_t>((saddr & 0x3ffffu) >> 4) | (static_cast<uint64_t>((lbo_bytes >> 4) & 0x3fffu) << 16) |
            (static_cast<uint64_t>((sbo_bytes >> 4) & 0x3fffu) << 32) | (1ull << 46) | (2ull << 61);
+}
+// Start-address field of a matrix descriptor.  The mask matters: in a cluster launch the shared::cta
+// address carries the CTA rank in its high bits, which must not leak into the LBO field.
+__device__ __forceinline__ uint64_t desc_addr(uint32_t saddr)
+{
+    return static_cast<uint64_t>((saddr & 0x3ffffu) >> 4);
 }
 // Instruction descriptor for kind::f16 with FP16 A/B and FP32 D:
 //   [4,6) D fmt: 1 = F32   [7,10) A fmt: 0 = F16   [10,13) B fmt: 0 = F16
