@@ -127,6 +127,13 @@ int heal_set_workspace(void *ptr, size_t bytes);
 /* Number of kernels heal_* calls have launched in this process (split + GEMM), for accounting. */
 uint64_t heal_launch_count(void);
 
+/*
+ * Debug hook: force the kernel family regardless of shape.  0 = automatic (default), 1 = large-M kernels
+ * even for M <= 64, 2 = small-M kernel whenever M <= 64 (the default rule), 3 = single-CTA large-M kernel
+ * instead of CTA pairs.  Results are bit-identical whichever kernel runs; only speed changes.
+ */
+int heal_debug_force_kernel(int which);
+
 /* Library version: major * 10000 + minor * 100 + patch. */
 int heal_version(void);
 

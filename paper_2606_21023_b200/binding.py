@@ -45,6 +45,8 @@ def lib():
         L.heal_workspace_size.argtypes = [i64, i64, i64, u32]
         L.heal_set_workspace.restype = ci
         L.heal_set_workspace.argtypes = [vp, ctypes.c_size_t]
+        L.heal_debug_force_kernel.restype = ci
+        L.heal_debug_force_kernel.argtypes = [ci]
         L.heal_launch_count.restype = ctypes.c_uint64
         L.heal_version.restype = ci
         L.heal_last_cuda_error.restype = ci
@@ -76,6 +78,11 @@ def status_string(st: int) -> str:
 
 def version() -> int:
     return lib().heal_version()
+
+
+def debug_force_kernel(which: int):
+    """0 auto, 1 large-M kernels only, 2 small-M for M <= 64, 3 single-CTA large-M kernel (debug)."""
+    _check(lib().heal_debug_force_kernel(which))
 
 
 def launch_count() -> int:

@@ -14,6 +14,7 @@
 
 #include "heal_gemm_smallm.cuh"
 #include "heal_gemm_umma.cuh"
+#include "heal_gemm_umma2.cuh"
 #include "heal_split.cuh"
 
 namespace {
@@ -30,6 +31,9 @@ struct State {
     int device = -1;
     int num_sms = 0;
     int *diag = nullptr;
+    float *xfer = nullptr;         // per-CTA running-sum hand-off slots of the balanced schedule (128 x 256 floats each)
+    uint32_t *flags = nullptr;
+    uint32_t epoch = 0;
     // workspace
     void *user_ws = nullptr;
     size_t user_ws_bytes = 0;
@@ -78,6 +82,12 @@ int ensure_init()
     if (e != cudaSuccess) return fail(cuda_fail(e));
     e = cudaMemset(g.diag, 0, 64);
     if (e != cudaSuccess) return fail(cuda_fail(e));
+    e = cudaMalloc(&g.xfer, static_cast<size_t>(g.num_sms) * kBM * 256 * sizeof(float));
+    if (e != cudaSuccess) return fail(cuda_fail(e));
+    e = cudaMalloc(&g.flags, static_cast<size_t>(g.num_sms) * sizeof(uint32_t));
+    if (e != cudaSuccess) return fail(cuda_fail(e));
+    e = cudaMemset(g.flags, 0, static_cast<size_t>(g.num_sms) * sizeof(uint32_t));
+    if (e != cudaSuccess) return fail(cuda_fail(e));
     return HEAL_OK;
 }
 
@@ -122,6 +132,23 @@ int launch_split(int64_t rows, int64_t cols, const float *X, int64_t ldx, __half
     return HEAL_OK;
 }
 
+// Balanced schedule when whole tiles do not divide evenly over the G CTAs (or CTA pairs); numerically
+// invisible.  Full waves stay tile-granular; the ragged remainder (plus one full wave when the remainder
+// alone would leave less than half a tile per CTA) is cut at K-segment granularity.
+void set_balance(GemmArgs &args, int64_t tiles, int64_t G)
+{
+    static const bool no_balance = std::getenv("HEAL_NO_BALANCE") != nullptr;      // debug only
+    args.balance = 0;
+    args.dp_tiles = static_cast<int>(tiles);
+    if (!no_balance && tiles > G && tiles % G != 0) {
+        const int64_t waves = tiles / G, rem = tiles % G;
+        int64_t sk = rem;
+        if (rem * 2 < G && waves >= 1) sk += G;
+        args.balance = 1;
+        args.dp_tiles = static_cast<int>(tiles - sk);
+    }
+}
+
 // ---- steps G + E launch -----------------------------------------------------------------------
 template <class Cfg>
 int launch_gemm_cfg(int64_t M, int64_t N, int64_t K, const void *A_hi, const void *A_lo, int64_t lda, const void *B_hi,
@@ -163,10 +190,90 @@ int launch_gemm_cfg(int64_t M, int64_t N, int64_t K, const void *A_hi, const voi
     args.diag = g.diag;
     const int64_t tiles = static_cast<int64_t>(args.tiles_m) * args.tiles_n;
     const unsigned grid = static_cast<unsigned>(tiles < g.num_sms ? tiles : g.num_sms);
+    set_balance(args, tiles, g.num_sms);
+    args.xfer = g.xfer;
+    args.flags = g.flags;
+    args.epoch = ++g.epoch;
     kern<<<grid, kGemmThreads, Cfg::SMEM_BYTES, stream>>>(ta_hi, ta_lo, tb_hi, tb_lo, args);
     g_launches.fetch_add(1);
     HEAL_CUDA(cudaGetLastError());
     return HEAL_OK;
+}
+
+// CTA-pair (cta_group::2) variant: 256 x BN tiles, cluster of 2
+template <class Cfg>
+int launch_gemm2_cfg(int64_t M, int64_t N, int64_t K, const void *A_hi, const void *A_lo, int64_t lda, const void *B_hi,
+                     const void *B_lo, int64_t ldb, float *C, int64_t ldc, cudaStream_t stream)
+{
+    static bool attr_set = false;
+    auto kern = heal_gemm_umma2_kernel<Cfg>;
+    if (!attr_set) {
+        HEAL_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::SMEM_BYTES));
+        attr_set = true;
+    }
+    CUtensorMap ta_hi, ta_lo, tb_hi, tb_lo;
+    int st = encode_f16_2d(&ta_hi, A_hi, K, M, lda, kBK, kBM);
+    if (st) return st;
+    if (Cfg::A_PLANES == 2) {
+        st = encode_f16_2d(&ta_lo, A_lo, K, M, lda, kBK, kBM);
+        if (st) return st;
+    } else {
+        ta_lo = ta_hi;
+    }
+    if (Cfg::B_MN) st = encode_f16_2d(&tb_hi, B_hi, N, K, ldb, 64, kBK);
+    else           st = encode_f16_2d(&tb_hi, B_hi, K, N, ldb, kBK, Cfg::BH);
+    if (st) return st;
+    if (Cfg::B_PLANES == 2) {
+        if (Cfg::B_MN) st = encode_f16_2d(&tb_lo, B_lo, N, K, ldb, 64, kBK);
+        else           st = encode_f16_2d(&tb_lo, B_lo, K, N, ldb, kBK, Cfg::BH);
+        if (st) return st;
+    } else {
+        tb_lo = tb_hi;
+    }
+    GemmArgs args;
+    args.C = C;
+    args.ldc = ldc;
+    args.M = static_cast<int>(M);
+    args.N = static_cast<int>(N);
+    args.K = static_cast<int>(K);
+    args.tiles_m = static_cast<int>((M + 2 * kBM - 1) / (2 * kBM));
+    args.tiles_n = static_cast<int>((N + Cfg::BN - 1) / Cfg::BN);
+    args.diag = g.diag;
+    const int64_t tiles = static_cast<int64_t>(args.tiles_m) * args.tiles_n;
+    const int64_t pairs = g.num_sms / 2;
+    const int64_t G = tiles < pairs ? tiles : pairs;
+    set_balance(args, tiles, G);
+    args.xfer = g.xfer;
+    args.flags = g.flags;
+    args.epoch = ++g.epoch;
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(static_cast<unsigned>(2 * G));
+    cfg.blockDim = dim3(kGemmThreads);
+    cfg.dynamicSmemBytes = Cfg::SMEM_BYTES;
+    cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = 2;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    HEAL_CUDA(cudaLaunchKernelEx(&cfg, kern, ta_hi, ta_lo, tb_hi, tb_lo, args));
+    g_launches.fetch_add(1);
+    return HEAL_OK;
+}
+
+template <bool B_MN>
+int launch_gemm2_np(int nprod, int64_t M, int64_t N, int64_t K, const void *A_hi, const void *A_lo, int64_t lda,
+                    const void *B_hi, const void *B_lo, int64_t ldb, float *C, int64_t ldc, cudaStream_t s)
+{
+    switch (nprod) {
+    case 1: return launch_gemm2_cfg<Gemm2Cfg<256, 1, B_MN>>(M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, C, ldc, s);
+    case 2: return launch_gemm2_cfg<Gemm2Cfg<256, 2, B_MN>>(M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, C, ldc, s);
+    case 3: return launch_gemm2_cfg<Gemm2Cfg<256, 3, B_MN>>(M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, C, ldc, s);
+    case 4: return launch_gemm2_cfg<Gemm2Cfg<256, 4, B_MN>>(M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, C, ldc, s);
+    }
+    return HEAL_ERR_UNSUPPORTED_MODE;
 }
 
 template <int BN, bool B_MN>
@@ -293,13 +400,16 @@ int launch_small(int nprod, int64_t M, int64_t N, int64_t K, const void *A_hi, c
     return launch_small_np<64, B_MN>(nprod, M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, C, ldc, s, handled);
 }
 
-// Debug only: HEAL_FORCE_KERNEL=large|small overrides the M-based kernel choice (results are bit-identical).
+// Debug only: HEAL_FORCE_KERNEL=large|small|1cta (or heal_debug_force_kernel) overrides the kernel choice;
+// results are bit-identical whichever kernel runs.
+std::atomic<int> g_force{-1};
 int forced_kernel()
 {
-    static int v = -1;
+    int v = g_force.load();
     if (v < 0) {
         const char *e = std::getenv("HEAL_FORCE_KERNEL");
-        v = !e ? 0 : (e[0] == 'l' ? 1 : (e[0] == 's' ? 2 : 0));
+        v = !e ? 0 : (e[0] == 'l' ? 1 : (e[0] == 's' ? 2 : (e[0] == '1' ? 3 : 0)));
+        g_force.store(v);
     }
     return v;
 }
@@ -328,6 +438,11 @@ int presplit_impl(int64_t M, int64_t N, int64_t K, const void *A_hi, const void 
         int st = b_nk ? launch_small<false>(nprod, M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, static_cast<float *>(C), ldc, stream, &handled)
                       : launch_small<true>(nprod, M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, static_cast<float *>(C), ldc, stream, &handled);
         if (st || handled) return st;
+    }
+    if (M > kBM && N > 128 && force != 3) {          // CTA pairs: 256 x 256 tiles
+        if (b_nk)
+            return launch_gemm2_np<false>(nprod, M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, static_cast<float *>(C), ldc, stream);
+        return launch_gemm2_np<true>(nprod, M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, static_cast<float *>(C), ldc, stream);
     }
     if (b_nk)
         return launch_gemm_bn<false>(nprod, M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, static_cast<float *>(C), ldc, stream);
@@ -381,6 +496,13 @@ int get_ws(size_t bytes, cudaStream_t stream, void **out)
 extern "C" {
 
 int heal_version(void) { return 100; }
+
+int heal_debug_force_kernel(int which)
+{
+    if (which < 0 || which > 3) return HEAL_ERR_INVALID_VALUE;
+    g_force.store(which);
+    return HEAL_OK;
+}
 
 int heal_last_cuda_error(void) { return g_last_cuda_error.load(); }
 

@@ -49,6 +49,83 @@ struct GemmArgs {
     int M, N, K;
     int tiles_m, tiles_n;
     int *diag;
+    // segment-granular load balancing (0 = plain tile round-robin)
+    int balance;
+    int dp_tiles;           // tiles dealt whole, round-robin (multiple of the grid size)
+    float *xfer;            // per-CTA hand-off slot: kBM * BN floats each
+    uint32_t *flags;        // per-CTA flag, holds `epoch` once the slot is written
+    uint32_t epoch;
+};
+
+// Work distribution.  The unit of work is (tile, K segment).  The first `dp_tiles` tiles (a multiple of
+// gridDim.x) are dealt round-robin, whole tiles, so the CTAs of a wave walk K in lockstep and share W / A
+// panels in L2.  With `balance`, the remaining tiles (the ragged last wave) are cut at segment granularity
+// into gridDim.x contiguous, equal ranges, so a tile may be shared by neighbouring CTAs: CTA c computes
+// the first segments of a tile and hands the FP32 running sum to CTA c+1, which adds the following ones --
+// the same ascending-segment sum, copied, never re-associated, so the result is bit-identical to the
+// unbalanced schedule.  Within its range a CTA processes its "head" (the part it hands on) first and its
+// "tail" (the part that needs a neighbour's prefix) last, so the prefix is almost never waited for.
+struct TileSched {
+    int n_seg, n_dp, n_sk, dp_tiles;
+    int t_first, t_last, s_first, s_last_end, has_head, has_tail;
+    int n_chunks, bid, G;
+    // bid / G_: index of this CTA (or CTA pair) and number of CTAs (pairs) sharing the work
+    __device__ __forceinline__ void init(const GemmArgs &a, int n_seg_, int bid_, int G_)
+    {
+        n_seg = n_seg_;
+        bid = bid_;
+        G = G_;
+        const int num_tiles = a.tiles_m * a.tiles_n;
+        dp_tiles = a.balance ? a.dp_tiles : num_tiles;
+        n_dp = (dp_tiles > bid) ? (dp_tiles - 1 - bid) / G + 1 : 0;
+        n_sk = 0;
+        has_head = has_tail = 0;
+        t_first = t_last = s_first = s_last_end = 0;
+        if (a.balance) {
+            const long long total = static_cast<long long>(num_tiles - dp_tiles) * n_seg;
+            const long long u0 = total * bid / G, u1 = total * (bid + 1) / G;
+            if (u1 > u0) {
+                t_first = static_cast<int>(u0 / n_seg);
+                s_first = static_cast<int>(u0 % n_seg);
+                t_last = static_cast<int>((u1 - 1) / n_seg);
+                s_last_end = static_cast<int>((u1 - 1) % n_seg) + 1;
+                n_sk = t_last - t_first + 1;
+                if (n_sk > 1) {
+                    has_head = (s_last_end < n_seg) ? 1 : 0;
+                    has_tail = (s_first > 0) ? 1 : 0;
+                }
+            }
+        }
+        n_chunks = n_dp + n_sk;
+    }
+    // i-th chunk in processing order: tile index and its segment range [sb, se)
+    __device__ __forceinline__ void get(int i, int &tile, int &sb, int &se) const
+    {
+        if (i < n_dp) {
+            tile = bid + i * G;
+            sb = 0;
+            se = n_seg;
+            return;
+        }
+        i -= n_dp;
+        if (n_sk == 1) {                       // one (possibly partial, possibly interior) piece of a tile
+            tile = dp_tiles + t_first;
+            sb = s_first;
+            se = s_last_end;
+        } else if (has_head && i == 0) {
+            tile = dp_tiles + t_last;
+            sb = 0;
+            se = s_last_end;
+        } else if (has_tail && i == n_sk - 1) {
+            tile = dp_tiles + t_first;
+            sb = s_first;
+            se = n_seg;
+        } else {
+            tile = dp_tiles + t_first + has_tail + (i - has_head);
+            sb = 0;
+            se = n_seg;
+        }
+    }
 };
 
 template <class Cfg>
@@ -71,9 +148,10 @@ heal_gemm_umma_kernel(const __grid_constant__ CUtensorMap tm_a_hi, const __grid_
         reinterpret_cast<volatile uint32_t *>(smem_raw + (tmem_slot - smem_u32(smem_raw)));
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int num_tiles = args.tiles_m * args.tiles_n;
     const int k_tiles = (args.K + kBK - 1) / kBK;
     const int n_seg = (k_tiles + kTilesPerSeg - 1) / kTilesPerSeg;
+    TileSched sched;
+    sched.init(args, n_seg, static_cast<int>(blockIdx.x), static_cast<int>(gridDim.x));
 
     if (warp == 0 && lane == 0) {
         tma_prefetch_desc(&tm_a_hi);
@@ -106,10 +184,13 @@ heal_gemm_umma_kernel(const __grid_constant__ CUtensorMap tm_a_hi, const __grid_
         if (lane == 0) {
             int stage = 0;
             uint32_t phase = 0;
-            for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
+            for (int ci = 0; ci < sched.n_chunks; ++ci) {
+                int tile, sb_seg, se_seg;
+                sched.get(ci, tile, sb_seg, se_seg);
                 const int m0 = (tile % args.tiles_m) * kBM;
                 const int n0 = (tile / args.tiles_m) * BN;
-                for (int kt = 0; kt < k_tiles; ++kt) {
+                const int kt_hi = min(k_tiles, se_seg * kTilesPerSeg);
+                for (int kt = sb_seg * kTilesPerSeg; kt < kt_hi; ++kt) {
                     mbar_wait(empty_bar(stage), phase ^ 1u, args.diag, 100 + stage);
                     const uint32_t sb = smem_base + stage * Cfg::STAGE_BYTES;
                     const uint32_t fb = full_bar(stage);
@@ -148,8 +229,10 @@ heal_gemm_umma_kernel(const __grid_constant__ CUtensorMap tm_a_hi, const __grid_
             uint32_t phase = 0;
             int buf = 0;
             uint32_t tphase = 0;                                // bit b = phase of TMEM buffer b
-            for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
-                for (int seg = 0; seg < n_seg; ++seg) {
+            for (int ci = 0; ci < sched.n_chunks; ++ci) {
+                int tile, sb_seg, se_seg;
+                sched.get(ci, tile, sb_seg, se_seg);
+                for (int seg = sb_seg; seg < se_seg; ++seg) {
                     mbar_wait(tempty_bar(buf), ((tphase >> buf) & 1u) ^ 1u, args.diag, 300 + buf);
                     tc_fence_after();
                     const uint32_t d_tmem = tmem_base + static_cast<uint32_t>(buf * BN);
@@ -192,10 +275,38 @@ heal_gemm_umma_kernel(const __grid_constant__ CUtensorMap tm_a_hi, const __grid_
         float run[CPW];
         int buf = 0;
         uint32_t tphase = 0;
-        for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
+        const int etid = threadIdx.x - 128;                      // 0..255 among the epilogue threads
+        for (int ci = 0; ci < sched.n_chunks; ++ci) {
+            int tile, sb_seg, se_seg;
+            sched.get(ci, tile, sb_seg, se_seg);
             const int m0 = (tile % args.tiles_m) * kBM;
             const int n0 = (tile / args.tiles_m) * BN;
-            for (int seg = 0; seg < n_seg; ++seg) {
+            if (sb_seg > 0) {
+                // tail of a shared tile: start from the neighbour's running sum (segments 0..sb_seg-1)
+                const uint32_t *flag = args.flags + (blockIdx.x - 1);
+                if (etid == 0) {
+                    const uint64_t t0 = globaltimer_ns();
+                    uint32_t f;
+                    do {
+                        asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(f) : "l"(flag) : "memory");
+                        if (f != args.epoch && globaltimer_ns() - t0 > 4000000000ull) {
+                            args.diag[0] = 800;
+                            args.diag[1] = static_cast<int>(blockIdx.x);
+                            __trap();
+                        }
+                    } while (f != args.epoch);
+                }
+                asm volatile("bar.sync 1, 256;" ::: "memory");
+                const float4 *src = reinterpret_cast<const float4 *>(args.xfer + static_cast<size_t>(blockIdx.x - 1) * (kBM * BN));
+#pragma unroll
+                for (int c = 0; c < CPW / 4; ++c) {
+                    float4 v;
+                    asm volatile("ld.global.cg.v4.f32 {%0, %1, %2, %3}, [%4];"
+                                 : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(src + c * 256 + etid) : "memory");
+                    run[c * 4] = v.x; run[c * 4 + 1] = v.y; run[c * 4 + 2] = v.z; run[c * 4 + 3] = v.w;
+                }
+            }
+            for (int seg = sb_seg; seg < se_seg; ++seg) {
                 mbar_wait(tfull_bar(buf), (tphase >> buf) & 1u, args.diag, 400 + buf);
                 tc_fence_after();
                 const uint32_t taddr = tmem_base + (static_cast<uint32_t>(quad * 32) << 16) +
@@ -218,6 +329,18 @@ heal_gemm_umma_kernel(const __grid_constant__ CUtensorMap tm_a_hi, const __grid_
                 if (lane == 0) mbar_arrive(tempty_bar(buf));
                 tphase ^= 1u << buf;
                 buf ^= 1;
+            }
+            if (se_seg < n_seg) {
+                // head of a shared tile: hand the running sum to the next CTA
+                float4 *dst = reinterpret_cast<float4 *>(args.xfer + static_cast<size_t>(blockIdx.x) * (kBM * BN));
+#pragma unroll
+                for (int c = 0; c < CPW / 4; ++c)
+                    dst[c * 256 + etid] = make_float4(run[c * 4], run[c * 4 + 1], run[c * 4 + 2], run[c * 4 + 3]);
+                __threadfence();
+                asm volatile("bar.sync 1, 256;" ::: "memory");
+                if (etid == 0)
+                    asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(args.flags + blockIdx.x), "r"(args.epoch) : "memory");
+                continue;
             }
             // ---- store: thread owns row m0 + quad*32 + lane, CPW consecutive columns
             const int row = m0 + quad * 32 + lane;

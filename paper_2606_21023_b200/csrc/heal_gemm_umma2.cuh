@@ -1,0 +1,278 @@
+// heal_gemm_umma2.cuh -- steps G + E with CTA pairs (tcgen05 cta_group::2): the two CTAs of a cluster
+// share one 256 x BN output tile.  Each CTA loads its own 128 rows of the A planes and HALF of the B
+// tile (BN/2 columns); the leader's single thread issues 256 x BN x 16 MMAs that read both CTAs' shared
+// memory and write each CTA's 128 rows of the accumulator into its own TMEM.  Per CTA and k-tile this
+// moves 48 KB (2P) / 64 KB (3P) from L2 instead of 64 / 96 KB for single-CTA tiles -- the L2 -> SM fabric,
+// not the tensor pipe, is what bounds the single-CTA kernel.
+//
+// Same numerical contract as heal_gemm_umma.cuh (K segments of 512, k16 slices ascending, products
+// hi.hi, hi.lo, lo.hi, lo.lo, segments added in FP32 RN ascending): bit-identical results.
+//
+// Barriers: full[stage] lives in the leader (2 producer arrivals + both CTAs' TMA bytes); empty[stage],
+// tmem_full[buf] are signalled in both CTAs by multicast tcgen05.commit; tmem_empty[buf] lives in the
+// leader (16 arrivals: 8 epilogue warps of each CTA).
+#pragma once
+#include "heal_gemm_umma.cuh"
+
+namespace heal {
+
+template <int BN_, int NPROD_, bool B_MN_>
+struct Gemm2Cfg {
+    static constexpr int BN = BN_;                       // pair-tile width; each CTA stages BN/2 columns of B
+    static constexpr int NPROD = NPROD_;
+    static constexpr bool B_MN = B_MN_;
+    static constexpr int A_PLANES = NPROD >= 2 ? 2 : 1;
+    static constexpr int B_PLANES = NPROD >= 3 ? 2 : 1;
+    static constexpr int A_TILE = kBM * kBK * 2;
+    static constexpr int BH = BN / 2;
+    static constexpr int B_TILE = BH * kBK * 2;
+    static constexpr int STAGE_BYTES = A_PLANES * A_TILE + B_PLANES * B_TILE;
+    static constexpr int BAR_BYTES = 256;
+    static constexpr int STAGES_RAW = (kSmemLimit - 1024 - BAR_BYTES) / STAGE_BYTES;
+    static constexpr int STAGES = STAGES_RAW > 8 ? 8 : STAGES_RAW;
+    static constexpr int SMEM_BYTES = 1024 + STAGES * STAGE_BYTES + BAR_BYTES;
+    static constexpr int TMEM_COLS = 512;
+    static constexpr int COLS_PER_WARP = BN / 2;
+    static_assert(BN == 256 || BN == 128, "BN");
+    static_assert(STAGES >= 2, "need at least two stages");
+};
+
+template <class Cfg>
+__global__ void __launch_bounds__(kGemmThreads, 1)
+heal_gemm_umma2_kernel(const __grid_constant__ CUtensorMap tm_a_hi, const __grid_constant__ CUtensorMap tm_a_lo,
+                       const __grid_constant__ CUtensorMap tm_b_hi, const __grid_constant__ CUtensorMap tm_b_lo,
+                       const GemmArgs args)
+{
+    constexpr int BN = Cfg::BN, NPROD = Cfg::NPROD, STAGES = Cfg::STAGES;
+    extern __shared__ uint8_t smem_raw[];
+    const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
+    const uint32_t bar_base = smem_base + STAGES * Cfg::STAGE_BYTES;
+    auto full_bar = [&](int s) { return bar_base + 8u * s; };
+    auto empty_bar = [&](int s) { return bar_base + 8u * (STAGES + s); };
+    auto tfull_bar = [&](int b) { return bar_base + 8u * (2 * STAGES + b); };
+    auto tempty_bar = [&](int b) { return bar_base + 8u * (2 * STAGES + 2 + b); };
+    const uint32_t tmem_slot = bar_base + 8u * (2 * STAGES + 4);
+    volatile uint32_t *tmem_slot_ptr =
+        reinterpret_cast<volatile uint32_t *>(smem_raw + (tmem_slot - smem_u32(smem_raw)));
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int rank = static_cast<int>(cluster_ctarank());          // 0 = leader
+    const int k_tiles = (args.K + kBK - 1) / kBK;
+    const int n_seg = (k_tiles + kTilesPerSeg - 1) / kTilesPerSeg;
+    TileSched sched;
+    sched.init(args, n_seg, static_cast<int>(blockIdx.x >> 1), static_cast<int>(gridDim.x >> 1));
+
+    if (warp == 0 && lane == 0) {
+        tma_prefetch_desc(&tm_a_hi);
+        if (Cfg::A_PLANES == 2) tma_prefetch_desc(&tm_a_lo);
+        tma_prefetch_desc(&tm_b_hi);
+        if (Cfg::B_PLANES == 2) tma_prefetch_desc(&tm_b_lo);
+    }
+    if (warp == 1 && lane == 0) {
+        for (int s = 0; s < STAGES; ++s) {
+            mbar_init(full_bar(s), 2);            // one arrive.expect_tx from each CTA's producer
+            mbar_init(empty_bar(s), 1);
+        }
+        for (int b = 0; b < 2; ++b) {
+            mbar_init(tfull_bar(b), 1);
+            mbar_init(tempty_bar(b), 16);         // 8 epilogue warps of each CTA
+        }
+        fence_mbar_init();
+    }
+    if (warp == 2) {
+        tmem_alloc_2cta(tmem_slot, Cfg::TMEM_COLS);
+        tmem_relinquish_2cta();
+    }
+    tc_fence_before();
+    __syncthreads();
+    cluster_sync_all();                            // peer barriers initialised before any remote arrive
+    tc_fence_after();
+    const uint32_t tmem_base = *tmem_slot_ptr;
+
+    if (warp == 0) {
+        // ================================ TMA producer (both CTAs) =====================
+        if (lane == 0) {
+            int stage = 0;
+            uint32_t phase = 0;
+            for (int ci = 0; ci < sched.n_chunks; ++ci) {
+                int tile, sb_seg, se_seg;
+                sched.get(ci, tile, sb_seg, se_seg);
+                const int m0 = (tile % args.tiles_m) * (2 * kBM) + rank * kBM;
+                const int n0 = (tile / args.tiles_m) * BN + rank * Cfg::BH;
+                const int kt_hi = min(k_tiles, se_seg * kTilesPerSeg);
+                for (int kt = sb_seg * kTilesPerSeg; kt < kt_hi; ++kt) {
+                    mbar_wait(empty_bar(stage), phase ^ 1u, args.diag, 100 + stage);
+                    const uint32_t sb = smem_base + stage * Cfg::STAGE_BYTES;
+                    const uint32_t fb = leader_addr(full_bar(stage));
+                    mbar_arrive_expect_tx_cluster(fb, Cfg::STAGE_BYTES);
+                    const int k0 = kt * kBK;
+                    tma_load_2d_2cta(sb, &tm_a_hi, fb, k0, m0);
+                    if (Cfg::A_PLANES == 2) tma_load_2d_2cta(sb + Cfg::A_TILE, &tm_a_lo, fb, k0, m0);
+                    const uint32_t sbB = sb + Cfg::A_PLANES * Cfg::A_TILE;
+                    if (Cfg::B_MN) {
+#pragma unroll
+                        for (int c = 0; c < Cfg::BH / 64; ++c) {
+                            tma_load_2d_2cta(sbB + c * (64 * kBK * 2), &tm_b_hi, fb, n0 + c * 64, k0);
+                            if (Cfg::B_PLANES == 2)
+                                tma_load_2d_2cta(sbB + Cfg::B_TILE + c * (64 * kBK * 2), &tm_b_lo, fb, n0 + c * 64, k0);
+                        }
+                    } else {
+                        tma_load_2d_2cta(sbB, &tm_b_hi, fb, k0, n0);
+                        if (Cfg::B_PLANES == 2) tma_load_2d_2cta(sbB + Cfg::B_TILE, &tm_b_lo, fb, k0, n0);
+                    }
+                    if (++stage == STAGES) { stage = 0; phase ^= 1u; }
+                }
+            }
+        }
+    } else if (warp == 1) {
+        // ================================ MMA issuer (leader only) =====================
+        if (lane == 0 && rank == 0) {
+            constexpr uint32_t idesc = umma_idesc_f16_f32(2 * kBM, BN, 0u, Cfg::B_MN ? 1u : 0u);
+            constexpr uint64_t adesc0 = umma_smem_desc_sw128(0, 16, 1024);
+            constexpr uint64_t bdesc0 = Cfg::B_MN ? umma_smem_desc_sw128(0, kBK * 128, 1024) : adesc0;
+            constexpr uint32_t a_step = 32 >> 4;
+            constexpr uint32_t b_step = (Cfg::B_MN ? 16 * 128 : 32) >> 4;
+            int stage = 0;
+            uint32_t phase = 0;
+            int buf = 0;
+            uint32_t tphase = 0;
+            for (int ci = 0; ci < sched.n_chunks; ++ci) {
+                int tile, sb_seg, se_seg;
+                sched.get(ci, tile, sb_seg, se_seg);
+                for (int seg = sb_seg; seg < se_seg; ++seg) {
+                    mbar_wait(tempty_bar(buf), ((tphase >> buf) & 1u) ^ 1u, args.diag, 300 + buf);
+                    tc_fence_after();
+                    const uint32_t d_tmem = tmem_base + static_cast<uint32_t>(buf * BN);
+                    const int kt_end = min(k_tiles, (seg + 1) * kTilesPerSeg);
+                    uint32_t accumulate = 0;
+                    for (int kt = seg * kTilesPerSeg; kt < kt_end; ++kt) {
+                        mbar_wait(full_bar(stage), phase, args.diag, 200 + stage);
+                        tc_fence_after();
+                        const uint32_t sb = smem_base + stage * Cfg::STAGE_BYTES;
+                        const uint64_t a_hi = adesc0 | desc_addr(sb);
+                        const uint64_t a_lo = adesc0 | desc_addr(sb + Cfg::A_TILE);
+                        const uint64_t b_hi = bdesc0 | desc_addr(sb + Cfg::A_PLANES * Cfg::A_TILE);
+                        const uint64_t b_lo = bdesc0 | desc_addr(sb + Cfg::A_PLANES * Cfg::A_TILE + Cfg::B_TILE);
+#pragma unroll
+                        for (int j = 0; j < kBK / 16; ++j) {
+                            const uint64_t ao = static_cast<uint64_t>(j * a_step), bo = static_cast<uint64_t>(j * b_step);
+                            umma_f16_2cta(d_tmem, a_hi + ao, b_hi + bo, idesc, accumulate);
+                            accumulate = 1;
+                            if (NPROD == 2) umma_f16_2cta(d_tmem, a_lo + ao, b_hi + bo, idesc, 1);
+                            if (NPROD >= 3) {
+                                umma_f16_2cta(d_tmem, a_hi + ao, b_lo + bo, idesc, 1);
+                                umma_f16_2cta(d_tmem, a_lo + ao, b_hi + bo, idesc, 1);
+                            }
+                            if (NPROD == 4) umma_f16_2cta(d_tmem, a_lo + ao, b_lo + bo, idesc, 1);
+                        }
+                        umma_commit_2cta(empty_bar(stage), 3);      // slot free in both CTAs
+                        if (++stage == STAGES) { stage = 0; phase ^= 1u; }
+                    }
+                    umma_commit_2cta(tfull_bar(buf), 3);            // segment partial complete in both TMEMs
+                    tphase ^= 1u << buf;
+                    buf ^= 1;
+                }
+            }
+        }
+    } else if (warp >= 4) {
+        // ================================ epilogue (both CTAs) =========================
+        constexpr int CPW = Cfg::COLS_PER_WARP;
+        const int quad = warp & 3;
+        const int chalf = (warp - 4) >> 2;
+        const int etid = threadIdx.x - 128;
+        float run[CPW];
+        int buf = 0;
+        uint32_t tphase = 0;
+        for (int ci = 0; ci < sched.n_chunks; ++ci) {
+            int tile, sb_seg, se_seg;
+            sched.get(ci, tile, sb_seg, se_seg);
+            const int m0 = (tile % args.tiles_m) * (2 * kBM) + rank * kBM;
+            const int n0 = (tile / args.tiles_m) * BN;
+            if (sb_seg > 0) {
+                const uint32_t *flag = args.flags + (blockIdx.x - 2);        // same rank, previous pair
+                if (etid == 0) {
+                    const uint64_t t0 = globaltimer_ns();
+                    uint32_t f;
+                    do {
+                        asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(f) : "l"(flag) : "memory");
+                        if (f != args.epoch && globaltimer_ns() - t0 > 4000000000ull) {
+                            args.diag[0] = 800;
+                            args.diag[1] = static_cast<int>(blockIdx.x);
+                            __trap();
+                        }
+                    } while (f != args.epoch);
+                }
+                asm volatile("bar.sync 1, 256;" ::: "memory");
+                const float4 *src = reinterpret_cast<const float4 *>(args.xfer + static_cast<size_t>(blockIdx.x - 2) * (kBM * 256));
+#pragma unroll
+                for (int c = 0; c < CPW / 4; ++c) {
+                    float4 v;
+                    asm volatile("ld.global.cg.v4.f32 {%0, %1, %2, %3}, [%4];"
+                                 : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(src + c * 256 + etid) : "memory");
+                    run[c * 4] = v.x; run[c * 4 + 1] = v.y; run[c * 4 + 2] = v.z; run[c * 4 + 3] = v.w;
+                }
+            }
+            for (int seg = sb_seg; seg < se_seg; ++seg) {
+                mbar_wait(tfull_bar(buf), (tphase >> buf) & 1u, args.diag, 400 + buf);
+                tc_fence_after();
+                const uint32_t taddr = tmem_base + (static_cast<uint32_t>(quad * 32) << 16) +
+                                       static_cast<uint32_t>(buf * BN + chalf * CPW);
+#pragma unroll
+                for (int c = 0; c < CPW / 16; ++c) {
+                    uint32_t v[16];
+                    tmem_ld_32x32b_x16(taddr + c * 16, v);
+                    tmem_ld_wait();
+                    if (seg == 0) {
+#pragma unroll
+                        for (int i = 0; i < 16; ++i) run[c * 16 + i] = __uint_as_float(v[i]);
+                    } else {
+#pragma unroll
+                        for (int i = 0; i < 16; ++i) run[c * 16 + i] = __fadd_rn(run[c * 16 + i], __uint_as_float(v[i]));
+                    }
+                }
+                tc_fence_before();
+                __syncwarp();
+                if (lane == 0) mbar_arrive_cluster(leader_addr(tempty_bar(buf)));
+                tphase ^= 1u << buf;
+                buf ^= 1;
+            }
+            if (se_seg < n_seg) {
+                float4 *dst = reinterpret_cast<float4 *>(args.xfer + static_cast<size_t>(blockIdx.x) * (kBM * 256));
+#pragma unroll
+                for (int c = 0; c < CPW / 4; ++c)
+                    dst[c * 256 + etid] = make_float4(run[c * 4], run[c * 4 + 1], run[c * 4 + 2], run[c * 4 + 3]);
+                __threadfence();
+                asm volatile("bar.sync 1, 256;" ::: "memory");
+                if (etid == 0)
+                    asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(args.flags + blockIdx.x), "r"(args.epoch) : "memory");
+                continue;
+            }
+            const int row = m0 + quad * 32 + lane;
+            const int col0 = n0 + chalf * CPW;
+            if (row < args.M) {
+                float *crow = args.C + static_cast<int64_t>(row) * args.ldc;
+#pragma unroll
+                for (int c = 0; c < CPW; c += 4) {
+                    const int col = col0 + c;
+                    if (col + 3 < args.N) {
+                        *reinterpret_cast<float4 *>(crow + col) = make_float4(run[c], run[c + 1], run[c + 2], run[c + 3]);
+                    } else {
+#pragma unroll
+                        for (int i = 0; i < 4; ++i)
+                            if (col + i < args.N) crow[col + i] = run[c + i];
+                    }
+                }
+            }
+        }
+    }
+
+    tc_fence_before();
+    __syncthreads();
+    cluster_sync_all();                            // the peer may still be reading this CTA's smem / signalling its barriers
+    if (warp == 2) {
+        tc_fence_after();
+        tmem_dealloc_2cta(tmem_base, Cfg::TMEM_COLS);
+    }
+}
+
+}  // namespace heal

@@ -301,6 +301,25 @@ def test_bitwise_across_m_row_position_and_padding(hb, inputs):
     assert np.array_equal(hb.heal_gemm(dev(A), Wnk, 2 | hb.B_NK).cpu().numpy(), full)
 
 
+@pytest.mark.parametrize("M,N,K,nprod,b_nk", [(40, 1032, 8192, 2, False), (64, 520, 4096, 3, False), (17, 264, 1000, 2, True),
+                                              (300, 520, 4104, 2, False), (700, 1032, 2056, 3, True), (1300, 4104, 2056, 2, False)])
+def test_kernel_families_bit_identical(hb, inputs, M, N, K, nprod, b_nk):
+    """The three kernel families (small-M swap-AB cluster kernel, single-CTA and CTA-pair large-M kernels, with
+    and without the segment-granular balanced schedule) implement one reduction order: same bits."""
+    A = dev(inputs.activations(M, K, seed=5, outliers=True))
+    B = inputs.weights_f32(K, N, seed=5, nk=b_nk) if nprod >= 3 else inputs.weights_f16(K, N, seed=5, nk=b_nk)
+    B = dev(B)
+    mode = nprod | (hb.B_NK if b_nk else 0)
+    outs = []
+    try:
+        for which in (0, 1, 3):          # auto | large-M kernels only | single-CTA large-M kernel
+            hb.debug_force_kernel(which)
+            outs.append(hb.heal_gemm(A, B, mode).clone())
+    finally:
+        hb.debug_force_kernel(0)
+    assert torch.equal(outs[0], outs[1]) and torch.equal(outs[0], outs[2])
+
+
 def test_presplit_and_host_variants_match(hb, inputs):
     A = inputs.activations(150, 1024, seed=4)
     B = inputs.weights_f32(1024, 264, seed=4)
