@@ -117,6 +117,28 @@ int encode_f16_2d(CUtensorMap *tm, const void *base, int64_t inner, int64_t oute
 
 namespace {
 
+// Launch attributes: optional cluster dimension + programmatic stream serialization (PDL), which lets the
+// kernel's prologue (barrier init, TMEM allocation, descriptor prefetch) overlap the previous kernel's tail;
+// every kernel calls griddepcontrol.wait before its first global-memory access.
+int fill_attrs(cudaLaunchAttribute *attr, unsigned cluster_x)
+{
+    static const bool no_pdl = std::getenv("HEAL_NO_PDL") != nullptr;          // debug only
+    int n = 0;
+    if (cluster_x > 1) {
+        attr[n].id = cudaLaunchAttributeClusterDimension;
+        attr[n].val.clusterDim.x = cluster_x;
+        attr[n].val.clusterDim.y = 1;
+        attr[n].val.clusterDim.z = 1;
+        ++n;
+    }
+    if (!no_pdl) {
+        attr[n].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        attr[n].val.programmaticStreamSerializationAllowed = 1;
+        ++n;
+    }
+    return n;
+}
+
 // ---- step S launch --------------------------------------------------------------------------
 int launch_split(int64_t rows, int64_t cols, const float *X, int64_t ldx, __half *hi, __half *lo, int64_t ld,
                  cudaStream_t stream)
@@ -126,9 +148,15 @@ int launch_split(int64_t rows, int64_t cols, const float *X, int64_t ldx, __half
     int64_t blocks = (vecs + 255) / 256;
     const int64_t cap = static_cast<int64_t>(g.num_sms) * 16;      // grid-stride beyond 16 CTAs per SM
     if (blocks > cap) blocks = cap;
-    heal_split_kernel<<<static_cast<unsigned>(blocks), 256, 0, stream>>>(X, ldx, rows, cols, hi, lo, ld);
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(static_cast<unsigned>(blocks));
+    cfg.blockDim = dim3(256);
+    cfg.stream = stream;
+    cudaLaunchAttribute attr[2];
+    cfg.numAttrs = fill_attrs(attr, 1);
+    cfg.attrs = attr;
+    HEAL_CUDA(cudaLaunchKernelEx(&cfg, heal_split_kernel, X, ldx, rows, cols, hi, lo, ld));
     g_launches.fetch_add(1);
-    HEAL_CUDA(cudaGetLastError());
     return HEAL_OK;
 }
 
@@ -194,9 +222,16 @@ int launch_gemm_cfg(int64_t M, int64_t N, int64_t K, const void *A_hi, const voi
     args.xfer = g.xfer;
     args.flags = g.flags;
     args.epoch = ++g.epoch;
-    kern<<<grid, kGemmThreads, Cfg::SMEM_BYTES, stream>>>(ta_hi, ta_lo, tb_hi, tb_lo, args);
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(grid);
+    cfg.blockDim = dim3(kGemmThreads);
+    cfg.dynamicSmemBytes = Cfg::SMEM_BYTES;
+    cfg.stream = stream;
+    cudaLaunchAttribute attr[2];
+    cfg.numAttrs = fill_attrs(attr, 1);
+    cfg.attrs = attr;
+    HEAL_CUDA(cudaLaunchKernelEx(&cfg, kern, ta_hi, ta_lo, tb_hi, tb_lo, args));
     g_launches.fetch_add(1);
-    HEAL_CUDA(cudaGetLastError());
     return HEAL_OK;
 }
 
@@ -251,13 +286,9 @@ int launch_gemm2_cfg(int64_t M, int64_t N, int64_t K, const void *A_hi, const vo
     cfg.blockDim = dim3(kGemmThreads);
     cfg.dynamicSmemBytes = Cfg::SMEM_BYTES;
     cfg.stream = stream;
-    cudaLaunchAttribute attr[1];
-    attr[0].id = cudaLaunchAttributeClusterDimension;
-    attr[0].val.clusterDim.x = 2;
-    attr[0].val.clusterDim.y = 1;
-    attr[0].val.clusterDim.z = 1;
+    cudaLaunchAttribute attr[2];
+    cfg.numAttrs = fill_attrs(attr, 2);
     cfg.attrs = attr;
-    cfg.numAttrs = 1;
     HEAL_CUDA(cudaLaunchKernelEx(&cfg, kern, ta_hi, ta_lo, tb_hi, tb_lo, args));
     g_launches.fetch_add(1);
     return HEAL_OK;
@@ -307,10 +338,15 @@ int launch_small_cfg(int64_t M, int64_t N, int64_t K, const void *A_hi, const vo
     *handled = false;
     const int n_seg = static_cast<int>((K + kKSeg - 1) / kKSeg);
     const int64_t panels = (N + kSmallBNW - 1) / kSmallBNW;
-    // Cluster size: enough CTAs to keep every SM streaming (about two per SM), at most 8 and at most
-    // n_seg.  Purely a performance choice: the result does not depend on it (segment sums are exact copies).
+    // Cluster size: the smallest that gives about 1.4 CTAs per SM (measured: enough to saturate HBM, while
+    // every doubling adds cluster-reduction overhead), at most 8 and at most n_seg.  Purely a performance
+    // choice: the result does not depend on it (segment sums are exact copies).
     int cs = 1;
-    while (cs * 2 <= 8 && cs * 2 <= n_seg && panels * cs < 2 * g.num_sms) cs *= 2;
+    while (cs * 2 <= 8 && cs * 2 <= n_seg && panels * cs * 5 < 7 * g.num_sms) cs *= 2;
+    if (const char *e = std::getenv("HEAL_SMALL_CS")) {                          // debug only
+        const int want = std::atoi(e);
+        if (want == 1 || want == 2 || want == 4 || want == 8) cs = want <= n_seg ? want : cs;
+    }
     int max_local = (n_seg + cs - 1) / cs;
     while (max_local * Cfg::MPAD > 512 && cs * 2 <= 8 && cs * 2 <= n_seg) {
         cs *= 2;
@@ -365,13 +401,9 @@ int launch_small_cfg(int64_t M, int64_t N, int64_t K, const void *A_hi, const vo
     cfg.blockDim = dim3(kSmallThreads);
     cfg.dynamicSmemBytes = smem;
     cfg.stream = stream;
-    cudaLaunchAttribute attr[1];
-    attr[0].id = cudaLaunchAttributeClusterDimension;
-    attr[0].val.clusterDim.x = static_cast<unsigned>(cs);
-    attr[0].val.clusterDim.y = 1;
-    attr[0].val.clusterDim.z = 1;
+    cudaLaunchAttribute attr[2];
+    cfg.numAttrs = fill_attrs(attr, static_cast<unsigned>(cs));
     cfg.attrs = attr;
-    cfg.numAttrs = 1;
     HEAL_CUDA(cudaLaunchKernelEx(&cfg, kern, tx_hi, tx_lo, tw_hi, tw_lo, args));
     g_launches.fetch_add(1);
     *handled = true;

@@ -105,6 +105,8 @@ heal_gemm_smallm_kernel(const __grid_constant__ CUtensorMap tm_x_hi, const __gri
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem_base = *tmem_slot_ptr;
+    pdl_wait();                       // everything above overlapped the previous kernel's tail
+    pdl_launch_dependents();
 
     if (warp == 0) {
         // ================================ TMA producer ================================

@@ -178,6 +178,8 @@ heal_gemm_umma_kernel(const __grid_constant__ CUtensorMap tm_a_hi, const __grid_
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem_base = *tmem_slot_ptr;
+    pdl_wait();
+    pdl_launch_dependents();
 
     if (warp == 0) {
         // ================================ TMA producer ================================

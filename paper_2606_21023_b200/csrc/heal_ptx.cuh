@@ -28,6 +28,12 @@ __device__ __forceinline__ uint64_t globaltimer_ns()
     return t;
 }
 
+// ---- programmatic dependent launch: lets this grid's prologue overlap the previous grid's tail.
+// pdl_wait() must precede the first global-memory access; it returns once every prerequisite grid has
+// completed and its writes are visible (a no-op when the launch carries no programmatic dependency).
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
 // ---- mbarrier ------------------------------------------------------------------------------
 __device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count)
 {

@@ -25,6 +25,8 @@ __global__ void __launch_bounds__(256)
 heal_split_kernel(const float *__restrict__ X, int64_t ldx, int64_t rows, int64_t cols,
                   __half *__restrict__ hi, __half *__restrict__ lo, int64_t ld)
 {
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     const int64_t cols8 = (cols + 7) >> 3;
     const int64_t total = rows * cols8;
     for (int64_t v = blockIdx.x * static_cast<int64_t>(blockDim.x) + threadIdx.x; v < total;
