@@ -24,6 +24,7 @@ using namespace heal;
 std::atomic<int> g_last_cuda_error{0};
 std::atomic<uint64_t> g_launches{0};
 std::mutex g_mu;
+std::mutex g_xf_mu;
 
 struct State {
     bool init = false;
@@ -31,9 +32,14 @@ struct State {
     int device = -1;
     int num_sms = 0;
     int *diag = nullptr;
-    float *xfer = nullptr;         // per-CTA running-sum hand-off slots of the balanced schedule (128 x 256 floats each)
-    uint32_t *flags = nullptr;
-    uint32_t epoch = 0;
+    // hand-off buffers of the balanced schedule, one set per stream (concurrent streams must not share them)
+    struct Xfer {
+        cudaStream_t stream = nullptr;
+        bool used = false;
+        float *xfer = nullptr;     // per-CTA running-sum slots (128 x 256 floats each)
+        uint32_t *flags = nullptr; // per-CTA flag: 1 = slot written, reset by the consumer
+    };
+    Xfer xf[8];
     // workspace
     void *user_ws = nullptr;
     size_t user_ws_bytes = 0;
@@ -81,12 +87,6 @@ int ensure_init()
     e = cudaMalloc(&g.diag, 64);
     if (e != cudaSuccess) return fail(cuda_fail(e));
     e = cudaMemset(g.diag, 0, 64);
-    if (e != cudaSuccess) return fail(cuda_fail(e));
-    e = cudaMalloc(&g.xfer, static_cast<size_t>(g.num_sms) * kBM * 256 * sizeof(float));
-    if (e != cudaSuccess) return fail(cuda_fail(e));
-    e = cudaMalloc(&g.flags, static_cast<size_t>(g.num_sms) * sizeof(uint32_t));
-    if (e != cudaSuccess) return fail(cuda_fail(e));
-    e = cudaMemset(g.flags, 0, static_cast<size_t>(g.num_sms) * sizeof(uint32_t));
     if (e != cudaSuccess) return fail(cuda_fail(e));
     return HEAL_OK;
 }
@@ -160,11 +160,46 @@ int launch_split(int64_t rows, int64_t cols, const float *X, int64_t ldx, __half
     return HEAL_OK;
 }
 
+// Hand-off buffers for `stream`: created on first use (19 MB per stream, at most 8 streams; further
+// streams simply run the unbalanced schedule, which gives the same bits).
+bool bind_xfer(GemmArgs &args, cudaStream_t stream)
+{
+    std::lock_guard<std::mutex> lk(g_xf_mu);
+    State::Xfer *slot = nullptr;
+    for (auto &x : g.xf)
+        if (x.used && x.stream == stream) { slot = &x; break; }
+    if (!slot) {
+        for (auto &x : g.xf)
+            if (!x.used) { slot = &x; break; }
+        if (!slot) return false;
+        cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+        if (cudaStreamIsCapturing(stream, &cap) != cudaSuccess || cap != cudaStreamCaptureStatusNone) return false;
+        float *xf = nullptr;
+        uint32_t *fl = nullptr;
+        if (cudaMalloc(&xf, static_cast<size_t>(g.num_sms) * kBM * 256 * sizeof(float)) != cudaSuccess) return false;
+        if (cudaMalloc(&fl, static_cast<size_t>(g.num_sms) * sizeof(uint32_t)) != cudaSuccess ||
+            cudaMemset(fl, 0, static_cast<size_t>(g.num_sms) * sizeof(uint32_t)) != cudaSuccess) {
+            cudaFree(xf);
+            if (fl) cudaFree(fl);
+            return false;
+        }
+        slot->stream = stream;
+        slot->used = true;
+        slot->xfer = xf;
+        slot->flags = fl;
+    }
+    args.xfer = slot->xfer;
+    args.flags = slot->flags;
+    return true;
+}
+
 // Balanced schedule when whole tiles do not divide evenly over the G CTAs (or CTA pairs); numerically
 // invisible.  Full waves stay tile-granular; the ragged remainder (plus one full wave when the remainder
 // alone would leave less than half a tile per CTA) is cut at K-segment granularity.
-void set_balance(GemmArgs &args, int64_t tiles, int64_t G)
+void set_balance(GemmArgs &args, int64_t tiles, int64_t G, cudaStream_t stream)
 {
+    args.xfer = nullptr;
+    args.flags = nullptr;
     static const bool no_balance = std::getenv("HEAL_NO_BALANCE") != nullptr;      // debug only
     args.balance = 0;
     args.dp_tiles = static_cast<int>(tiles);
@@ -172,8 +207,10 @@ void set_balance(GemmArgs &args, int64_t tiles, int64_t G)
         const int64_t waves = tiles / G, rem = tiles % G;
         int64_t sk = rem;
         if (rem * 2 < G && waves >= 1) sk += G;
-        args.balance = 1;
-        args.dp_tiles = static_cast<int>(tiles - sk);
+        if (bind_xfer(args, stream)) {
+            args.balance = 1;
+            args.dp_tiles = static_cast<int>(tiles - sk);
+        }
     }
 }
 
@@ -218,10 +255,7 @@ int launch_gemm_cfg(int64_t M, int64_t N, int64_t K, const void *A_hi, const voi
     args.diag = g.diag;
     const int64_t tiles = static_cast<int64_t>(args.tiles_m) * args.tiles_n;
     const unsigned grid = static_cast<unsigned>(tiles < g.num_sms ? tiles : g.num_sms);
-    set_balance(args, tiles, g.num_sms);
-    args.xfer = g.xfer;
-    args.flags = g.flags;
-    args.epoch = ++g.epoch;
+    set_balance(args, tiles, g.num_sms, stream);
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(grid);
     cfg.blockDim = dim3(kGemmThreads);
@@ -277,10 +311,7 @@ int launch_gemm2_cfg(int64_t M, int64_t N, int64_t K, const void *A_hi, const vo
     const int64_t tiles = static_cast<int64_t>(args.tiles_m) * args.tiles_n;
     const int64_t pairs = g.num_sms / 2;
     const int64_t G = tiles < pairs ? tiles : pairs;
-    set_balance(args, tiles, G);
-    args.xfer = g.xfer;
-    args.flags = g.flags;
-    args.epoch = ++g.epoch;
+    set_balance(args, tiles, G, stream);
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(static_cast<unsigned>(2 * G));
     cfg.blockDim = dim3(kGemmThreads);

@@ -53,8 +53,7 @@ struct GemmArgs {
     int balance;
     int dp_tiles;           // tiles dealt whole, round-robin (multiple of the grid size)
     float *xfer;            // per-CTA hand-off slot: kBM * BN floats each
-    uint32_t *flags;        // per-CTA flag, holds `epoch` once the slot is written
-    uint32_t epoch;
+    uint32_t *flags;        // per-CTA flag: 1 once the slot is written, reset to 0 by its consumer
 };
 
 // Work distribution.  The unit of work is (tile, K segment).  The first `dp_tiles` tiles (a multiple of
@@ -291,12 +290,12 @@ heal_gemm_umma_kernel(const __grid_constant__ CUtensorMap tm_a_hi, const __grid_
                     uint32_t f;
                     do {
                         asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(f) : "l"(flag) : "memory");
-                        if (f != args.epoch && globaltimer_ns() - t0 > 4000000000ull) {
+                        if (f == 0u && globaltimer_ns() - t0 > 4000000000ull) {
                             args.diag[0] = 800;
                             args.diag[1] = static_cast<int>(blockIdx.x);
                             __trap();
                         }
-                    } while (f != args.epoch);
+                    } while (f == 0u);
                 }
                 asm volatile("bar.sync 1, 256;" ::: "memory");
                 const float4 *src = reinterpret_cast<const float4 *>(args.xfer + static_cast<size_t>(blockIdx.x - 1) * (kBM * BN));
@@ -307,6 +306,10 @@ heal_gemm_umma_kernel(const __grid_constant__ CUtensorMap tm_a_hi, const __grid_
                                  : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(src + c * 256 + etid) : "memory");
                     run[c * 4] = v.x; run[c * 4 + 1] = v.y; run[c * 4 + 2] = v.z; run[c * 4 + 3] = v.w;
                 }
+                // consumed: re-arm the flag for the next launch (launches on a stream are serialised, and
+                // 0/1 flags -- unlike launch counters -- stay correct when a captured graph is replayed)
+                asm volatile("bar.sync 1, 256;" ::: "memory");
+                if (etid == 0) asm volatile("st.relaxed.gpu.global.u32 [%0], %1;" ::"l"(flag), "r"(0u) : "memory");
             }
             for (int seg = sb_seg; seg < se_seg; ++seg) {
                 mbar_wait(tfull_bar(buf), (tphase >> buf) & 1u, args.diag, 400 + buf);
@@ -341,7 +344,7 @@ heal_gemm_umma_kernel(const __grid_constant__ CUtensorMap tm_a_hi, const __grid_
                 __threadfence();
                 asm volatile("bar.sync 1, 256;" ::: "memory");
                 if (etid == 0)
-                    asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(args.flags + blockIdx.x), "r"(args.epoch) : "memory");
+                    asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(args.flags + blockIdx.x), "r"(1u) : "memory");
                 continue;
             }
             // ---- store: thread owns row m0 + quad*32 + lane, CPW consecutive columns

@@ -320,6 +320,39 @@ def test_kernel_families_bit_identical(hb, inputs, M, N, K, nprod, b_nk):
     assert torch.equal(outs[0], outs[1]) and torch.equal(outs[0], outs[2])
 
 
+def test_balanced_schedule_graph_replay_and_two_streams(hb, inputs):
+    """A shape whose tiles do not divide over the SMs (segment-granular hand-off between CTAs): replaying a
+    captured CUDA graph and running on two streams at once must reproduce the eager result bit for bit."""
+    M, N, K = 1300, 4104, 2056
+    A = dev(inputs.activations(M, K, seed=6, outliers=True))
+    W = dev(inputs.weights_f16(K, N, seed=6))
+    ref = hb.heal_gemm(A, W, 2).clone()
+    ah, al = hb.heal_split(A)
+    C = torch.zeros_like(ref)
+    s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+    torch.cuda.synchronize()
+    with torch.cuda.stream(s1):
+        hb.heal_gemm_presplit(ah, al, W, None, 2, C=C)          # binds this stream's hand-off buffers
+        s1.synchronize()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=s1):
+            hb.heal_gemm_presplit(ah, al, W, None, 2, C=C)
+            hb.heal_gemm_presplit(ah, al, W, None, 2, C=C)
+        for _ in range(5):
+            C.zero_()
+            g.replay()
+            s1.synchronize()
+            assert torch.equal(C, ref)
+    C1, C2 = torch.zeros_like(ref), torch.zeros_like(ref)
+    for _ in range(3):
+        with torch.cuda.stream(s1):
+            hb.heal_gemm_presplit(ah, al, W, None, 2, C=C1)
+        with torch.cuda.stream(s2):
+            hb.heal_gemm_presplit(ah, al, W, None, 2, C=C2)
+    torch.cuda.synchronize()
+    assert torch.equal(C1, ref) and torch.equal(C2, ref)
+
+
 def test_presplit_and_host_variants_match(hb, inputs):
     A = inputs.activations(150, 1024, seed=4)
     B = inputs.weights_f32(1024, 264, seed=4)
