@@ -230,7 +230,7 @@ def run_ours(args):
             "config": {"workload": WORKLOAD, "global_tokens": world * M_TOK, "parallelism": f"dp{world} over token batches",
                        "l2": "inputs larger than L2 (A+W+C = 268 MB per GEMM vs 126 MB L2)",
                        "tensor_tflops": N_PROD * value},
-            "roofline": {"bound": "tensor", "kernel": "heal_gemm_umma_kernel<BN=256,2P>", "achieved": achieved, "peak": peak,
+            "roofline": {"bound": "tensor", "kernel": "heal_gemm_umma2_kernel<BN=256,2P> (CTA pairs)", "achieved": achieved, "peak": peak,
                          "unit": "TFLOP/s", "frac": achieved / peak, "traffic": traffic,
                          "peak_kind": f"{peaks['src']} cuBLAS bf16 {'sustained' if long_run else 'burst'} (fp16 = bf16 rate)",
                          "frac_of_nominal_2250": achieved / 2250.0, "avg_launch_ms": ms_gemm,
