@@ -59,6 +59,11 @@ typedef enum {
 #define HEAL_MODE_4P 4u        /* 3P + lo.lo (diagnostic)   B is FP32                              */
 #define HEAL_B_NK 0x10u        /* B is stored N x K (K contiguous) -- the paper's W^T /
                                   nn.Linear layout; default is K x N (N contiguous) */
+#define HEAL_B_STATIC 0x20u    /* promise: B (static weights, the inference case) is not written by the
+                                  operations enqueued on `stream` just before this call.  The kernel may
+                                  then start streaming B while its stream predecessor is still finishing
+                                  (programmatic dependent launch); everything that reads A or writes C
+                                  still waits for the predecessor.  Same bits with or without the flag. */
 
 /*
  * C[M x N] (FP32) = A[M x K] (FP32) . B          one pass of the whole path: split, MMAs, epilogue.

@@ -15,6 +15,7 @@ LIB_PATH = os.path.join(_HERE, "libheal.so")
 
 MODE_1P, MODE_2P, MODE_3P, MODE_4P = 1, 2, 3, 4
 B_NK = 0x10
+B_STATIC = 0x20
 K_SEGMENT = 512
 
 _lib = None

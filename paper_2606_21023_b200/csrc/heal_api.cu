@@ -361,17 +361,31 @@ int launch_gemm_bn(int nprod, int64_t M, int64_t N, int64_t K, const void *A_hi,
     return launch_gemm_np<256, B_MN>(nprod, M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, C, ldc, s);
 }
 
+#ifdef HEAL_TRACE
+unsigned long long *g_trace = nullptr;
+unsigned g_trace_seq = 0;
+#endif
+
 // ---- small-M (decode) launch: swap-AB, K segments spread over a cluster ----------------------------
+// Activations come either as hi/lo planes (A_hi/A_lo, pitch lda) or, with Cfg::FUSED, as the FP32 matrix
+// A32 (pitch lda32) which the kernel splits itself.
+struct SmallIn {
+    const void *A_hi, *A_lo;
+    int64_t lda;
+    const float *A32;
+    int64_t lda32;
+    bool b_static;
+};
+
 template <class Cfg>
-int launch_small_cfg(int64_t M, int64_t N, int64_t K, const void *A_hi, const void *A_lo, int64_t lda, const void *B_hi,
-                     const void *B_lo, int64_t ldb, float *C, int64_t ldc, cudaStream_t stream, bool *handled)
+int launch_small_cfg(int64_t M, int64_t N, int64_t K, const SmallIn &in, const void *B_hi, const void *B_lo, int64_t ldb,
+                     float *C, int64_t ldc, cudaStream_t stream, bool *handled)
 {
     *handled = false;
     const int n_seg = static_cast<int>((K + kKSeg - 1) / kKSeg);
     const int64_t panels = (N + kSmallBNW - 1) / kSmallBNW;
-    // Cluster size: the smallest that gives about 1.4 CTAs per SM (measured: enough to saturate HBM, while
-    // every doubling adds cluster-reduction overhead), at most 8 and at most n_seg.  Purely a performance
-    // choice: the result does not depend on it (segment sums are exact copies).
+    // Cluster size: the smallest that gives about 1.4 CTAs per SM (measured: enough to saturate HBM), at most 8
+    // and at most n_seg.  Purely a performance choice: the result does not depend on it (segment sums are exact copies).
     int cs = 1;
     while (cs * 2 <= 8 && cs * 2 <= n_seg && panels * cs * 5 < 7 * g.num_sms) cs *= 2;
     if (const char *e = std::getenv("HEAL_SMALL_CS")) {                          // debug only
@@ -386,10 +400,31 @@ int launch_small_cfg(int64_t M, int64_t N, int64_t K, const void *A_hi, const vo
     int tmem_cols = 32;
     while (tmem_cols < max_local * Cfg::MPAD) tmem_cols *= 2;
     if (tmem_cols > 512) return HEAL_OK;                        // leave to the large-M kernel
-    const size_t pipe = static_cast<size_t>(Cfg::STAGES) * Cfg::STAGE_BYTES;
-    const size_t stage_area = cs > 1 ? static_cast<size_t>(max_local) * Cfg::MPAD * kSmallBNW * 4 : 0;
-    size_t smem = 1024 + (pipe > stage_area ? pipe : stage_area) + Cfg::BAR_BYTES;
-    if (smem > static_cast<size_t>(kSmemLimit)) return HEAL_OK;
+    const int rpr = cs > 1 ? static_cast<int>((M + cs - 1) / cs) : 0;
+    const size_t red = cs > 1 ? static_cast<size_t>(n_seg) * rpr * kSmallBNW * 4 : 0;
+    // Shared memory.  Measured on B200 (decode 4096 x 4096, LM head): what matters is how many CTAs are resident
+    // -- the next kernel's CTAs run their prologue (and with HEAL_B_STATIC prefetch W) beside this kernel's --
+    // rather than the depth of one CTA's pipeline: aim for three CTAs per SM (two when a stage exceeds 24 KB,
+    // one when the CTA needs more than half of TMEM), at least 2 stages, at most 8 and no more than the CTA
+    // has k-tiles.
+    // Partial sums pushed by the cluster: a dedicated area when small (decode), else overlaid on the pipeline.
+    const bool red_alias = red > static_cast<size_t>(16 * 1024);
+    const size_t fixed = 1024 + (red_alias ? 0 : red) + Cfg::BAR_BYTES;
+    size_t budget = tmem_cols > 256 ? static_cast<size_t>(kSmemLimit)
+                    : (Cfg::STAGE_BYTES <= 24 * 1024 && cs > 1 ? static_cast<size_t>(74 * 1024) : static_cast<size_t>(112 * 1024));
+    if (budget < fixed + 3 * static_cast<size_t>(Cfg::STAGE_BYTES) && budget < static_cast<size_t>(112 * 1024)) budget = static_cast<size_t>(112 * 1024);
+    if (budget < fixed + 3 * static_cast<size_t>(Cfg::STAGE_BYTES)) budget = static_cast<size_t>(kSmemLimit);
+    if (budget < fixed + 2 * static_cast<size_t>(Cfg::STAGE_BYTES)) return HEAL_OK;      // large-M kernel
+    if (red_alias && fixed + red > static_cast<size_t>(kSmemLimit)) return HEAL_OK;
+    int stages = static_cast<int>((budget - fixed) / Cfg::STAGE_BYTES);
+    if (stages > kSmallMaxStages) stages = kSmallMaxStages;
+    if (stages > max_local * kTilesPerSeg) stages = max_local * kTilesPerSeg;
+    if (const char *e = std::getenv("HEAL_SMALL_STAGES")) {                      // debug only
+        const int want = std::atoi(e);
+        if (want >= 2 && want <= kSmallMaxStages && fixed + static_cast<size_t>(want) * Cfg::STAGE_BYTES <= static_cast<size_t>(kSmemLimit)) stages = want;
+    }
+    size_t smem = fixed + static_cast<size_t>(stages) * Cfg::STAGE_BYTES;
+    if (red_alias && smem < fixed + red) smem = fixed + red;
     // more than half of TMEM: make sure only one CTA fits per SM (two could not both allocate)
     if (tmem_cols > 256 && smem < static_cast<size_t>(kSmemLimit) / 2 + 2048) smem = static_cast<size_t>(kSmemLimit) / 2 + 2048;
     auto kern = heal_gemm_smallm_kernel<Cfg>;
@@ -399,14 +434,7 @@ int launch_small_cfg(int64_t M, int64_t N, int64_t K, const void *A_hi, const vo
         attr_smem = smem;
     }
     CUtensorMap tx_hi, tx_lo, tw_hi, tw_lo;
-    int st = encode_f16_2d(&tx_hi, A_hi, K, M, lda, kBK, Cfg::MPAD);
-    if (st) return st;
-    if (Cfg::A_PLANES == 2) {
-        st = encode_f16_2d(&tx_lo, A_lo, K, M, lda, kBK, Cfg::MPAD);
-        if (st) return st;
-    } else {
-        tx_lo = tx_hi;
-    }
+    int st;
     if (Cfg::B_MN) st = encode_f16_2d(&tw_hi, B_hi, N, K, ldb, 64, kBK);
     else           st = encode_f16_2d(&tw_hi, B_hi, K, N, ldb, kBK, kSmallBNW);
     if (st) return st;
@@ -417,16 +445,43 @@ int launch_small_cfg(int64_t M, int64_t N, int64_t K, const void *A_hi, const vo
     } else {
         tw_lo = tw_hi;
     }
+    if (Cfg::FUSED) {
+        tx_hi = tx_lo = tw_hi;                                  // unused by the fused kernel
+    } else {
+        st = encode_f16_2d(&tx_hi, in.A_hi, K, M, in.lda, kBK, Cfg::MPAD);
+        if (st) return st;
+        if (Cfg::A_PLANES == 2) {
+            st = encode_f16_2d(&tx_lo, in.A_lo, K, M, in.lda, kBK, Cfg::MPAD);
+            if (st) return st;
+        } else {
+            tx_lo = tx_hi;
+        }
+    }
     SmallArgs args;
     args.C = C;
     args.ldc = ldc;
+    args.A = in.A32;
+    args.lda = in.lda32;
     args.M = static_cast<int>(M);
     args.N = static_cast<int>(N);
     args.K = static_cast<int>(K);
     args.n_seg = n_seg;
     args.max_local = max_local;
     args.tmem_cols = tmem_cols;
+    args.stages = stages;
+    args.rows_per_rank = rpr;
+    args.red_bytes = static_cast<int>(red);
+    args.red_alias = red_alias ? 1 : 0;
+    static const bool no_static = std::getenv("HEAL_NO_STATIC") != nullptr;       // debug only
+    args.b_static = (in.b_static && !no_static) ? 1 : 0;
     args.diag = g.diag;
+    args.trace = nullptr;
+#ifdef HEAL_TRACE
+    if (g_trace) {                      // 16 rotating regions of 1024 CTAs x 16 stamps
+        args.trace = g_trace + (g_trace_seq % 16) * (1024 * 64);
+        ++g_trace_seq;
+    }
+#endif
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(static_cast<unsigned>(panels * cs));
     cfg.blockDim = dim3(kSmallThreads);
@@ -442,25 +497,32 @@ int launch_small_cfg(int64_t M, int64_t N, int64_t K, const void *A_hi, const vo
 }
 
 template <int MPAD, bool B_MN>
-int launch_small_np(int nprod, int64_t M, int64_t N, int64_t K, const void *A_hi, const void *A_lo, int64_t lda,
-                    const void *B_hi, const void *B_lo, int64_t ldb, float *C, int64_t ldc, cudaStream_t s, bool *handled)
+int launch_small_np(int nprod, int64_t M, int64_t N, int64_t K, const SmallIn &in, const void *B_hi, const void *B_lo,
+                    int64_t ldb, float *C, int64_t ldc, cudaStream_t s, bool *handled)
 {
+    if (in.A32) {                                               // fused split: FP16 weights only
+        switch (nprod) {
+        case 1: return launch_small_cfg<SmallCfg<MPAD, 1, B_MN, true>>(M, N, K, in, B_hi, B_lo, ldb, C, ldc, s, handled);
+        case 2: return launch_small_cfg<SmallCfg<MPAD, 2, B_MN, true>>(M, N, K, in, B_hi, B_lo, ldb, C, ldc, s, handled);
+        }
+        return HEAL_ERR_UNSUPPORTED_MODE;
+    }
     switch (nprod) {
-    case 1: return launch_small_cfg<SmallCfg<MPAD, 1, B_MN>>(M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, C, ldc, s, handled);
-    case 2: return launch_small_cfg<SmallCfg<MPAD, 2, B_MN>>(M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, C, ldc, s, handled);
-    case 3: return launch_small_cfg<SmallCfg<MPAD, 3, B_MN>>(M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, C, ldc, s, handled);
-    case 4: return launch_small_cfg<SmallCfg<MPAD, 4, B_MN>>(M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, C, ldc, s, handled);
+    case 1: return launch_small_cfg<SmallCfg<MPAD, 1, B_MN, false>>(M, N, K, in, B_hi, B_lo, ldb, C, ldc, s, handled);
+    case 2: return launch_small_cfg<SmallCfg<MPAD, 2, B_MN, false>>(M, N, K, in, B_hi, B_lo, ldb, C, ldc, s, handled);
+    case 3: return launch_small_cfg<SmallCfg<MPAD, 3, B_MN, false>>(M, N, K, in, B_hi, B_lo, ldb, C, ldc, s, handled);
+    case 4: return launch_small_cfg<SmallCfg<MPAD, 4, B_MN, false>>(M, N, K, in, B_hi, B_lo, ldb, C, ldc, s, handled);
     }
     return HEAL_ERR_UNSUPPORTED_MODE;
 }
 
 template <bool B_MN>
-int launch_small(int nprod, int64_t M, int64_t N, int64_t K, const void *A_hi, const void *A_lo, int64_t lda,
-                 const void *B_hi, const void *B_lo, int64_t ldb, float *C, int64_t ldc, cudaStream_t s, bool *handled)
+int launch_small(int nprod, int64_t M, int64_t N, int64_t K, const SmallIn &in, const void *B_hi, const void *B_lo,
+                 int64_t ldb, float *C, int64_t ldc, cudaStream_t s, bool *handled)
 {
-    if (M <= 16) return launch_small_np<16, B_MN>(nprod, M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, C, ldc, s, handled);
-    if (M <= 32) return launch_small_np<32, B_MN>(nprod, M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, C, ldc, s, handled);
-    return launch_small_np<64, B_MN>(nprod, M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, C, ldc, s, handled);
+    if (M <= 16) return launch_small_np<16, B_MN>(nprod, M, N, K, in, B_hi, B_lo, ldb, C, ldc, s, handled);
+    if (M <= 32) return launch_small_np<32, B_MN>(nprod, M, N, K, in, B_hi, B_lo, ldb, C, ldc, s, handled);
+    return launch_small_np<64, B_MN>(nprod, M, N, K, in, B_hi, B_lo, ldb, C, ldc, s, handled);
 }
 
 // Debug only: HEAL_FORCE_KERNEL=large|small|1cta (or heal_debug_force_kernel) overrides the kernel choice;
@@ -479,7 +541,7 @@ int forced_kernel()
 
 int validate_mode(uint32_t mode, int *nprod, bool *b_nk)
 {
-    if (mode & ~(HEAL_MODE_PRODUCTS_MASK | HEAL_B_NK)) return HEAL_ERR_UNSUPPORTED_MODE;
+    if (mode & ~(HEAL_MODE_PRODUCTS_MASK | HEAL_B_NK | HEAL_B_STATIC)) return HEAL_ERR_UNSUPPORTED_MODE;
     const uint32_t p = mode & HEAL_MODE_PRODUCTS_MASK;
     if (p < 1 || p > 4) return HEAL_ERR_UNSUPPORTED_MODE;
     *nprod = static_cast<int>(p);
@@ -487,9 +549,12 @@ int validate_mode(uint32_t mode, int *nprod, bool *b_nk)
     return HEAL_OK;
 }
 
+// A32 != nullptr: FP32 activations for the fused small-M kernel (M <= 64, FP16 weights) instead of planes
 int presplit_impl(int64_t M, int64_t N, int64_t K, const void *A_hi, const void *A_lo, int64_t lda, const void *B_hi,
-                  const void *B_lo, int64_t ldb, void *C, int64_t ldc, int nprod, bool b_nk, cudaStream_t stream)
+                  const void *B_lo, int64_t ldb, void *C, int64_t ldc, int nprod, bool b_nk, bool b_static,
+                  cudaStream_t stream, const float *A32 = nullptr, int64_t lda32 = 0, bool *handled_out = nullptr)
 {
+    if (handled_out) *handled_out = true;
     if (K == 0) {
         HEAL_CUDA(cudaMemset2DAsync(C, static_cast<size_t>(ldc) * 4, 0, static_cast<size_t>(N) * 4,
                                     static_cast<size_t>(M), stream));
@@ -498,9 +563,14 @@ int presplit_impl(int64_t M, int64_t N, int64_t K, const void *A_hi, const void 
     const int force = forced_kernel();
     if ((M <= 64 && force != 1) || (force == 2 && M <= 64)) {
         bool handled = false;
-        int st = b_nk ? launch_small<false>(nprod, M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, static_cast<float *>(C), ldc, stream, &handled)
-                      : launch_small<true>(nprod, M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, static_cast<float *>(C), ldc, stream, &handled);
+        const SmallIn in{A_hi, A_lo, lda, A32, lda32, b_static};
+        int st = b_nk ? launch_small<false>(nprod, M, N, K, in, B_hi, B_lo, ldb, static_cast<float *>(C), ldc, stream, &handled)
+                      : launch_small<true>(nprod, M, N, K, in, B_hi, B_lo, ldb, static_cast<float *>(C), ldc, stream, &handled);
         if (st || handled) return st;
+    }
+    if (A32) {                                         // the caller must split first and come back with planes
+        *handled_out = false;
+        return HEAL_OK;
     }
     if (M > kBM && N > 128 && force != 3) {          // CTA pairs: 256 x 256 tiles
         if (b_nk)
@@ -566,6 +636,16 @@ int heal_debug_force_kernel(int which)
     g_force.store(which);
     return HEAL_OK;
 }
+
+#ifdef HEAL_TRACE
+// trace builds only (not part of include/heal.h): device buffer of 16 x 1024 x 16 uint64 phase stamps
+int heal_debug_set_trace(void *ptr)
+{
+    g_trace = static_cast<unsigned long long *>(ptr);
+    g_trace_seq = 0;
+    return HEAL_OK;
+}
+#endif
 
 int heal_last_cuda_error(void) { return g_last_cuda_error.load(); }
 
@@ -638,7 +718,7 @@ int heal_gemm_presplit(int64_t M, int64_t N, int64_t K, const void *A_hi, const 
     if (!aligned16(C) || (ldc & 3)) return HEAL_ERR_MISALIGNED;
     st = ensure_init();
     if (st) return st;
-    return presplit_impl(M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, C, ldc, nprod, b_nk,
+    return presplit_impl(M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, C, ldc, nprod, b_nk, (mode & HEAL_B_STATIC) != 0,
                          static_cast<cudaStream_t>(stream));
 }
 
@@ -663,7 +743,17 @@ int heal_gemm(int64_t M, int64_t N, int64_t K, const void *A, int64_t lda, const
     st = ensure_init();
     if (st) return st;
     cudaStream_t stream = static_cast<cudaStream_t>(stream_);
-    if (K == 0) return presplit_impl(M, N, K, nullptr, nullptr, lda, nullptr, nullptr, ldb, C, ldc, nprod, b_nk, stream);
+    const bool b_static = (mode & HEAL_B_STATIC) != 0;
+    if (K == 0) return presplit_impl(M, N, K, nullptr, nullptr, lda, nullptr, nullptr, ldb, C, ldc, nprod, b_nk, b_static, stream);
+    static const bool no_fused = std::getenv("HEAL_NO_FUSED") != nullptr;          // debug only
+    if (M <= 16 && !b_f32 && !no_fused && forced_kernel() != 1) {
+        // decode shapes (M <= 16) with FP16 weights: step S runs inside the GEMM kernel (no planes, one launch);
+        // above that the in-kernel conversion costs more than the split launch it saves (measured)
+        bool handled = false;
+        st = presplit_impl(M, N, K, nullptr, nullptr, 0, B, nullptr, ldb, C, ldc, nprod, b_nk, b_static, stream,
+                           static_cast<const float *>(A), lda, &handled);
+        if (st || handled) return st;
+    }
 
     std::lock_guard<std::mutex> lk(g_mu);
     const WsPlan p = plan_ws(M, N, K, nprod, b_nk);
@@ -688,7 +778,7 @@ int heal_gemm(int64_t M, int64_t N, int64_t K, const void *A, int64_t lda, const
         b_lo = bl;
         ldb_eff = p.ldb_p;
     }
-    return presplit_impl(M, N, K, a_hi, a_lo, p.lda_p, b_hi, b_lo, ldb_eff, C, ldc, nprod, b_nk, stream);
+    return presplit_impl(M, N, K, a_hi, a_lo, p.lda_p, b_hi, b_lo, ldb_eff, C, ldc, nprod, b_nk, b_static, stream);
 }
 
 int heal_gemm_host(int64_t M, int64_t N, int64_t K, const void *A_host, int64_t lda, const void *B_host, int64_t ldb,

@@ -1,61 +1,78 @@
-// heal_gemm_smallm.cuh -- steps G + E for small M (decode / LM-head shapes, M <= 64): the weight
+// heal_gemm_smallm.cuh -- steps (S +) G + E for small M (decode / LM-head shapes, M <= 64): the weight
 // matrix is streamed once from HBM and is the tensor core's 128-row operand ("swap-AB"), the few
 // token rows are the UMMA N side (16/32/64), and the K segments of one 128-column weight panel are
 // spread over the CTAs of a thread-block cluster so that enough CTAs stream HBM.
 //
 // Same reduction order as heal_gemm_umma.cuh (include/heal.h): inside a 512-long K segment the tensor
 // core accumulates k16 slices in ascending k, products hi.hi, hi.lo, lo.hi, lo.lo; the segment partial
-// sums are then added in ascending segment order in FP32 RN -- here by a distributed reduction over
-// the cluster's shared memory (DSMEM), no atomics.  Results are bit-identical to the large-M kernel.
+// sums are then added in ascending segment order in FP32 RN.  Results are bit-identical to the
+// large-M kernels.
 //
 // Cluster of CS CTAs = one 128-column panel; CTA rank r owns segments r, r+CS, r+2CS, ... (local slot
-// j = s / CS lives in TMEM columns j*MPAD..).  Roles per CTA (192 threads): warp 0 TMA producer,
-// warp 1 MMA issuer + TMEM allocator, warps 2-5 epilogue (warp w owns TMEM lanes 32*(w%4)..+31).
+// j = s / CS lives in TMEM columns j*MPAD..).  Token rows are dealt to the ranks in contiguous blocks: every rank
+// PUSHES its segment partials of that row straight from its TMEM registers into the owner's shared
+// memory (st.shared::cluster) and then arrives (release.cluster) on the owner's mbarrier; the owner adds
+// the n_seg partials in ascending segment order and stores C.  No atomics, no cluster-wide barrier
+// after the main loop.
+//
+// FUSED variant (heal_gemm, B already FP16): step S runs inside the kernel -- the four epilogue warps
+// convert the FP32 activations of each k-tile to hi/lo FP16 (same arithmetic as
+// heal_split.cuh) directly into the swizzled shared-memory operand tiles while the TMA producer streams W;
+// no hi/lo planes in HBM, no split launch.
+//
+// Static weights (HEAL_B_STATIC): the producer starts streaming W before griddepcontrol.wait, i.e. while
+// the previous kernel on the stream is still in its tail; everything that touches activations or C waits.
+//
+// Roles per CTA (192 threads): warp 0 TMA producer, warp 1 MMA issuer + TMEM allocator, warps 2-5
+// converter (FUSED) and epilogue (warp w owns TMEM lanes 32*(w%4)..+31).
 #pragma once
 #include "heal_ptx.cuh"
+#include "heal_split.cuh"
 
 namespace heal {
 
 constexpr int kSmallThreads = 192;
 constexpr int kSmallBNW = 128;          // weight columns per panel (UMMA M)
+constexpr int kSmallMaxStages = 8;
 
-__device__ __forceinline__ uint32_t map_to_cta(uint32_t saddr, uint32_t rank)
-{
-    uint32_t r;
-    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(saddr), "r"(rank));
-    return r;
-}
-__device__ __forceinline__ float ld_dsmem_f32(uint32_t addr)
-{
-    float v;
-    asm volatile("ld.shared::cluster.f32 %0, [%1];" : "=f"(v) : "r"(addr) : "memory");
-    return v;
-}
-
-template <int MPAD_, int NPROD_, bool B_MN_>
+template <int MPAD_, int NPROD_, bool B_MN_, bool FUSED_>
 struct SmallCfg {
     static constexpr int MPAD = MPAD_;                  // UMMA N: padded token count
     static constexpr int NPROD = NPROD_;
     static constexpr bool B_MN = B_MN_;                 // weights stored K x N (N contiguous)
+    static constexpr bool FUSED = FUSED_;               // split the FP32 activations in the kernel
     static constexpr int A_PLANES = NPROD >= 2 ? 2 : 1; // activation planes
     static constexpr int B_PLANES = NPROD >= 3 ? 2 : 1; // weight planes
     static constexpr int W_TILE = kSmallBNW * kBK * 2;  // 16 KB
     static constexpr int X_TILE = MPAD * kBK * 2;
     static constexpr int X_TILE_AL = (X_TILE + 1023) / 1024 * 1024;
     static constexpr int STAGE_BYTES = B_PLANES * W_TILE + A_PLANES * X_TILE_AL;
-    static constexpr int STAGES = (96 * 1024 / STAGE_BYTES) < 2 ? 2 : (96 * 1024 / STAGE_BYTES) > 8 ? 8 : (96 * 1024 / STAGE_BYTES);
+    static constexpr int W_BYTES = B_PLANES * W_TILE;
+    static constexpr int TX_BYTES = W_BYTES + (FUSED ? 0 : A_PLANES * X_TILE);
     static constexpr int BAR_BYTES = 256;
+    static constexpr int TASKS = MPAD / 16;             // FUSED: 8-float chunks per converter thread per k-tile
+    static constexpr int PF = MPAD <= 32 ? 4 : 2;       // FUSED: k-tiles of activations kept in flight in registers
     static_assert(MPAD % 16 == 0 && MPAD >= 16 && MPAD <= 64, "MPAD");
+    static_assert(!FUSED || NPROD <= 2, "the fused split needs FP16 weights");
 };
 
 struct SmallArgs {
     float *C;
     int64_t ldc;
+    const float *A;       // FUSED: FP32 activations, row pitch lda (elements)
+    int64_t lda;
     int M, N, K;
     int n_seg;            // ceil(K / 512)
     int max_local;        // ceil(n_seg / CS)
     int tmem_cols;        // power of two >= max(32, max_local * MPAD)
+    int stages;           // pipeline depth (2..8)
+    int rows_per_rank;    // ceil(M / CS): token rows finished by one rank (CS > 1)
+    int red_bytes;        // CS > 1: n_seg * rows_per_rank * 128 floats of partial sums pushed by the cluster
+    int red_alias;        // the pushed partial sums reuse the pipeline stages (large M * K): needs a second cluster
+                          // barrier ("every rank's main loop is over") before anybody pushes
+    int b_static;         // HEAL_B_STATIC: W may be read before the stream predecessor has completed
     int *diag;
+    unsigned long long *trace;   // phase stamps (HEAL_TRACE builds only), else unused
 };
 
 template <class Cfg>
@@ -64,82 +81,143 @@ heal_gemm_smallm_kernel(const __grid_constant__ CUtensorMap tm_x_hi, const __gri
                         const __grid_constant__ CUtensorMap tm_w_hi, const __grid_constant__ CUtensorMap tm_w_lo,
                         const SmallArgs args)
 {
-    constexpr int MPAD = Cfg::MPAD, NPROD = Cfg::NPROD, STAGES = Cfg::STAGES;
+    constexpr int MPAD = Cfg::MPAD, NPROD = Cfg::NPROD;
+    constexpr bool FUSED = Cfg::FUSED;
     extern __shared__ uint8_t smem_raw[];
     const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
-    // layout: [pipeline stages | aliased after the main loop by the segment staging area][barriers]
-    const uint32_t pipe_bytes = STAGES * Cfg::STAGE_BYTES;
+    // layout: [pipeline stages][partial sums pushed by the cluster][barriers]; with red_alias the partial sums
+    // overlay the pipeline stages instead
+    const int STAGES = args.stages;
     const uint32_t cs = cluster_nctarank();
     const uint32_t rank = cluster_ctarank();
-    const uint32_t stage_area = cs > 1 ? static_cast<uint32_t>(args.max_local) * MPAD * kSmallBNW * 4 : 0u;
-    const uint32_t bar_base = smem_base + (pipe_bytes > stage_area ? pipe_bytes : stage_area);
+    const uint32_t pipe_bytes = static_cast<uint32_t>(STAGES) * Cfg::STAGE_BYTES;
+    const uint32_t red_base = args.red_alias ? smem_base : smem_base + pipe_bytes;
+    const uint32_t bar_base = args.red_alias ? smem_base + max(pipe_bytes, static_cast<uint32_t>(args.red_bytes))
+                                             : red_base + static_cast<uint32_t>(args.red_bytes);
     auto full_bar = [&](int s) { return bar_base + 8u * s; };
-    auto empty_bar = [&](int s) { return bar_base + 8u * (STAGES + s); };
-    const uint32_t done_bar = bar_base + 8u * (2 * STAGES);
-    const uint32_t tmem_slot = bar_base + 8u * (2 * STAGES + 1);
+    auto empty_bar = [&](int s) { return bar_base + 64u + 8u * s; };
+    auto xfull_bar = [&](int s) { return bar_base + 128u + 8u * s; };
+    const uint32_t done_bar = bar_base + 192u;
+    const uint32_t red_bar = bar_base + 200u;
+    const uint32_t tmem_slot = bar_base + 208u;
     volatile uint32_t *tmem_slot_ptr = reinterpret_cast<volatile uint32_t *>(smem_raw + (tmem_slot - smem_u32(smem_raw)));
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    if (threadIdx.x == 0) HEAL_STAMP(args.trace, 0);
     const int panel = blockIdx.x / cs;
     const int n0 = panel * kSmallBNW;
     const int k_tiles = (args.K + kBK - 1) / kBK;
     const int n_local = (args.n_seg > static_cast<int>(rank)) ? (args.n_seg - 1 - static_cast<int>(rank)) / static_cast<int>(cs) + 1 : 0;
+    // local k-tiles, flattened: t -> slot j = t / 8, k-tile (rank + j*cs) * 8 + t % 8; only the last segment
+    // of K can be short, and it is the last slot of the rank that owns it
+    int n_t = 0;
+    if (n_local > 0) {
+        const int last_seg = static_cast<int>(rank) + (n_local - 1) * static_cast<int>(cs);
+        n_t = (n_local - 1) * kTilesPerSeg + (min(k_tiles, (last_seg + 1) * kTilesPerSeg) - last_seg * kTilesPerSeg);
+    }
+    // ranks that finish at least one token row (rank r owns rows [r * rows_per_rank, (r + 1) * rows_per_rank))
+    const int owners = cs > 1 ? (args.M + args.rows_per_rank - 1) / args.rows_per_rank : 1;
 
     if (warp == 0 && lane == 0) {
-        tma_prefetch_desc(&tm_x_hi);
-        if (Cfg::A_PLANES == 2) tma_prefetch_desc(&tm_x_lo);
+        if (!FUSED) {
+            tma_prefetch_desc(&tm_x_hi);
+            if (Cfg::A_PLANES == 2) tma_prefetch_desc(&tm_x_lo);
+        }
         tma_prefetch_desc(&tm_w_hi);
         if (Cfg::B_PLANES == 2) tma_prefetch_desc(&tm_w_lo);
         for (int s = 0; s < STAGES; ++s) {
             mbar_init(full_bar(s), 1);
             mbar_init(empty_bar(s), 1);
+            mbar_init(xfull_bar(s), 4);                  // one arrival per converter warp
         }
         mbar_init(done_bar, 1);
+        mbar_init(red_bar, cs * 4);                      // one arrival per epilogue warp of every rank
         fence_mbar_init();
     }
     if (warp == 1) {
         tmem_alloc(tmem_slot, static_cast<uint32_t>(args.tmem_cols));
         tmem_relinquish();
+        if (lane == 0) HEAL_STAMP(args.trace, 13);
+    }
+    if (FUSED) {
+        // token rows >= M of the operand tiles are never written by the converters: zero them once
+        for (int s = 0; s < STAGES; ++s) {
+            const uint32_t sx = smem_base + s * Cfg::STAGE_BYTES + Cfg::W_BYTES;
+            for (int o = threadIdx.x * 16; o < Cfg::A_PLANES * Cfg::X_TILE_AL; o += kSmallThreads * 16)
+                asm volatile("st.shared.v4.b32 [%0], {%1, %1, %1, %1};" ::"r"(sx + o), "r"(0u) : "memory");
+        }
+        fence_proxy_async_smem();
     }
     tc_fence_before();
     __syncthreads();
+    if (threadIdx.x == 0) HEAL_STAMP(args.trace, 12);
+    if (cs > 1) cluster_arrive();                        // matched by cluster_wait() before the first remote access
     tc_fence_after();
     const uint32_t tmem_base = *tmem_slot_ptr;
-    pdl_wait();                       // everything above overlapped the previous kernel's tail
-    pdl_launch_dependents();
+    if (threadIdx.x == 0) HEAL_STAMP(args.trace, 1);
+    const bool early_w = args.b_static != 0 && warp == 0;
+    if (!early_w) {
+        pdl_wait();                   // everything above overlapped the previous kernel's tail
+        pdl_launch_dependents();      // the next kernel may start its prologue (and, with static weights, its W stream)
+    }
+    if (threadIdx.x == 32) HEAL_STAMP(args.trace, 2);
 
     if (warp == 0) {
         // ================================ TMA producer ================================
         if (lane == 0) {
             const uint64_t pol_w = l2_policy_evict_first();      // weights are streamed once
-            int stage = 0;
-            uint32_t phase = 0;
-            for (int j = 0; j < n_local; ++j) {
-                const int seg = static_cast<int>(rank) + j * static_cast<int>(cs);
-                const int kt_end = min(k_tiles, (seg + 1) * kTilesPerSeg);
-                for (int kt = seg * kTilesPerSeg; kt < kt_end; ++kt) {
-                    mbar_wait(empty_bar(stage), phase ^ 1u, args.diag, 500 + stage);
-                    const uint32_t sb = smem_base + stage * Cfg::STAGE_BYTES;
-                    const uint32_t fb = full_bar(stage);
-                    mbar_arrive_expect_tx(fb, Cfg::B_PLANES * Cfg::W_TILE + Cfg::A_PLANES * Cfg::X_TILE);
-                    const int k0 = kt * kBK;
-                    if (Cfg::B_MN) {
+            auto load_w = [&](int t, uint32_t sb, uint32_t fb) {
+                const int k0 = ((static_cast<int>(rank) + (t >> 3) * static_cast<int>(cs)) * kTilesPerSeg + (t & 7)) * kBK;
+                if (Cfg::B_MN) {
 #pragma unroll
-                        for (int c = 0; c < 2; ++c) {
-                            tma_load_2d_hint(sb + c * 8192, &tm_w_hi, fb, n0 + c * 64, k0, pol_w);
-                            if (Cfg::B_PLANES == 2)
-                                tma_load_2d_hint(sb + Cfg::W_TILE + c * 8192, &tm_w_lo, fb, n0 + c * 64, k0, pol_w);
-                        }
-                    } else {
-                        tma_load_2d_hint(sb, &tm_w_hi, fb, k0, n0, pol_w);
-                        if (Cfg::B_PLANES == 2) tma_load_2d_hint(sb + Cfg::W_TILE, &tm_w_lo, fb, k0, n0, pol_w);
+                    for (int c = 0; c < 2; ++c) {
+                        tma_load_2d_hint(sb + c * 8192, &tm_w_hi, fb, n0 + c * 64, k0, pol_w);
+                        if (Cfg::B_PLANES == 2)
+                            tma_load_2d_hint(sb + Cfg::W_TILE + c * 8192, &tm_w_lo, fb, n0 + c * 64, k0, pol_w);
                     }
-                    const uint32_t sx = sb + Cfg::B_PLANES * Cfg::W_TILE;
-                    tma_load_2d(sx, &tm_x_hi, fb, k0, 0);
-                    if (Cfg::A_PLANES == 2) tma_load_2d(sx + Cfg::X_TILE_AL, &tm_x_lo, fb, k0, 0);
-                    if (++stage == STAGES) { stage = 0; phase ^= 1u; }
+                } else {
+                    tma_load_2d_hint(sb, &tm_w_hi, fb, k0, n0, pol_w);
+                    if (Cfg::B_PLANES == 2) tma_load_2d_hint(sb + Cfg::W_TILE, &tm_w_lo, fb, k0, n0, pol_w);
                 }
+            };
+            auto load_x = [&](int t, uint32_t sb, uint32_t fb) {
+                const int k0 = ((static_cast<int>(rank) + (t >> 3) * static_cast<int>(cs)) * kTilesPerSeg + (t & 7)) * kBK;
+                const uint32_t sx = sb + Cfg::W_BYTES;
+                tma_load_2d(sx, &tm_x_hi, fb, k0, 0);
+                if (Cfg::A_PLANES == 2) tma_load_2d(sx + Cfg::X_TILE_AL, &tm_x_lo, fb, k0, 0);
+            };
+            int stage = 0, t = 0;
+            uint32_t phase = 0;
+            if (early_w && !FUSED) {
+                // static weights: fill the pipeline with W tiles now, add the activation tiles once the
+                // stream predecessor (which may have produced them) has completed
+                const int pre = min(STAGES, n_t);
+                for (int s = 0; s < pre; ++s) {
+                    mbar_arrive_expect_tx(full_bar(s), Cfg::TX_BYTES);
+                    load_w(s, smem_base + s * Cfg::STAGE_BYTES, full_bar(s));
+                }
+                HEAL_STAMP(args.trace, 3);
+                pdl_wait();
+                for (int s = 0; s < pre; ++s) load_x(s, smem_base + s * Cfg::STAGE_BYTES, full_bar(s));
+                t = pre;
+                if (pre == STAGES) phase = 1u; else stage = pre;
             }
+            for (; t < n_t; ++t) {
+                mbar_wait(empty_bar(stage), phase ^ 1u, args.diag, 500 + stage);
+                const uint32_t sb = smem_base + stage * Cfg::STAGE_BYTES;
+                const uint32_t fb = full_bar(stage);
+                mbar_arrive_expect_tx(fb, Cfg::TX_BYTES);
+                load_w(t, sb, fb);
+                if (!FUSED) load_x(t, sb, fb);
+                if (t == 0) HEAL_STAMP(args.trace, 3);
+                if (++stage == STAGES) { stage = 0; phase ^= 1u; }
+            }
+        }
+        if (cs > 1 && args.red_alias) {
+            __syncwarp();
+            mbar_wait(done_bar, 0, args.diag, 701);
+            cluster_wait();
+            cluster_arrive();
         }
     } else if (warp == 1) {
         // ================================ MMA issuer ==================================
@@ -152,48 +230,121 @@ heal_gemm_smallm_kernel(const __grid_constant__ CUtensorMap tm_x_hi, const __gri
             constexpr uint32_t x_step = 32 >> 4;
             int stage = 0;
             uint32_t phase = 0;
-            for (int j = 0; j < n_local; ++j) {
-                const int seg = static_cast<int>(rank) + j * static_cast<int>(cs);
-                const int kt_end = min(k_tiles, (seg + 1) * kTilesPerSeg);
-                const uint32_t d_tmem = tmem_base + static_cast<uint32_t>(j * MPAD);
-                uint32_t accumulate = 0;
-                for (int kt = seg * kTilesPerSeg; kt < kt_end; ++kt) {
-                    mbar_wait(full_bar(stage), phase, args.diag, 600 + stage);
-                    tc_fence_after();
-                    const uint32_t sb = smem_base + stage * Cfg::STAGE_BYTES;
-                    const uint64_t w_hi = wdesc0 | desc_addr(sb);
-                    const uint64_t w_lo = wdesc0 | desc_addr(sb + Cfg::W_TILE);
-                    const uint32_t sx = sb + Cfg::B_PLANES * Cfg::W_TILE;
-                    const uint64_t x_hi = kdesc0 | desc_addr(sx);
-                    const uint64_t x_lo = kdesc0 | ((sx + Cfg::X_TILE_AL) >> 4);
+            uint32_t accumulate = 0;
+            for (int t = 0; t < n_t; ++t) {
+                if ((t & 7) == 0) accumulate = 0;                 // new segment -> new TMEM slot
+                const uint32_t d_tmem = tmem_base + static_cast<uint32_t>((t >> 3) * MPAD);
+                mbar_wait(full_bar(stage), phase, args.diag, 600 + stage);
+                if (FUSED) mbar_wait(xfull_bar(stage), phase, args.diag, 620 + stage);
+                tc_fence_after();
+                if (t == 0) HEAL_STAMP(args.trace, 4);
+                if (t == n_t - 1) HEAL_STAMP(args.trace, 5);
+                const uint32_t sb = smem_base + stage * Cfg::STAGE_BYTES;
+                const uint64_t w_hi = wdesc0 | desc_addr(sb);
+                const uint64_t w_lo = wdesc0 | desc_addr(sb + Cfg::W_TILE);
+                const uint32_t sx = sb + Cfg::W_BYTES;
+                const uint64_t x_hi = kdesc0 | desc_addr(sx);
+                const uint64_t x_lo = kdesc0 | desc_addr(sx + Cfg::X_TILE_AL);
 #pragma unroll
-                    for (int q = 0; q < kBK / 16; ++q) {
-                        const uint64_t wo = static_cast<uint64_t>(q * w_step), xo = static_cast<uint64_t>(q * x_step);
-                        // product order as in the large-M kernel: a_hi.b_hi, a_hi.b_lo, a_lo.b_hi, a_lo.b_lo
-                        umma_f16(d_tmem, w_hi + wo, x_hi + xo, idesc, accumulate);
-                        accumulate = 1;
-                        if (NPROD == 2) umma_f16(d_tmem, w_hi + wo, x_lo + xo, idesc, 1);
-                        if (NPROD >= 3) {
-                            umma_f16(d_tmem, w_lo + wo, x_hi + xo, idesc, 1);
-                            umma_f16(d_tmem, w_hi + wo, x_lo + xo, idesc, 1);
-                        }
-                        if (NPROD == 4) umma_f16(d_tmem, w_lo + wo, x_lo + xo, idesc, 1);
+                for (int q = 0; q < kBK / 16; ++q) {
+                    const uint64_t wo = static_cast<uint64_t>(q * w_step), xo = static_cast<uint64_t>(q * x_step);
+                    // product order as in the large-M kernel: a_hi.b_hi, a_hi.b_lo, a_lo.b_hi, a_lo.b_lo
+                    umma_f16(d_tmem, w_hi + wo, x_hi + xo, idesc, accumulate);
+                    accumulate = 1;
+                    if (NPROD == 2) umma_f16(d_tmem, w_hi + wo, x_lo + xo, idesc, 1);
+                    if (NPROD >= 3) {
+                        umma_f16(d_tmem, w_lo + wo, x_hi + xo, idesc, 1);
+                        umma_f16(d_tmem, w_hi + wo, x_lo + xo, idesc, 1);
                     }
-                    umma_commit(empty_bar(stage));
-                    if (++stage == STAGES) { stage = 0; phase ^= 1u; }
+                    if (NPROD == 4) umma_f16(d_tmem, w_lo + wo, x_lo + xo, idesc, 1);
                 }
+                umma_commit(empty_bar(stage));
+                if (++stage == STAGES) { stage = 0; phase ^= 1u; }
             }
             umma_commit(done_bar);                         // all local segments complete in TMEM
         }
+        if (cs > 1 && args.red_alias) {
+            __syncwarp();
+            mbar_wait(done_bar, 0, args.diag, 702);
+            cluster_wait();
+            cluster_arrive();
+        }
     } else {
-        // ================================ epilogue: TMEM -> staging ======================
+        const int et = threadIdx.x - 64;                   // 0..127 among the converter / epilogue threads
+        if (FUSED) {
+            // ============================ step S: FP32 activations -> hi/lo operand tiles ==========
+            // Thread `et` owns 16-byte chunk c = et % 8 (k = 8c..8c+7 of the k-tile) of token rows
+            // et/8, et/8 + 16, ...; K-major 128B-swizzled tile: row m at (m/8)*1024 + (m%8)*128, chunk c
+            // stored at position c ^ (m%8).
+            constexpr int TASKS = Cfg::TASKS, PF = Cfg::PF;
+            const int c = et & 7, r0 = et >> 3;
+            float4 buf[PF][TASKS][2];
+            auto fetch = [&](int t, float4 (&dst)[TASKS][2]) {
+                const int k = ((static_cast<int>(rank) + (t >> 3) * static_cast<int>(cs)) * kTilesPerSeg + (t & 7)) * kBK + c * 8;
+#pragma unroll
+                for (int q = 0; q < TASKS; ++q) {
+                    const int m = r0 + q * 16;
+                    dst[q][0] = dst[q][1] = make_float4(0.f, 0.f, 0.f, 0.f);
+                    if (m < args.M) {
+                        const float *src = args.A + static_cast<int64_t>(m) * args.lda + k;
+                        if (k + 8 <= args.K) {
+                            dst[q][0] = __ldg(reinterpret_cast<const float4 *>(src));
+                            dst[q][1] = __ldg(reinterpret_cast<const float4 *>(src) + 1);
+                        } else {
+                            float v[8];
+#pragma unroll
+                            for (int i = 0; i < 8; ++i) v[i] = (k + i < args.K) ? __ldg(src + i) : 0.f;
+                            dst[q][0] = make_float4(v[0], v[1], v[2], v[3]);
+                            dst[q][1] = make_float4(v[4], v[5], v[6], v[7]);
+                        }
+                    }
+                }
+            };
+#pragma unroll
+            for (int p = 0; p < PF; ++p)
+                if (p < n_t) fetch(p, buf[p]);
+            int stage = 0;
+            uint32_t phase = 0;
+            for (int t0 = 0; t0 < n_t; t0 += PF) {
+#pragma unroll
+                for (int p = 0; p < PF; ++p) {
+                    const int t = t0 + p;
+                    if (t < n_t) {
+                        mbar_wait(empty_bar(stage), phase ^ 1u, args.diag, 540 + stage);
+                        const uint32_t sx = smem_base + stage * Cfg::STAGE_BYTES + Cfg::W_BYTES;
+#pragma unroll
+                        for (int q = 0; q < TASKS; ++q) {
+                            const int m = r0 + q * 16;
+                            if (m < args.M) {
+                                uint4 h, l;
+                                split2(buf[p][q][0].x, buf[p][q][0].y, h.x, l.x);
+                                split2(buf[p][q][0].z, buf[p][q][0].w, h.y, l.y);
+                                split2(buf[p][q][1].x, buf[p][q][1].y, h.z, l.z);
+                                split2(buf[p][q][1].z, buf[p][q][1].w, h.w, l.w);
+                                const uint32_t off = static_cast<uint32_t>((m >> 3) * 1024 + (m & 7) * 128 + ((c ^ (m & 7)) << 4));
+                                asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(sx + off), "r"(h.x), "r"(h.y), "r"(h.z), "r"(h.w) : "memory");
+                                if (Cfg::A_PLANES == 2)
+                                    asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(sx + Cfg::X_TILE_AL + off), "r"(l.x), "r"(l.y), "r"(l.z), "r"(l.w) : "memory");
+                            }
+                        }
+                        fence_proxy_async_smem();           // generic-proxy writes -> visible to the tensor core
+                        __syncwarp();
+                        if (lane == 0) mbar_arrive(xfull_bar(stage));
+                        if (t + PF < n_t) fetch(t + PF, buf[p]);
+                        if (++stage == STAGES) { stage = 0; phase ^= 1u; }
+                    }
+                }
+            }
+        }
+        // ================================ epilogue ====================================
         const int quad = warp & 3;
         const int nl = quad * 32 + lane;                   // weight column within the panel = TMEM lane
+        const int col = n0 + nl;
         mbar_wait(done_bar, 0, args.diag, 700);
         tc_fence_after();
+        if (et == 0) HEAL_STAMP(args.trace, 6);
         if (cs == 1) {
             // single-CTA panel: all segments are local slots; sum them in ascending order in registers
-            const int col = n0 + nl;
 #pragma unroll
             for (int c = 0; c < MPAD / 16; ++c) {
                 if (c * 16 < args.M) {
@@ -217,52 +368,97 @@ heal_gemm_smallm_kernel(const __grid_constant__ CUtensorMap tm_x_hi, const __gri
                     }
                 }
             }
+            tc_fence_before();
         } else {
-            // the pipeline buffers are dead now (every TMA load has been consumed by a completed MMA)
+            cluster_wait();                                // every rank's red_bar is initialised
+            if (args.red_alias) {                          // ... and every rank's pipeline buffers are dead
+                cluster_arrive();
+                cluster_wait();
+            }
+            // push this rank's partials: token m -> rank m / rpr, float (seg * 128 + nl) * rpr + m % rpr of its
+            // red area (the rpr values a thread sends for one segment are contiguous: vector stores)
+            const int rpr = args.rows_per_rank;
             for (int j = 0; j < n_local; ++j) {
+                const int seg = static_cast<int>(rank) + j * static_cast<int>(cs);
+                const uint32_t row_off = static_cast<uint32_t>((seg * kSmallBNW + nl) * rpr) * 4u;
 #pragma unroll
                 for (int c = 0; c < MPAD / 16; ++c) {
-                    uint32_t v[16];
-                    tmem_ld_32x32b_x16(tmem_base + (static_cast<uint32_t>(quad * 32) << 16) + static_cast<uint32_t>(j * MPAD + c * 16), v);
-                    tmem_ld_wait();
+                    if (c * 16 < args.M) {
+                        uint32_t v[16];
+                        tmem_ld_32x32b_x16(tmem_base + (static_cast<uint32_t>(quad * 32) << 16) + static_cast<uint32_t>(j * MPAD + c * 16), v);
+                        tmem_ld_wait();
+                        if ((rpr & 3) == 0) {
 #pragma unroll
-                    for (int i = 0; i < 16; ++i) {
-                        const uint32_t off = (static_cast<uint32_t>(j * MPAD + c * 16 + i) * kSmallBNW + nl) * 4u;
-                        asm volatile("st.shared.b32 [%0], %1;" ::"r"(smem_base + off), "r"(v[i]) : "memory");
+                            for (int i = 0; i < 16; i += 4) {
+                                const int m = c * 16 + i;
+                                if (m < args.M) {         // m % 4 == 0 and rpr % 4 == 0: rows m..m+3 have one owner (rows >= M: unused zeros)
+                                    const uint32_t dst = static_cast<uint32_t>(m / rpr), ml = static_cast<uint32_t>(m % rpr);
+                                    st_dsmem_v4(map_to_cta(red_base + row_off + ml * 4u, dst), v[i], v[i + 1], v[i + 2], v[i + 3]);
+                                }
+                            }
+                        } else {
+#pragma unroll
+                            for (int i = 0; i < 16; ++i) {
+                                const int m = c * 16 + i;
+                                if (m < args.M) {
+                                    const uint32_t dst = static_cast<uint32_t>(m / rpr), ml = static_cast<uint32_t>(m % rpr);
+                                    st_dsmem_b32(map_to_cta(red_base + row_off + ml * 4u, dst), v[i]);
+                                }
+                            }
+                        }
                     }
                 }
             }
-        }
-        tc_fence_before();
-    }
-
-    if (cs > 1) {
-        // ---- every CTA's segment partials are staged: reduce over the cluster in ascending segment order
-        __syncwarp();
-        cluster_sync_all();
-        if (warp >= 2) {
-            const int nl = (warp & 3) * 32 + lane;
-            const int col = n0 + nl;
-            for (int m = static_cast<int>(rank); m < args.M; m += static_cast<int>(cs)) {
-                float acc = 0.f;
-#pragma unroll 8
-                for (int s = 0; s < args.n_seg; ++s) {
-                    const uint32_t src = static_cast<uint32_t>(s) % cs, slot = static_cast<uint32_t>(s) / cs;
-                    const uint32_t off = ((slot * MPAD + static_cast<uint32_t>(m)) * kSmallBNW + nl) * 4u;
-                    const float v = ld_dsmem_f32(map_to_cta(smem_base + off, src));
-                    acc = (s == 0) ? v : __fadd_rn(acc, v);
+            tc_fence_before();
+            fence_acq_rel_cluster();
+            __syncwarp();
+            if (lane < owners) mbar_arrive_cluster(map_to_cta(red_bar, static_cast<uint32_t>(lane)));
+            if (et == 0) HEAL_STAMP(args.trace, 7);
+            if (static_cast<int>(rank) < owners) {
+                mbar_wait_cluster(red_bar, 0, args.diag, 710);
+                if (et == 0) HEAL_STAMP(args.trace, 8);
+                // this rank finishes rows [rank * rpr, min(M, (rank + 1) * rpr)): ascending segment order, FP32 RN
+                const float *red = reinterpret_cast<const float *>(smem_raw + (red_base - smem_u32(smem_raw)));
+                const int m_lo = static_cast<int>(rank) * rpr;
+                const int rows = min(rpr, args.M - m_lo);
+                const int seg_stride = kSmallBNW * rpr;
+                if ((rpr & 3) == 0) {
+                    for (int r4 = 0; r4 < rows; r4 += 4) {
+                        const float4 *src = reinterpret_cast<const float4 *>(red + nl * rpr + r4);
+                        float4 acc = src[0];
+#pragma unroll 4
+                        for (int s = 1; s < args.n_seg; ++s) {
+                            const float4 v = src[static_cast<size_t>(s) * (seg_stride / 4)];
+                            acc.x = __fadd_rn(acc.x, v.x); acc.y = __fadd_rn(acc.y, v.y);
+                            acc.z = __fadd_rn(acc.z, v.z); acc.w = __fadd_rn(acc.w, v.w);
+                        }
+                        if (col < args.N) {
+                            float *dst = args.C + static_cast<int64_t>(m_lo + r4) * args.ldc + col;
+                            dst[0] = acc.x;
+                            if (r4 + 1 < rows) dst[args.ldc] = acc.y;
+                            if (r4 + 2 < rows) dst[2 * args.ldc] = acc.z;
+                            if (r4 + 3 < rows) dst[3 * args.ldc] = acc.w;
+                        }
+                    }
+                } else {
+                    for (int r = 0; r < rows; ++r) {
+                        const float *src = red + nl * rpr + r;
+                        float acc = src[0];
+#pragma unroll 4
+                        for (int s = 1; s < args.n_seg; ++s) acc = __fadd_rn(acc, src[static_cast<size_t>(s) * seg_stride]);
+                        if (col < args.N) args.C[static_cast<int64_t>(m_lo + r) * args.ldc + col] = acc;
+                    }
                 }
-                if (col < args.N) args.C[static_cast<int64_t>(m) * args.ldc + col] = acc;
+                if (et == 0) HEAL_STAMP(args.trace, 9);
             }
         }
-        __syncwarp();
-        cluster_sync_all();                                 // nobody leaves while its smem is being read
-    } else {
-        __syncthreads();
     }
+
+    __syncthreads();
     if (warp == 1) {
         tc_fence_after();
         tmem_dealloc(tmem_base, static_cast<uint32_t>(args.tmem_cols));
+        if (lane == 0) HEAL_STAMP(args.trace, 11);
     }
 }
 

@@ -28,6 +28,16 @@ __device__ __forceinline__ uint64_t globaltimer_ns()
     return t;
 }
 
+// ---- optional phase trace (builds with -DHEAL_TRACE only; the product library compiles it out)
+#ifdef HEAL_TRACE
+#define HEAL_STAMP(tr, slot)                                                              \
+    do {                                                                                  \
+        if (tr) (tr)[static_cast<size_t>(blockIdx.x) * 64 + (slot)] = heal::globaltimer_ns(); \
+    } while (0)
+#else
+#define HEAL_STAMP(tr, slot) do { } while (0)
+#endif
+
 // ---- programmatic dependent launch: lets this grid's prologue overlap the previous grid's tail.
 // pdl_wait() must precede the first global-memory access; it returns once every prerequisite grid has
 // completed and its writes are visible (a no-op when the launch carries no programmatic dependency).
@@ -241,6 +251,55 @@ __device__ __forceinline__ void cluster_sync_all()
 {
     asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
 }
+
+// ---- distributed shared memory (cluster) ---------------------------------------------------------
+__device__ __forceinline__ uint32_t map_to_cta(uint32_t saddr, uint32_t rank)
+{
+    uint32_t r;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(saddr), "r"(rank));
+    return r;
+}
+__device__ __forceinline__ void st_dsmem_b32(uint32_t addr, uint32_t v)
+{
+    asm volatile("st.shared::cluster.b32 [%0], %1;" ::"r"(addr), "r"(v) : "memory");
+}
+__device__ __forceinline__ void st_dsmem_v4(uint32_t addr, uint32_t a, uint32_t b, uint32_t c, uint32_t d)
+{
+    asm volatile("st.shared::cluster.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(a), "r"(b), "r"(c), "r"(d) : "memory");
+}
+__device__ __forceinline__ void fence_acq_rel_cluster() { asm volatile("fence.acq_rel.cluster;" ::: "memory"); }
+// generic-proxy shared-memory writes -> visible to the async proxy (TMA / tcgen05 operand reads)
+__device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+// wait with cluster-scope acquire: pairs with mbar_arrive_cluster (release.cluster) from other CTAs
+__device__ __forceinline__ void mbar_wait_cluster(uint32_t bar, uint32_t parity, int *diag, int code)
+{
+    const uint64_t t0 = globaltimer_ns();
+    uint32_t spins = 0;
+    for (;;) {
+        uint32_t ok;
+        asm volatile(
+            "{\n\t.reg .pred p;\n\t"
+            "mbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 p, [%1], %2;\n\t"
+            "selp.u32 %0, 1, 0, p;\n\t}"
+            : "=r"(ok)
+            : "r"(bar), "r"(parity)
+            : "memory");
+        if (ok) return;
+        if ((++spins & 0x3ffu) == 0 && globaltimer_ns() - t0 > 4000000000ull) {
+            if (diag) {
+                diag[0] = code;
+                diag[1] = static_cast<int>(blockIdx.x);
+                diag[2] = static_cast<int>(parity);
+            }
+            __threadfence_system();
+            __trap();
+        }
+    }
+}
+
+// split cluster barrier: every thread of every CTA arrives once; only the threads that need the guarantee wait
+__device__ __forceinline__ void cluster_arrive() { asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory"); }
+__device__ __forceinline__ void cluster_wait() { asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory"); }
 
 // ---- descriptors (PTX ISA tcgen05 "matrix descriptor" / "instruction descriptor") -----------
 // Shared-memory matrix descriptor, 128-byte swizzle:

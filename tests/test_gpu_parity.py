@@ -320,6 +320,78 @@ def test_kernel_families_bit_identical(hb, inputs, M, N, K, nprod, b_nk):
     assert torch.equal(outs[0], outs[1]) and torch.equal(outs[0], outs[2])
 
 
+@pytest.mark.parametrize("M,N,K,b_nk", [(1, 4096, 4096, False), (8, 1032, 4096, False), (16, 520, 14336, False), (13, 264, 1000, True),
+                                        (5, 4096, 520, True), (16, 128, 8192, False)])
+def test_fused_split_small_m_bit_identical(hb, oracle, inputs, M, N, K, b_nk):
+    """M <= 16 with FP16 weights: heal_gemm splits the activations inside the GEMM kernel (no planes, one launch).
+    Same bits as the split kernel + planes kernel, with and without HEAL_B_STATIC, and within the gate of the oracle."""
+    A = inputs.activations(M, K, seed=11, outliers=True)
+    W = inputs.weights_f16(K, N, seed=11, nk=b_nk)
+    Ad, Wd = dev_padded(A, 4), dev(W)
+    mode = 2 | (hb.B_NK if b_nk else 0)
+    n0 = hb.launch_count()
+    fused = hb.heal_gemm(Ad, Wd, mode)
+    assert hb.launch_count() - n0 == 1                         # one kernel: no split launch
+    ah, al = hb.heal_split(Ad)
+    planes = hb.heal_gemm_presplit(ah, al, Wd, None, mode)
+    assert torch.equal(fused, planes)
+    assert torch.equal(hb.heal_gemm(Ad, Wd, mode | hb.B_STATIC), planes)
+    assert torch.equal(hb.heal_gemm_presplit(ah, al, Wd, None, mode | hb.B_STATIC), planes)
+    for nprod in (1,):                                         # the one-product (HEAL-Base) GEMM takes the same path
+        assert torch.equal(hb.heal_gemm(Ad, Wd, nprod | (mode & ~0xF)), hb.heal_gemm_presplit(ah, None, Wd, None, nprod | (mode & ~0xF)))
+    try:
+        hb.debug_force_kernel(1)                               # large-M kernels on the same inputs
+        assert torch.equal(hb.heal_gemm(Ad, Wd, mode), planes)
+    finally:
+        hb.debug_force_kernel(0)
+    ref = oracle.gemm_f64(A, W, b_nk=b_nk)
+    assert oracle.normwise_error(fused.cpu().numpy(), ref, A, W) <= GATE
+
+
+@pytest.mark.parametrize("M,N,K", [(64, 4096, 4096), (64, 1032, 14336), (33, 520, 16384), (48, 264, 30000 // 8 * 8)])
+def test_small_m_large_reduction_area_bit_identical(hb, inputs, M, N, K):
+    """Large M * K in the small-M kernel: the partial sums pushed over the cluster overlay the pipeline buffers
+    (second cluster barrier).  Same bits as the large-M kernels."""
+    A = dev(inputs.activations(M, K, seed=12, outliers=True))
+    W = dev(inputs.weights_f16(K, N, seed=12))
+    outs = []
+    try:
+        for which in (0, 1):
+            hb.debug_force_kernel(which)
+            outs.append(hb.heal_gemm(A, W, 2).clone())
+    finally:
+        hb.debug_force_kernel(0)
+    assert torch.equal(outs[0], outs[1])
+
+
+def test_static_weights_graph_chain(hb, inputs):
+    """HEAL_B_STATIC in a captured chain of decode GEMMs (each kernel streams its weights while its predecessor
+    finishes; activations and C wait): every replay reproduces the eager results bit for bit, including a chain
+    where each GEMM consumes the previous one's output."""
+    K = N = 1024
+    x0 = dev(inputs.activations(8, K, seed=13, outliers=True))
+    Ws = [dev(inputs.weights_f16(K, N, seed=20 + i)) for i in range(4)]
+    ref = x0
+    for W in Ws:
+        ref = hb.heal_gemm(ref, W, 2)
+    bufs = [torch.zeros(8, N, device="cuda") for _ in Ws]
+    s = torch.cuda.Stream()
+    torch.cuda.synchronize()
+    with torch.cuda.stream(s):
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=s):
+            x = x0
+            for W, buf in zip(Ws, bufs):
+                hb.heal_gemm(x, W, 2 | hb.B_STATIC, C=buf)
+                x = buf
+        for _ in range(5):
+            for b in bufs:
+                b.zero_()
+            g.replay()
+            s.synchronize()
+            assert torch.equal(bufs[-1], ref)
+
+
 def test_balanced_schedule_graph_replay_and_two_streams(hb, inputs):
     """A shape whose tiles do not divide over the SMs (segment-granular hand-off between CTAs): replaying a
     captured CUDA graph and running on two streams at once must reproduce the eager result bit for bit."""
@@ -391,12 +463,16 @@ def test_error_codes(hb):
     assert raw(8, 16, 64, a, 64, w, 16, c, 16, 0) == 4
     assert raw(8, 16, 64, a, 64, w, 16, c, 16, 0x102) == 4
     assert raw(8, 16, 64, a, 64, w, 16, c, 16, 2) == 0
+    # M > 16 needs hi/lo planes in the workspace (M <= 16 with FP16 weights splits inside the GEMM kernel)
+    A2 = torch.zeros((32, 64), device="cuda")
+    C2 = torch.zeros((32, 16), device="cuda")
     ws = torch.zeros(256, dtype=torch.uint8, device="cuda")
     hb.set_workspace(ws)
-    assert raw(8, 16, 64, a, 64, w, 16, c, 16, 2) == 6                 # supplied workspace too small
-    big = torch.zeros(hb.workspace_size(8, 16, 64, 2), dtype=torch.uint8, device="cuda")
+    assert raw(32, 16, 64, A2.data_ptr(), 64, w, 16, C2.data_ptr(), 16, 2) == 6       # supplied workspace too small
+    assert raw(8, 16, 64, a, 64, w, 16, c, 16, 2) == 0                               # fused path: no workspace needed
+    big = torch.zeros(hb.workspace_size(32, 16, 64, 2), dtype=torch.uint8, device="cuda")
     hb.set_workspace(big)
-    assert raw(8, 16, 64, a, 64, w, 16, c, 16, 2) == 0
+    assert raw(32, 16, 64, A2.data_ptr(), 64, w, 16, C2.data_ptr(), 16, 2) == 0
     hb.set_workspace(None)
     torch.cuda.synchronize()
 
