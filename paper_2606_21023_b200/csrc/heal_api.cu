@@ -38,6 +38,10 @@ struct State {
         bool used = false;
         float *xfer = nullptr;     // per-CTA running-sum slots (128 x 256 floats each)
         uint32_t *flags = nullptr; // per-CTA flag: 1 = slot written, reset by the consumer
+        uint64_t last_use = 0;     // for recycling the least recently used slot when all 8 are taken
+        float *part = nullptr;     // ordered split-K: segment partials, grown on demand (never while capturing)
+        size_t part_bytes = 0;
+        uint32_t *cnt = nullptr;   // ordered split-K: two counters per (tile, rank), all zero between launches
     };
     Xfer xf[8];
     // workspace
@@ -160,58 +164,112 @@ int launch_split(int64_t rows, int64_t cols, const float *X, int64_t ldx, __half
     return HEAL_OK;
 }
 
-// Hand-off buffers for `stream`: created on first use (19 MB per stream, at most 8 streams; further
-// streams simply run the unbalanced schedule, which gives the same bits).
-bool bind_xfer(GemmArgs &args, cudaStream_t stream)
+// Hand-off buffers for `stream`: created on first use (19 MB per stream + the split-K partial area, grown on
+// demand); 8 slots, the least recently used one is recycled (after a device synchronise) when a ninth stream
+// shows up.  During stream capture nothing is allocated: an unbound stream runs the unbalanced schedule (same bits).
+bool bind_xfer(GemmArgs &args, cudaStream_t stream, size_t part_bytes = 0)
 {
     std::lock_guard<std::mutex> lk(g_xf_mu);
     State::Xfer *slot = nullptr;
     for (auto &x : g.xf)
         if (x.used && x.stream == stream) { slot = &x; break; }
+    cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+    const bool capturing = cudaStreamIsCapturing(stream, &cap) != cudaSuccess || cap != cudaStreamCaptureStatusNone;
+    static uint64_t tick = 0;
+    if (!slot && !capturing) {
+        // all slots taken (streams come and go): recycle the least recently used one once the device is idle
+        bool any_free = false;
+        for (auto &x : g.xf) any_free = any_free || !x.used;
+        if (!any_free && cudaDeviceSynchronize() == cudaSuccess) {
+            State::Xfer *lru = &g.xf[0];
+            for (auto &x : g.xf)
+                if (x.last_use < lru->last_use) lru = &x;
+            lru->stream = stream;
+            slot = lru;
+        }
+    }
     if (!slot) {
         for (auto &x : g.xf)
             if (!x.used) { slot = &x; break; }
-        if (!slot) return false;
-        cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
-        if (cudaStreamIsCapturing(stream, &cap) != cudaSuccess || cap != cudaStreamCaptureStatusNone) return false;
+        if (!slot || capturing) return false;
         float *xf = nullptr;
-        uint32_t *fl = nullptr;
+        uint32_t *fl = nullptr, *cn = nullptr;
+        const size_t cnt_bytes = static_cast<size_t>(g.num_sms) * 4 * sizeof(uint32_t);
         if (cudaMalloc(&xf, static_cast<size_t>(g.num_sms) * kBM * 256 * sizeof(float)) != cudaSuccess) return false;
         if (cudaMalloc(&fl, static_cast<size_t>(g.num_sms) * sizeof(uint32_t)) != cudaSuccess ||
-            cudaMemset(fl, 0, static_cast<size_t>(g.num_sms) * sizeof(uint32_t)) != cudaSuccess) {
+            cudaMemset(fl, 0, static_cast<size_t>(g.num_sms) * sizeof(uint32_t)) != cudaSuccess ||
+            cudaMalloc(&cn, cnt_bytes) != cudaSuccess || cudaMemset(cn, 0, cnt_bytes) != cudaSuccess) {
             cudaFree(xf);
             if (fl) cudaFree(fl);
+            if (cn) cudaFree(cn);
             return false;
         }
         slot->stream = stream;
         slot->used = true;
         slot->xfer = xf;
         slot->flags = fl;
+        slot->cnt = cn;
     }
+    if (part_bytes > slot->part_bytes) {
+        // grow the partial-sum area: the stream may still be using the old one, so wait for it first
+        if (capturing || cudaStreamSynchronize(stream) != cudaSuccess) return false;
+        if (slot->part) cudaFree(slot->part);
+        slot->part = nullptr;
+        slot->part_bytes = 0;
+        if (cudaMalloc(&slot->part, part_bytes) != cudaSuccess) return false;
+        slot->part_bytes = part_bytes;
+    }
+    slot->last_use = ++tick;
     args.xfer = slot->xfer;
     args.flags = slot->flags;
+    args.part = slot->part;
+    args.cnt = slot->cnt;
     return true;
 }
 
-// Balanced schedule when whole tiles do not divide evenly over the G CTAs (or CTA pairs); numerically
-// invisible.  Full waves stay tile-granular; the ragged remainder (plus one full wave when the remainder
-// alone would leave less than half a tile per CTA) is cut at K-segment granularity.
-void set_balance(GemmArgs &args, int64_t tiles, int64_t G, cudaStream_t stream)
+// Balanced schedule when whole tiles do not divide evenly over the G_max CTAs (or CTA pairs); numerically
+// invisible.  Returns the number of CTAs (pairs) to launch.
+//  * tiles >= G_max: full waves stay tile-granular; the ragged remainder (plus one full wave when the remainder
+//    alone would leave less than half a tile per CTA) is cut at K-segment granularity.
+//  * tiles < G_max (mid-size M, small N): ordered split-K, see below.
+int64_t set_balance(GemmArgs &args, int64_t tiles, int64_t n_seg, int64_t G_max, int ctas_per_tile, int bn, cudaStream_t stream)
 {
     args.xfer = nullptr;
     args.flags = nullptr;
+    args.part = nullptr;
+    args.cnt = nullptr;
+    args.sk = 0;
     static const bool no_balance = std::getenv("HEAL_NO_BALANCE") != nullptr;      // debug only
     args.balance = 0;
     args.dp_tiles = static_cast<int>(tiles);
-    if (!no_balance && tiles > G && tiles % G != 0) {
-        const int64_t waves = tiles / G, rem = tiles % G;
+    if (tiles < G_max) {
+        // Ordered split-K: (tile, segment) units are dealt contiguously to up to tiles * n_seg CTAs; every
+        // segment partial is parked in global memory and the CTAs of a tile each finish a share of its columns.
+        const int64_t units = tiles * n_seg;
+        const int64_t G = units < G_max ? units : G_max;
+        const size_t part_bytes = static_cast<size_t>(units) * ctas_per_tile * kBM * bn * sizeof(float);
+        // Worth it only while a CTA gets few units: parking and re-reading a partial costs about 1.4 segments of
+        // L2 traffic (measured: a parked unit takes 2.4x a plain segment), whole tiles cost n_seg segments.
+        const int64_t units_per_cta = (units + G - 1) / G;
+        if (!no_balance && n_seg > 1 && G > tiles && 12 * units_per_cta < 5 * n_seg &&
+            part_bytes <= (static_cast<size_t>(128) << 20) && bind_xfer(args, stream, part_bytes)) {
+            args.balance = 1;
+            args.sk = 1;
+            args.dp_tiles = 0;
+            return G;
+        }
+        return tiles;
+    }
+    if (!no_balance && tiles % G_max != 0) {
+        const int64_t waves = tiles / G_max, rem = tiles % G_max;
         int64_t sk = rem;
-        if (rem * 2 < G && waves >= 1) sk += G;
+        if (rem * 2 < G_max && waves >= 1) sk += G_max;
         if (bind_xfer(args, stream)) {
             args.balance = 1;
             args.dp_tiles = static_cast<int>(tiles - sk);
         }
     }
+    return G_max;
 }
 
 // ---- steps G + E launch -----------------------------------------------------------------------
@@ -254,8 +312,7 @@ int launch_gemm_cfg(int64_t M, int64_t N, int64_t K, const void *A_hi, const voi
     args.tiles_n = static_cast<int>((N + Cfg::BN - 1) / Cfg::BN);
     args.diag = g.diag;
     const int64_t tiles = static_cast<int64_t>(args.tiles_m) * args.tiles_n;
-    const unsigned grid = static_cast<unsigned>(tiles < g.num_sms ? tiles : g.num_sms);
-    set_balance(args, tiles, g.num_sms, stream);
+    const unsigned grid = static_cast<unsigned>(set_balance(args, tiles, (K + kKSeg - 1) / kKSeg, g.num_sms, 1, Cfg::BN, stream));
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(grid);
     cfg.blockDim = dim3(kGemmThreads);
@@ -309,9 +366,7 @@ int launch_gemm2_cfg(int64_t M, int64_t N, int64_t K, const void *A_hi, const vo
     args.tiles_n = static_cast<int>((N + Cfg::BN - 1) / Cfg::BN);
     args.diag = g.diag;
     const int64_t tiles = static_cast<int64_t>(args.tiles_m) * args.tiles_n;
-    const int64_t pairs = g.num_sms / 2;
-    const int64_t G = tiles < pairs ? tiles : pairs;
-    set_balance(args, tiles, G, stream);
+    const int64_t G = set_balance(args, tiles, (K + kKSeg - 1) / kKSeg, g.num_sms / 2, 2, Cfg::BN, stream);
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(static_cast<unsigned>(2 * G));
     cfg.blockDim = dim3(kGemmThreads);

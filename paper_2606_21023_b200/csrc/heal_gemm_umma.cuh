@@ -54,6 +54,11 @@ struct GemmArgs {
     int dp_tiles;           // tiles dealt whole, round-robin (multiple of the grid size)
     float *xfer;            // per-CTA hand-off slot: kBM * BN floats each
     uint32_t *flags;        // per-CTA flag: 1 once the slot is written, reset to 0 by its consumer
+    // ordered split-K (few tiles, many CTAs): every (tile, segment) partial goes to `part`, the CTAs that
+    // computed a tile's segments then each finish a share of its columns, adding the partials in ascending order
+    int sk;
+    float *part;            // [(tile * R + rank) * n_seg + seg] x (kBM * BN) floats, R = CTAs per tile
+    uint32_t *cnt;          // [(tile * R + rank) * 2]: partials written, shares finished (both back to 0 at the end)
 };
 
 // Work distribution.  The unit of work is (tile, K segment).  The first `dp_tiles` tiles (a multiple of
@@ -126,6 +131,93 @@ struct TileSched {
         }
     }
 };
+
+// ---- ordered split-K helpers (256 epilogue threads, etid = 0..255; thread owns row quad*32+lane, CPW columns) ----
+// Partial layout: float4 index c4 * 256 + etid, c4 = 0..CPW/4-1 (the thread's columns 4*c4..4*c4+3): coalesced for
+// the writer and for the finisher, which use the same thread mapping.
+template <int CPW>
+__device__ __forceinline__ void sk_store_partial(float *part, uint32_t taddr, int etid)
+{
+    float4 *dst = reinterpret_cast<float4 *>(part);
+#pragma unroll
+    for (int c = 0; c < CPW / 16; ++c) {
+        uint32_t v[16];
+        tmem_ld_32x32b_x16(taddr + c * 16, v);
+        tmem_ld_wait();
+#pragma unroll
+        for (int q = 0; q < 4; ++q)
+            dst[(c * 4 + q) * 256 + etid] = make_float4(__uint_as_float(v[4 * q]), __uint_as_float(v[4 * q + 1]),
+                                                        __uint_as_float(v[4 * q + 2]), __uint_as_float(v[4 * q + 3]));
+    }
+}
+__device__ __forceinline__ void sk_signal(uint32_t *ctr, int etid)
+{
+    __threadfence();
+    asm volatile("bar.sync 1, 256;" ::: "memory");
+    if (etid == 0) asm volatile("red.release.gpu.global.add.u32 [%0], %1;" ::"l"(ctr), "r"(1u) : "memory");
+}
+__device__ __forceinline__ void sk_wait(const uint32_t *ctr, uint32_t want, int etid, int *diag)
+{
+    if (etid == 0) {
+        const uint64_t t0 = globaltimer_ns();
+        uint32_t f;
+        do {
+            asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(f) : "l"(ctr) : "memory");
+            if (f < want && globaltimer_ns() - t0 > 4000000000ull) {
+                diag[0] = 810;
+                diag[1] = static_cast<int>(blockIdx.x);
+                __trap();
+            }
+        } while (f < want);
+    }
+    asm volatile("bar.sync 1, 256;" ::: "memory");
+}
+// The CTA that computed segment `seg` finishes float4 chunks [seg*NC/n_seg, (seg+1)*NC/n_seg) of every row:
+// ascending-segment FP32 RN sum of the n_seg partials, then the predicated store to C.
+template <int CPW>
+__device__ __forceinline__ void sk_finish(const float *part0, int n_seg, int seg, int etid, float *crow, int col0, int N, bool row_ok)
+{
+    constexpr int NC = CPW / 4;
+    const int c_lo = seg * NC / n_seg, c_hi = (seg + 1) * NC / n_seg;
+    const float4 *src = reinterpret_cast<const float4 *>(part0);
+    const size_t seg_stride = static_cast<size_t>(kBM) * (2 * CPW) / 4;        // float4 per partial (kBM x BN floats)
+    for (int c4 = c_lo; c4 < c_hi; ++c4) {
+        float4 acc;
+        asm volatile("ld.global.cg.v4.f32 {%0, %1, %2, %3}, [%4];"
+                     : "=f"(acc.x), "=f"(acc.y), "=f"(acc.z), "=f"(acc.w) : "l"(src + c4 * 256 + etid) : "memory");
+        for (int s = 1; s < n_seg; ++s) {
+            float4 v;
+            asm volatile("ld.global.cg.v4.f32 {%0, %1, %2, %3}, [%4];"
+                         : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(src + s * seg_stride + c4 * 256 + etid) : "memory");
+            acc.x = __fadd_rn(acc.x, v.x); acc.y = __fadd_rn(acc.y, v.y);
+            acc.z = __fadd_rn(acc.z, v.z); acc.w = __fadd_rn(acc.w, v.w);
+        }
+        if (row_ok) {
+            const int col = col0 + c4 * 4;
+            if (col + 3 < N) {
+                *reinterpret_cast<float4 *>(crow + col) = acc;
+            } else {
+                if (col < N) crow[col] = acc.x;
+                if (col + 1 < N) crow[col + 1] = acc.y;
+                if (col + 2 < N) crow[col + 2] = acc.z;
+                if (col + 3 < N) crow[col + 3] = acc.w;
+            }
+        }
+    }
+}
+// last finisher of a (tile, rank): re-arm both counters for the next launch on this stream
+__device__ __forceinline__ void sk_done(uint32_t *ctr, uint32_t n_seg, int etid)
+{
+    asm volatile("bar.sync 1, 256;" ::: "memory");
+    if (etid == 0) {
+        uint32_t old;
+        asm volatile("atom.acq_rel.gpu.global.add.u32 %0, [%1], %2;" : "=r"(old) : "l"(ctr + 1), "r"(1u) : "memory");
+        if (old == n_seg - 1) {
+            asm volatile("st.relaxed.gpu.global.u32 [%0], %1;" ::"l"(ctr), "r"(0u) : "memory");
+            asm volatile("st.relaxed.gpu.global.u32 [%0], %1;" ::"l"(ctr + 1), "r"(0u) : "memory");
+        }
+    }
+}
 
 template <class Cfg>
 __global__ void __launch_bounds__(kGemmThreads, 1)
@@ -282,6 +374,23 @@ heal_gemm_umma_kernel(const __grid_constant__ CUtensorMap tm_a_hi, const __grid_
             sched.get(ci, tile, sb_seg, se_seg);
             const int m0 = (tile % args.tiles_m) * kBM;
             const int n0 = (tile / args.tiles_m) * BN;
+            if (args.sk) {
+                // ordered split-K: park every segment partial in global memory; the sums are formed below
+                for (int seg = sb_seg; seg < se_seg; ++seg) {
+                    mbar_wait(tfull_bar(buf), (tphase >> buf) & 1u, args.diag, 400 + buf);
+                    tc_fence_after();
+                    const uint32_t taddr = tmem_base + (static_cast<uint32_t>(quad * 32) << 16) +
+                                           static_cast<uint32_t>(buf * BN + chalf * CPW);
+                    sk_store_partial<CPW>(args.part + (static_cast<size_t>(tile) * n_seg + seg) * (kBM * BN), taddr, etid);
+                    tc_fence_before();
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(tempty_bar(buf));
+                    tphase ^= 1u << buf;
+                    buf ^= 1;
+                    sk_signal(args.cnt + 2 * tile, etid);
+                }
+                continue;
+            }
             if (sb_seg > 0) {
                 // tail of a shared tile: start from the neighbour's running sum (segments 0..sb_seg-1)
                 const uint32_t *flag = args.flags + (blockIdx.x - 1);
@@ -362,6 +471,22 @@ heal_gemm_umma_kernel(const __grid_constant__ CUtensorMap tm_a_hi, const __grid_
                         for (int i = 0; i < 4; ++i)
                             if (col + i < args.N) crow[col + i] = run[c + i];
                     }
+                }
+            }
+        }
+        if (args.sk) {
+            // every partial of this CTA is parked: finish a share of the columns of each unit's tile
+            for (int ci = 0; ci < sched.n_chunks; ++ci) {
+                int tile, sb_seg, se_seg;
+                sched.get(ci, tile, sb_seg, se_seg);
+                const int m0 = (tile % args.tiles_m) * kBM;
+                const int n0 = (tile / args.tiles_m) * BN;
+                const int row = m0 + quad * 32 + lane;
+                sk_wait(args.cnt + 2 * tile, static_cast<uint32_t>(n_seg), etid, args.diag);
+                for (int seg = sb_seg; seg < se_seg; ++seg) {
+                    sk_finish<CPW>(args.part + static_cast<size_t>(tile) * n_seg * (kBM * BN), n_seg, seg, etid,
+                                   args.C + static_cast<int64_t>(row) * args.ldc, n0 + chalf * CPW, args.N, row < args.M);
+                    sk_done(args.cnt + 2 * tile, static_cast<uint32_t>(n_seg), etid);
                 }
             }
         }

@@ -190,6 +190,23 @@ heal_gemm_umma2_kernel(const __grid_constant__ CUtensorMap tm_a_hi, const __grid
             sched.get(ci, tile, sb_seg, se_seg);
             const int m0 = (tile % args.tiles_m) * (2 * kBM) + rank * kBM;
             const int n0 = (tile / args.tiles_m) * BN;
+            if (args.sk) {
+                // ordered split-K (see heal_gemm_umma.cuh): park every segment partial of this CTA's 128 rows
+                for (int seg = sb_seg; seg < se_seg; ++seg) {
+                    mbar_wait(tfull_bar(buf), (tphase >> buf) & 1u, args.diag, 400 + buf);
+                    tc_fence_after();
+                    const uint32_t taddr = tmem_base + (static_cast<uint32_t>(quad * 32) << 16) +
+                                           static_cast<uint32_t>(buf * BN + chalf * CPW);
+                    sk_store_partial<CPW>(args.part + ((static_cast<size_t>(tile) * 2 + rank) * n_seg + seg) * (kBM * BN), taddr, etid);
+                    tc_fence_before();
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive_cluster(leader_addr(tempty_bar(buf)));
+                    tphase ^= 1u << buf;
+                    buf ^= 1;
+                    sk_signal(args.cnt + 2 * (tile * 2 + rank), etid);
+                }
+                continue;
+            }
             if (sb_seg > 0) {
                 const uint32_t *flag = args.flags + (blockIdx.x - 2);        // same rank, previous pair
                 if (etid == 0) {
@@ -267,6 +284,22 @@ heal_gemm_umma2_kernel(const __grid_constant__ CUtensorMap tm_a_hi, const __grid
                         for (int i = 0; i < 4; ++i)
                             if (col + i < args.N) crow[col + i] = run[c + i];
                     }
+                }
+            }
+        }
+        if (args.sk) {
+            for (int ci = 0; ci < sched.n_chunks; ++ci) {
+                int tile, sb_seg, se_seg;
+                sched.get(ci, tile, sb_seg, se_seg);
+                const int m0 = (tile % args.tiles_m) * (2 * kBM) + rank * kBM;
+                const int n0 = (tile / args.tiles_m) * BN;
+                const int row = m0 + quad * 32 + lane;
+                uint32_t *ctr = args.cnt + 2 * (tile * 2 + rank);
+                sk_wait(ctr, static_cast<uint32_t>(n_seg), etid, args.diag);
+                for (int seg = sb_seg; seg < se_seg; ++seg) {
+                    sk_finish<CPW>(args.part + (static_cast<size_t>(tile) * 2 + rank) * n_seg * (kBM * BN), n_seg, seg, etid,
+                                   args.C + static_cast<int64_t>(row) * args.ldc, n0 + chalf * CPW, args.N, row < args.M);
+                    sk_done(ctr, static_cast<uint32_t>(n_seg), etid);
                 }
             }
         }

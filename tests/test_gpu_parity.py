@@ -364,6 +364,38 @@ def test_small_m_large_reduction_area_bit_identical(hb, inputs, M, N, K):
     assert torch.equal(outs[0], outs[1])
 
 
+@pytest.mark.parametrize("M,N,K,nprod", [(128, 1032, 4096, 2), (300, 520, 14336, 2), (256, 264, 2056, 3), (1000, 1032, 1536, 2), (96, 4096, 1024, 2)])
+def test_ordered_split_k_mid_m(hb, oracle, inputs, M, N, K, nprod):
+    """Few output tiles, many SMs: the large-M kernels cut every tile at K-segment granularity, park the segment
+    partials in global memory and add them in ascending order (ordered split-K).  Same bits as the small-M kernel on
+    64-row blocks of the same input, stable under CUDA-graph replay (counters re-arm), and inside the gate."""
+    A = inputs.activations(M, K, seed=14, outliers=True)
+    B = inputs.weights_f32(K, N, seed=14) if nprod >= 3 else inputs.weights_f16(K, N, seed=14)
+    Ad, Bd = dev(A), dev(B)
+    full = hb.heal_gemm(Ad, Bd, nprod).clone()
+    for r0 in range(0, M, 64):
+        blk = hb.heal_gemm(Ad[r0:r0 + 64], Bd, nprod)           # M <= 64: swap-AB cluster kernel
+        assert torch.equal(blk, full[r0:r0 + 64]), r0
+    ah, al = hb.heal_split(Ad)
+    bh, bl = hb.heal_split(Bd) if nprod >= 3 else (Bd, None)
+    C = torch.zeros_like(full)
+    s = torch.cuda.Stream()
+    torch.cuda.synchronize()
+    with torch.cuda.stream(s):
+        hb.heal_gemm_presplit(ah, al, bh, bl, nprod, C=C)
+        s.synchronize()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=s):
+            hb.heal_gemm_presplit(ah, al, bh, bl, nprod, C=C)
+            hb.heal_gemm_presplit(ah, al, bh, bl, nprod, C=C)
+        for _ in range(4):
+            C.zero_()
+            g.replay()
+            s.synchronize()
+            assert torch.equal(C, full)
+    assert oracle.normwise_error(full.cpu().numpy(), oracle.gemm_f64(A, B), A, B) <= GATE
+
+
 def test_static_weights_graph_chain(hb, inputs):
     """HEAL_B_STATIC in a captured chain of decode GEMMs (each kernel streams its weights while its predecessor
     finishes; activations and C wait): every replay reproduces the eager results bit for bit, including a chain
