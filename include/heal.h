@@ -108,6 +108,34 @@ int heal_gemm_presplit(int64_t M, int64_t N, int64_t K,
                        uint32_t mode, void *stream);
 
 /*
+ * Extended epilogue (step E options):
+ *   scale_exp   the result is multiplied by 2^-scale_exp before it is stored -- the inverse of the
+ *               per-weight-matrix power-of-two scale 2^p the paper applies to the weights before the
+ *               GEMM ("invert the scale after the GEMM output").  Exact (a power of two)
+ *               unless the product leaves the FP32 normal range.  -126 <= scale_exp <= 126; 0 = none.
+ *   C_hi, C_lo  optional FP16 M x N planes (leading dimension ldc16 >= N elements, % 8 == 0, 16-byte
+ *               aligned; both or neither): the chained output -- hi = r16(c), lo = r16(c - hi) of every
+ *               scaled result c, i.e. exactly heal_split() of the FP32 output, written by
+ *               the GEMM epilogue so that the next compensated GEMM (heal_gemm_presplit) needs no pass
+ *               over C.
+ *   C           may be NULL when the planes are requested (then ldc is ignored); otherwise as heal_gemm.
+ * Everything else as heal_gemm / heal_gemm_presplit; heal_gemm(...) == heal_gemm_ex(..., NULL, NULL, 0, 0, ...).
+ */
+int heal_gemm_ex(int64_t M, int64_t N, int64_t K,
+                 const void *A, int64_t lda,
+                 const void *B, int64_t ldb,
+                 void *C, int64_t ldc,
+                 void *C_hi, void *C_lo, int64_t ldc16, int32_t scale_exp,
+                 uint32_t mode, void *stream);
+
+int heal_gemm_presplit_ex(int64_t M, int64_t N, int64_t K,
+                          const void *A_hi, const void *A_lo, int64_t lda,
+                          const void *B_hi, const void *B_lo, int64_t ldb,
+                          void *C, int64_t ldc,
+                          void *C_hi, void *C_lo, int64_t ldc16, int32_t scale_exp,
+                          uint32_t mode, void *stream);
+
+/*
  * HOST-buffer variant of heal_gemm: A, B, C are HOST pointers (ideally pinned).  Copies A and B to
  * the device, runs the path, copies C back and synchronises `stream` before returning.  Same
  * layout rules as heal_gemm except that alignment applies to the internal device copies only.

@@ -42,6 +42,11 @@ def lib():
         L.heal_split.argtypes = [i64, i64, vp, i64, vp, vp, i64, vp]
         L.heal_gemm_presplit.restype = ci
         L.heal_gemm_presplit.argtypes = [i64, i64, i64, vp, vp, i64, vp, vp, i64, vp, i64, u32, vp]
+        i32 = ctypes.c_int32
+        L.heal_gemm_ex.restype = ci
+        L.heal_gemm_ex.argtypes = [i64, i64, i64, vp, i64, vp, i64, vp, i64, vp, vp, i64, i32, u32, vp]
+        L.heal_gemm_presplit_ex.restype = ci
+        L.heal_gemm_presplit_ex.argtypes = [i64, i64, i64, vp, vp, i64, vp, vp, i64, vp, i64, vp, vp, i64, i32, u32, vp]
         L.heal_workspace_size.restype = ctypes.c_size_t
         L.heal_workspace_size.argtypes = [i64, i64, i64, u32]
         L.heal_set_workspace.restype = ci
@@ -115,6 +120,45 @@ def heal_gemm(A: torch.Tensor, B: torch.Tensor, mode: int = MODE_2P, C: torch.Te
     _check(lib().heal_gemm(M, N, K, A.data_ptr(), _ld(A), B.data_ptr(), _ld(B), C.data_ptr(), _ld(C), mode,
                            _stream(stream)))
     return C
+
+
+def _planes(M, N, device):
+    ld = (N + 7) // 8 * 8
+    return (torch.empty((M, ld), dtype=torch.float16, device=device)[:, :N],
+            torch.empty((M, ld), dtype=torch.float16, device=device)[:, :N])
+
+
+def heal_gemm_ex(A: torch.Tensor, B: torch.Tensor, mode: int = MODE_2P, C: torch.Tensor | None = None, want_c: bool = True,
+                 want_planes: bool = True, scale_exp: int = 0, C_hi=None, C_lo=None, stream=None):
+    """heal_gemm with the extended epilogue: returns (C or None, C_hi or None, C_lo or None); every output is the
+    result times 2^-scale_exp, the planes are its hi/lo split for a following heal_gemm_presplit."""
+    assert A.is_cuda and B.is_cuda and A.dtype == torch.float32
+    M, K = A.shape
+    N = B.shape[0] if mode & B_NK else B.shape[1]
+    if C is None and want_c:
+        C = torch.empty((M, N), dtype=torch.float32, device=A.device)
+    if want_planes and C_hi is None:
+        C_hi, C_lo = _planes(M, N, A.device)
+    p = lambda t: None if t is None else t.data_ptr()
+    _check(lib().heal_gemm_ex(M, N, K, A.data_ptr(), _ld(A), B.data_ptr(), _ld(B), p(C), 0 if C is None else _ld(C),
+                              p(C_hi), p(C_lo), 0 if C_hi is None else _ld(C_hi), scale_exp, mode, _stream(stream)))
+    return C, C_hi, C_lo
+
+
+def heal_gemm_presplit_ex(A_hi, A_lo, B_hi, B_lo, mode: int, C: torch.Tensor | None = None, want_c: bool = True,
+                          want_planes: bool = True, scale_exp: int = 0, C_hi=None, C_lo=None, stream=None):
+    """heal_gemm_presplit with the extended epilogue (see heal_gemm_ex)."""
+    M, K = A_hi.shape
+    N = B_hi.shape[0] if mode & B_NK else B_hi.shape[1]
+    if C is None and want_c:
+        C = torch.empty((M, N), dtype=torch.float32, device=A_hi.device)
+    if want_planes and C_hi is None:
+        C_hi, C_lo = _planes(M, N, A_hi.device)
+    p = lambda t: None if t is None else t.data_ptr()
+    _check(lib().heal_gemm_presplit_ex(M, N, K, p(A_hi), p(A_lo), _ld(A_hi), p(B_hi), p(B_lo), _ld(B_hi), p(C),
+                                       0 if C is None else _ld(C), p(C_hi), p(C_lo), 0 if C_hi is None else _ld(C_hi),
+                                       scale_exp, mode, _stream(stream)))
+    return C, C_hi, C_lo
 
 
 def heal_gemm_raw(M, N, K, A_ptr, lda, B_ptr, ldb, C_ptr, ldc, mode, stream_ptr=None) -> int:

@@ -10,6 +10,7 @@
 
 #include <atomic>
 #include <cstdlib>
+#include <cstring>
 #include <mutex>
 
 #include "heal_gemm_smallm.cuh"
@@ -275,7 +276,7 @@ int64_t set_balance(GemmArgs &args, int64_t tiles, int64_t n_seg, int64_t G_max,
 // ---- steps G + E launch -----------------------------------------------------------------------
 template <class Cfg>
 int launch_gemm_cfg(int64_t M, int64_t N, int64_t K, const void *A_hi, const void *A_lo, int64_t lda, const void *B_hi,
-                    const void *B_lo, int64_t ldb, float *C, int64_t ldc, cudaStream_t stream)
+                    const void *B_lo, int64_t ldb, const OutArgs &out, cudaStream_t stream)
 {
     static bool attr_set = false;
     auto kern = heal_gemm_umma_kernel<Cfg>;
@@ -303,8 +304,7 @@ int launch_gemm_cfg(int64_t M, int64_t N, int64_t K, const void *A_hi, const voi
         tb_lo = tb_hi;
     }
     GemmArgs args;
-    args.C = C;
-    args.ldc = ldc;
+    args.out = out;
     args.M = static_cast<int>(M);
     args.N = static_cast<int>(N);
     args.K = static_cast<int>(K);
@@ -329,7 +329,7 @@ int launch_gemm_cfg(int64_t M, int64_t N, int64_t K, const void *A_hi, const voi
 // CTA-pair (cta_group::2) variant: 256 x BN tiles, cluster of 2
 template <class Cfg>
 int launch_gemm2_cfg(int64_t M, int64_t N, int64_t K, const void *A_hi, const void *A_lo, int64_t lda, const void *B_hi,
-                     const void *B_lo, int64_t ldb, float *C, int64_t ldc, cudaStream_t stream)
+                     const void *B_lo, int64_t ldb, const OutArgs &out, cudaStream_t stream)
 {
     static bool attr_set = false;
     auto kern = heal_gemm_umma2_kernel<Cfg>;
@@ -357,8 +357,7 @@ int launch_gemm2_cfg(int64_t M, int64_t N, int64_t K, const void *A_hi, const vo
         tb_lo = tb_hi;
     }
     GemmArgs args;
-    args.C = C;
-    args.ldc = ldc;
+    args.out = out;
     args.M = static_cast<int>(M);
     args.N = static_cast<int>(N);
     args.K = static_cast<int>(K);
@@ -382,26 +381,26 @@ int launch_gemm2_cfg(int64_t M, int64_t N, int64_t K, const void *A_hi, const vo
 
 template <bool B_MN>
 int launch_gemm2_np(int nprod, int64_t M, int64_t N, int64_t K, const void *A_hi, const void *A_lo, int64_t lda,
-                    const void *B_hi, const void *B_lo, int64_t ldb, float *C, int64_t ldc, cudaStream_t s)
+                    const void *B_hi, const void *B_lo, int64_t ldb, const OutArgs &out, cudaStream_t s)
 {
     switch (nprod) {
-    case 1: return launch_gemm2_cfg<Gemm2Cfg<256, 1, B_MN>>(M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, C, ldc, s);
-    case 2: return launch_gemm2_cfg<Gemm2Cfg<256, 2, B_MN>>(M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, C, ldc, s);
-    case 3: return launch_gemm2_cfg<Gemm2Cfg<256, 3, B_MN>>(M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, C, ldc, s);
-    case 4: return launch_gemm2_cfg<Gemm2Cfg<256, 4, B_MN>>(M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, C, ldc, s);
+    case 1: return launch_gemm2_cfg<Gemm2Cfg<256, 1, B_MN>>(M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, out, s);
+    case 2: return launch_gemm2_cfg<Gemm2Cfg<256, 2, B_MN>>(M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, out, s);
+    case 3: return launch_gemm2_cfg<Gemm2Cfg<256, 3, B_MN>>(M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, out, s);
+    case 4: return launch_gemm2_cfg<Gemm2Cfg<256, 4, B_MN>>(M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, out, s);
     }
     return HEAL_ERR_UNSUPPORTED_MODE;
 }
 
 template <int BN, bool B_MN>
 int launch_gemm_np(int nprod, int64_t M, int64_t N, int64_t K, const void *A_hi, const void *A_lo, int64_t lda,
-                   const void *B_hi, const void *B_lo, int64_t ldb, float *C, int64_t ldc, cudaStream_t s)
+                   const void *B_hi, const void *B_lo, int64_t ldb, const OutArgs &out, cudaStream_t s)
 {
     switch (nprod) {
-    case 1: return launch_gemm_cfg<GemmCfg<BN, 1, B_MN>>(M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, C, ldc, s);
-    case 2: return launch_gemm_cfg<GemmCfg<BN, 2, B_MN>>(M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, C, ldc, s);
-    case 3: return launch_gemm_cfg<GemmCfg<BN, 3, B_MN>>(M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, C, ldc, s);
-    case 4: return launch_gemm_cfg<GemmCfg<BN, 4, B_MN>>(M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, C, ldc, s);
+    case 1: return launch_gemm_cfg<GemmCfg<BN, 1, B_MN>>(M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, out, s);
+    case 2: return launch_gemm_cfg<GemmCfg<BN, 2, B_MN>>(M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, out, s);
+    case 3: return launch_gemm_cfg<GemmCfg<BN, 3, B_MN>>(M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, out, s);
+    case 4: return launch_gemm_cfg<GemmCfg<BN, 4, B_MN>>(M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, out, s);
     }
     return HEAL_ERR_UNSUPPORTED_MODE;
 }
@@ -409,11 +408,11 @@ int launch_gemm_np(int nprod, int64_t M, int64_t N, int64_t K, const void *A_hi,
 // Tile width: a function of N only (never of M), so the schedule cannot make results depend on M.
 template <bool B_MN>
 int launch_gemm_bn(int nprod, int64_t M, int64_t N, int64_t K, const void *A_hi, const void *A_lo, int64_t lda,
-                   const void *B_hi, const void *B_lo, int64_t ldb, float *C, int64_t ldc, cudaStream_t s)
+                   const void *B_hi, const void *B_lo, int64_t ldb, const OutArgs &out, cudaStream_t s)
 {
-    if (N <= 64) return launch_gemm_np<64, B_MN>(nprod, M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, C, ldc, s);
-    if (N <= 128) return launch_gemm_np<128, B_MN>(nprod, M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, C, ldc, s);
-    return launch_gemm_np<256, B_MN>(nprod, M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, C, ldc, s);
+    if (N <= 64) return launch_gemm_np<64, B_MN>(nprod, M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, out, s);
+    if (N <= 128) return launch_gemm_np<128, B_MN>(nprod, M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, out, s);
+    return launch_gemm_np<256, B_MN>(nprod, M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, out, s);
 }
 
 #ifdef HEAL_TRACE
@@ -434,7 +433,7 @@ struct SmallIn {
 
 template <class Cfg>
 int launch_small_cfg(int64_t M, int64_t N, int64_t K, const SmallIn &in, const void *B_hi, const void *B_lo, int64_t ldb,
-                     float *C, int64_t ldc, cudaStream_t stream, bool *handled)
+                     const OutArgs &out, cudaStream_t stream, bool *handled)
 {
     *handled = false;
     const int n_seg = static_cast<int>((K + kKSeg - 1) / kKSeg);
@@ -513,8 +512,7 @@ int launch_small_cfg(int64_t M, int64_t N, int64_t K, const SmallIn &in, const v
         }
     }
     SmallArgs args;
-    args.C = C;
-    args.ldc = ldc;
+    args.out = out;
     args.A = in.A32;
     args.lda = in.lda32;
     args.M = static_cast<int>(M);
@@ -553,31 +551,31 @@ int launch_small_cfg(int64_t M, int64_t N, int64_t K, const SmallIn &in, const v
 
 template <int MPAD, bool B_MN>
 int launch_small_np(int nprod, int64_t M, int64_t N, int64_t K, const SmallIn &in, const void *B_hi, const void *B_lo,
-                    int64_t ldb, float *C, int64_t ldc, cudaStream_t s, bool *handled)
+                    int64_t ldb, const OutArgs &out, cudaStream_t s, bool *handled)
 {
     if (in.A32) {                                               // fused split: FP16 weights only
         switch (nprod) {
-        case 1: return launch_small_cfg<SmallCfg<MPAD, 1, B_MN, true>>(M, N, K, in, B_hi, B_lo, ldb, C, ldc, s, handled);
-        case 2: return launch_small_cfg<SmallCfg<MPAD, 2, B_MN, true>>(M, N, K, in, B_hi, B_lo, ldb, C, ldc, s, handled);
+        case 1: return launch_small_cfg<SmallCfg<MPAD, 1, B_MN, true>>(M, N, K, in, B_hi, B_lo, ldb, out, s, handled);
+        case 2: return launch_small_cfg<SmallCfg<MPAD, 2, B_MN, true>>(M, N, K, in, B_hi, B_lo, ldb, out, s, handled);
         }
         return HEAL_ERR_UNSUPPORTED_MODE;
     }
     switch (nprod) {
-    case 1: return launch_small_cfg<SmallCfg<MPAD, 1, B_MN, false>>(M, N, K, in, B_hi, B_lo, ldb, C, ldc, s, handled);
-    case 2: return launch_small_cfg<SmallCfg<MPAD, 2, B_MN, false>>(M, N, K, in, B_hi, B_lo, ldb, C, ldc, s, handled);
-    case 3: return launch_small_cfg<SmallCfg<MPAD, 3, B_MN, false>>(M, N, K, in, B_hi, B_lo, ldb, C, ldc, s, handled);
-    case 4: return launch_small_cfg<SmallCfg<MPAD, 4, B_MN, false>>(M, N, K, in, B_hi, B_lo, ldb, C, ldc, s, handled);
+    case 1: return launch_small_cfg<SmallCfg<MPAD, 1, B_MN, false>>(M, N, K, in, B_hi, B_lo, ldb, out, s, handled);
+    case 2: return launch_small_cfg<SmallCfg<MPAD, 2, B_MN, false>>(M, N, K, in, B_hi, B_lo, ldb, out, s, handled);
+    case 3: return launch_small_cfg<SmallCfg<MPAD, 3, B_MN, false>>(M, N, K, in, B_hi, B_lo, ldb, out, s, handled);
+    case 4: return launch_small_cfg<SmallCfg<MPAD, 4, B_MN, false>>(M, N, K, in, B_hi, B_lo, ldb, out, s, handled);
     }
     return HEAL_ERR_UNSUPPORTED_MODE;
 }
 
 template <bool B_MN>
 int launch_small(int nprod, int64_t M, int64_t N, int64_t K, const SmallIn &in, const void *B_hi, const void *B_lo,
-                 int64_t ldb, float *C, int64_t ldc, cudaStream_t s, bool *handled)
+                 int64_t ldb, const OutArgs &out, cudaStream_t s, bool *handled)
 {
-    if (M <= 16) return launch_small_np<16, B_MN>(nprod, M, N, K, in, B_hi, B_lo, ldb, C, ldc, s, handled);
-    if (M <= 32) return launch_small_np<32, B_MN>(nprod, M, N, K, in, B_hi, B_lo, ldb, C, ldc, s, handled);
-    return launch_small_np<64, B_MN>(nprod, M, N, K, in, B_hi, B_lo, ldb, C, ldc, s, handled);
+    if (M <= 16) return launch_small_np<16, B_MN>(nprod, M, N, K, in, B_hi, B_lo, ldb, out, s, handled);
+    if (M <= 32) return launch_small_np<32, B_MN>(nprod, M, N, K, in, B_hi, B_lo, ldb, out, s, handled);
+    return launch_small_np<64, B_MN>(nprod, M, N, K, in, B_hi, B_lo, ldb, out, s, handled);
 }
 
 // Debug only: HEAL_FORCE_KERNEL=large|small|1cta (or heal_debug_force_kernel) overrides the kernel choice;
@@ -606,21 +604,28 @@ int validate_mode(uint32_t mode, int *nprod, bool *b_nk)
 
 // A32 != nullptr: FP32 activations for the fused small-M kernel (M <= 64, FP16 weights) instead of planes
 int presplit_impl(int64_t M, int64_t N, int64_t K, const void *A_hi, const void *A_lo, int64_t lda, const void *B_hi,
-                  const void *B_lo, int64_t ldb, void *C, int64_t ldc, int nprod, bool b_nk, bool b_static,
+                  const void *B_lo, int64_t ldb, const OutArgs &out, int nprod, bool b_nk, bool b_static,
                   cudaStream_t stream, const float *A32 = nullptr, int64_t lda32 = 0, bool *handled_out = nullptr)
 {
     if (handled_out) *handled_out = true;
-    if (K == 0) {
-        HEAL_CUDA(cudaMemset2DAsync(C, static_cast<size_t>(ldc) * 4, 0, static_cast<size_t>(N) * 4,
-                                    static_cast<size_t>(M), stream));
+    if (K == 0) {                                       // empty sum: zeros in every requested output
+        if (out.C)
+            HEAL_CUDA(cudaMemset2DAsync(out.C, static_cast<size_t>(out.ldc) * 4, 0, static_cast<size_t>(N) * 4,
+                                        static_cast<size_t>(M), stream));
+        if (out.hi) {
+            HEAL_CUDA(cudaMemset2DAsync(out.hi, static_cast<size_t>(out.ld16) * 2, 0, static_cast<size_t>(N) * 2,
+                                        static_cast<size_t>(M), stream));
+            HEAL_CUDA(cudaMemset2DAsync(out.lo, static_cast<size_t>(out.ld16) * 2, 0, static_cast<size_t>(N) * 2,
+                                        static_cast<size_t>(M), stream));
+        }
         return HEAL_OK;
     }
     const int force = forced_kernel();
     if ((M <= 64 && force != 1) || (force == 2 && M <= 64)) {
         bool handled = false;
         const SmallIn in{A_hi, A_lo, lda, A32, lda32, b_static};
-        int st = b_nk ? launch_small<false>(nprod, M, N, K, in, B_hi, B_lo, ldb, static_cast<float *>(C), ldc, stream, &handled)
-                      : launch_small<true>(nprod, M, N, K, in, B_hi, B_lo, ldb, static_cast<float *>(C), ldc, stream, &handled);
+        int st = b_nk ? launch_small<false>(nprod, M, N, K, in, B_hi, B_lo, ldb, out, stream, &handled)
+                      : launch_small<true>(nprod, M, N, K, in, B_hi, B_lo, ldb, out, stream, &handled);
         if (st || handled) return st;
     }
     if (A32) {                                         // the caller must split first and come back with planes
@@ -629,12 +634,12 @@ int presplit_impl(int64_t M, int64_t N, int64_t K, const void *A_hi, const void 
     }
     if (M > kBM && N > 128 && force != 3) {          // CTA pairs: 256 x 256 tiles
         if (b_nk)
-            return launch_gemm2_np<false>(nprod, M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, static_cast<float *>(C), ldc, stream);
-        return launch_gemm2_np<true>(nprod, M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, static_cast<float *>(C), ldc, stream);
+            return launch_gemm2_np<false>(nprod, M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, out, stream);
+        return launch_gemm2_np<true>(nprod, M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, out, stream);
     }
     if (b_nk)
-        return launch_gemm_bn<false>(nprod, M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, static_cast<float *>(C), ldc, stream);
-    return launch_gemm_bn<true>(nprod, M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, static_cast<float *>(C), ldc, stream);
+        return launch_gemm_bn<false>(nprod, M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, out, stream);
+    return launch_gemm_bn<true>(nprod, M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, out, stream);
 }
 
 // workspace layout for heal_gemm: [A_hi][A_lo][B_hi][B_lo], each plane 256-byte aligned
@@ -750,9 +755,34 @@ int heal_split(int64_t rows, int64_t cols, const void *X, int64_t ldx, void *hi,
                         static_cast<__half *>(lo), ld, static_cast<cudaStream_t>(stream));
 }
 
-int heal_gemm_presplit(int64_t M, int64_t N, int64_t K, const void *A_hi, const void *A_lo, int64_t lda,
-                       const void *B_hi, const void *B_lo, int64_t ldb, void *C, int64_t ldc, uint32_t mode,
-                       void *stream)
+// Output validation shared by the _ex entry points: builds the OutArgs of step E.
+static int make_out(int64_t M, int64_t N, void *C, int64_t ldc, void *C_hi, void *C_lo, int64_t ldc16, int scale_exp,
+                    heal::OutArgs *out)
+{
+    if (scale_exp < -126 || scale_exp > 126) return HEAL_ERR_INVALID_VALUE;
+    if ((C || !C_hi) && ldc < N) return HEAL_ERR_INVALID_VALUE;
+    if ((C_hi || C_lo) && ldc16 < N) return HEAL_ERR_INVALID_VALUE;
+    if (M == 0 || N == 0) return HEAL_OK;
+    if (!C && !C_hi) return HEAL_ERR_NULL_POINTER;
+    if ((C_hi == nullptr) != (C_lo == nullptr)) return HEAL_ERR_NULL_POINTER;
+    if (C && (!aligned16(C) || (ldc & 3))) return HEAL_ERR_MISALIGNED;
+    if (C_hi && (!aligned16(C_hi) || !aligned16(C_lo) || (ldc16 & 7))) return HEAL_ERR_MISALIGNED;
+    out->C = static_cast<float *>(C);
+    out->ldc = ldc;
+    out->hi = static_cast<__half *>(C_hi);
+    out->lo = static_cast<__half *>(C_lo);
+    out->ld16 = ldc16;
+    // 2^-scale_exp, built from its bit pattern (normal for |scale_exp| <= 126)
+    const uint32_t bits = static_cast<uint32_t>(127 - scale_exp) << 23;
+    float sc;
+    memcpy(&sc, &bits, 4);
+    out->scale = sc;
+    return HEAL_OK;
+}
+
+int heal_gemm_presplit_ex(int64_t M, int64_t N, int64_t K, const void *A_hi, const void *A_lo, int64_t lda,
+                          const void *B_hi, const void *B_lo, int64_t ldb, void *C, int64_t ldc, void *C_hi, void *C_lo,
+                          int64_t ldc16, int32_t scale_exp, uint32_t mode, void *stream)
 {
     int nprod;
     bool b_nk;
@@ -760,9 +790,11 @@ int heal_gemm_presplit(int64_t M, int64_t N, int64_t K, const void *A_hi, const 
     if (st) return st;
     if (M < 0 || N < 0 || K < 0) return HEAL_ERR_INVALID_VALUE;
     if (M > 0x7fffff00 || N > 0x7fffff00 || K > 0x7fffff00) return HEAL_ERR_INVALID_VALUE;
-    if (lda < K || ldc < N || ldb < (b_nk ? K : N)) return HEAL_ERR_INVALID_VALUE;
+    if (lda < K || ldb < (b_nk ? K : N)) return HEAL_ERR_INVALID_VALUE;
+    heal::OutArgs out = {};
+    st = make_out(M, N, C, ldc, C_hi, C_lo, ldc16, scale_exp, &out);
+    if (st) return st;
     if (M == 0 || N == 0) return HEAL_OK;
-    if (!C) return HEAL_ERR_NULL_POINTER;
     if (K > 0) {
         if (!A_hi || !B_hi) return HEAL_ERR_NULL_POINTER;
         if (nprod >= 2 && !A_lo) return HEAL_ERR_NULL_POINTER;
@@ -770,15 +802,21 @@ int heal_gemm_presplit(int64_t M, int64_t N, int64_t K, const void *A_hi, const 
         if (!aligned16(A_hi) || !aligned16(A_lo) || !aligned16(B_hi) || !aligned16(B_lo) || (lda & 7) || (ldb & 7))
             return HEAL_ERR_MISALIGNED;
     }
-    if (!aligned16(C) || (ldc & 3)) return HEAL_ERR_MISALIGNED;
     st = ensure_init();
     if (st) return st;
-    return presplit_impl(M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, C, ldc, nprod, b_nk, (mode & HEAL_B_STATIC) != 0,
+    return presplit_impl(M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, out, nprod, b_nk, (mode & HEAL_B_STATIC) != 0,
                          static_cast<cudaStream_t>(stream));
 }
 
-int heal_gemm(int64_t M, int64_t N, int64_t K, const void *A, int64_t lda, const void *B, int64_t ldb, void *C,
-              int64_t ldc, uint32_t mode, void *stream_)
+int heal_gemm_presplit(int64_t M, int64_t N, int64_t K, const void *A_hi, const void *A_lo, int64_t lda,
+                       const void *B_hi, const void *B_lo, int64_t ldb, void *C, int64_t ldc, uint32_t mode,
+                       void *stream)
+{
+    return heal_gemm_presplit_ex(M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, C, ldc, nullptr, nullptr, 0, 0, mode, stream);
+}
+
+int heal_gemm_ex(int64_t M, int64_t N, int64_t K, const void *A, int64_t lda, const void *B, int64_t ldb, void *C,
+                 int64_t ldc, void *C_hi, void *C_lo, int64_t ldc16, int32_t scale_exp, uint32_t mode, void *stream_)
 {
     int nprod;
     bool b_nk;
@@ -786,26 +824,27 @@ int heal_gemm(int64_t M, int64_t N, int64_t K, const void *A, int64_t lda, const
     if (st) return st;
     if (M < 0 || N < 0 || K < 0) return HEAL_ERR_INVALID_VALUE;
     if (M > 0x7fffff00 || N > 0x7fffff00 || K > 0x7fffff00) return HEAL_ERR_INVALID_VALUE;
-    if (lda < K || ldc < N || ldb < (b_nk ? K : N)) return HEAL_ERR_INVALID_VALUE;
+    if (lda < K || ldb < (b_nk ? K : N)) return HEAL_ERR_INVALID_VALUE;
+    heal::OutArgs out = {};
+    st = make_out(M, N, C, ldc, C_hi, C_lo, ldc16, scale_exp, &out);
+    if (st) return st;
     if (M == 0 || N == 0) return HEAL_OK;
-    if (!C) return HEAL_ERR_NULL_POINTER;
     const bool b_f32 = nprod >= 3;
     if (K > 0) {
         if (!A || !B) return HEAL_ERR_NULL_POINTER;
         if (!aligned16(A) || !aligned16(B) || (lda & 3) || (ldb & (b_f32 ? 3 : 7))) return HEAL_ERR_MISALIGNED;
     }
-    if (!aligned16(C) || (ldc & 3)) return HEAL_ERR_MISALIGNED;
     st = ensure_init();
     if (st) return st;
     cudaStream_t stream = static_cast<cudaStream_t>(stream_);
     const bool b_static = (mode & HEAL_B_STATIC) != 0;
-    if (K == 0) return presplit_impl(M, N, K, nullptr, nullptr, lda, nullptr, nullptr, ldb, C, ldc, nprod, b_nk, b_static, stream);
+    if (K == 0) return presplit_impl(M, N, K, nullptr, nullptr, lda, nullptr, nullptr, ldb, out, nprod, b_nk, b_static, stream);
     static const bool no_fused = std::getenv("HEAL_NO_FUSED") != nullptr;          // debug only
     if (M <= 16 && !b_f32 && !no_fused && forced_kernel() != 1) {
         // decode shapes (M <= 16) with FP16 weights: step S runs inside the GEMM kernel (no planes, one launch);
         // above that the in-kernel conversion costs more than the split launch it saves (measured)
         bool handled = false;
-        st = presplit_impl(M, N, K, nullptr, nullptr, 0, B, nullptr, ldb, C, ldc, nprod, b_nk, b_static, stream,
+        st = presplit_impl(M, N, K, nullptr, nullptr, 0, B, nullptr, ldb, out, nprod, b_nk, b_static, stream,
                            static_cast<const float *>(A), lda, &handled);
         if (st || handled) return st;
     }
@@ -833,7 +872,13 @@ int heal_gemm(int64_t M, int64_t N, int64_t K, const void *A, int64_t lda, const
         b_lo = bl;
         ldb_eff = p.ldb_p;
     }
-    return presplit_impl(M, N, K, a_hi, a_lo, p.lda_p, b_hi, b_lo, ldb_eff, C, ldc, nprod, b_nk, b_static, stream);
+    return presplit_impl(M, N, K, a_hi, a_lo, p.lda_p, b_hi, b_lo, ldb_eff, out, nprod, b_nk, b_static, stream);
+}
+
+int heal_gemm(int64_t M, int64_t N, int64_t K, const void *A, int64_t lda, const void *B, int64_t ldb, void *C,
+              int64_t ldc, uint32_t mode, void *stream_)
+{
+    return heal_gemm_ex(M, N, K, A, lda, B, ldb, C, ldc, nullptr, nullptr, 0, 0, mode, stream_);
 }
 
 int heal_gemm_host(int64_t M, int64_t N, int64_t K, const void *A_host, int64_t lda, const void *B_host, int64_t ldb,

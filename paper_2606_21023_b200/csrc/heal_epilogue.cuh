@@ -1,0 +1,74 @@
+// heal_epilogue.cuh -- step E: what the GEMM kernels do with a finished FP32 sum.
+//   * FP32 output ("keep GEMM outputs in FP32");
+//   * optional exact power-of-two output scale 2^-p, the inverse of the per-weight-matrix 2^p pre-scale
+//     the paper applies before the GEMM;
+//   * optional chained output: the hi/lo FP16 planes of the (scaled) result, i.e. step S of the NEXT
+//     compensated GEMM done in this epilogue instead of a separate pass over C.
+// The planes are exactly heal_split() of the FP32 value this epilogue would store (same split2 code).
+#pragma once
+#include <cuda_fp16.h>
+#include <stdint.h>
+
+#include "heal_split.cuh"
+
+namespace heal {
+
+struct OutArgs {
+    float *C;             // FP32 M x N, pitch ldc (elements); may be null when the planes are written
+    int64_t ldc;
+    __half *hi, *lo;      // FP16 M x N planes, pitch ld16 (elements, % 8 == 0); null = not requested
+    int64_t ld16;
+    float scale;          // 2^-p, exactly representable; 1.0f = none
+};
+
+// four consecutive columns col..col+3 of one row (col % 4 == 0); columns >= N are not written
+__device__ __forceinline__ void emit4(const OutArgs &o, int64_t row, int col, float4 v, int N)
+{
+    v.x *= o.scale; v.y *= o.scale; v.z *= o.scale; v.w *= o.scale;
+    const bool full = col + 3 < N;
+    if (o.C) {
+        float *c = o.C + row * o.ldc + col;
+        if (full) {
+            *reinterpret_cast<float4 *>(c) = v;
+        } else {
+            if (col < N) c[0] = v.x;
+            if (col + 1 < N) c[1] = v.y;
+            if (col + 2 < N) c[2] = v.z;
+        }
+    }
+    if (o.hi) {
+        uint2 h, l;
+        split2(v.x, v.y, h.x, l.x);
+        split2(v.z, v.w, h.y, l.y);
+        __half *ph = o.hi + row * o.ld16 + col, *pl = o.lo + row * o.ld16 + col;
+        if (full) {
+            *reinterpret_cast<uint2 *>(ph) = h;
+            *reinterpret_cast<uint2 *>(pl) = l;
+        } else {
+            const uint16_t hs[4] = {static_cast<uint16_t>(h.x), static_cast<uint16_t>(h.x >> 16),
+                                    static_cast<uint16_t>(h.y), static_cast<uint16_t>(h.y >> 16)};
+            const uint16_t ls[4] = {static_cast<uint16_t>(l.x), static_cast<uint16_t>(l.x >> 16),
+                                    static_cast<uint16_t>(l.y), static_cast<uint16_t>(l.y >> 16)};
+#pragma unroll
+            for (int i = 0; i < 3; ++i)
+                if (col + i < N) {
+                    reinterpret_cast<uint16_t *>(ph)[i] = hs[i];
+                    reinterpret_cast<uint16_t *>(pl)[i] = ls[i];
+                }
+        }
+    }
+}
+
+// one element (the small-M kernel: a warp's lanes are consecutive columns of one row)
+__device__ __forceinline__ void emit1(const OutArgs &o, int64_t row, int col, float v)
+{
+    v *= o.scale;
+    if (o.C) o.C[row * o.ldc + col] = v;
+    if (o.hi) {
+        const __half h = __float2half_rn(v);
+        o.hi[row * o.ld16 + col] = h;
+        o.lo[row * o.ld16 + col] = __float2half_rn(__fsub_rn(v, __half2float(h)));
+    }
+}
+
+}  // namespace heal

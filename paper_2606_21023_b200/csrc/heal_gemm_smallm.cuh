@@ -26,8 +26,8 @@
 // Roles per CTA (192 threads): warp 0 TMA producer, warp 1 MMA issuer + TMEM allocator, warps 2-5
 // converter (FUSED) and epilogue (warp w owns TMEM lanes 32*(w%4)..+31).
 #pragma once
+#include "heal_epilogue.cuh"
 #include "heal_ptx.cuh"
-#include "heal_split.cuh"
 
 namespace heal {
 
@@ -57,8 +57,7 @@ struct SmallCfg {
 };
 
 struct SmallArgs {
-    float *C;
-    int64_t ldc;
+    OutArgs out;          // step E: FP32 C and/or hi/lo planes, optional 2^-p scale
     const float *A;       // FUSED: FP32 activations, row pitch lda (elements)
     int64_t lda;
     int M, N, K;
@@ -364,7 +363,7 @@ heal_gemm_smallm_kernel(const __grid_constant__ CUtensorMap tm_x_hi, const __gri
                     if (col < args.N) {
 #pragma unroll
                         for (int i = 0; i < 16; ++i)
-                            if (c * 16 + i < args.M) args.C[static_cast<int64_t>(c * 16 + i) * args.ldc + col] = acc[i];
+                            if (c * 16 + i < args.M) emit1(args.out, c * 16 + i, col, acc[i]);
                     }
                 }
             }
@@ -433,11 +432,10 @@ heal_gemm_smallm_kernel(const __grid_constant__ CUtensorMap tm_x_hi, const __gri
                             acc.z = __fadd_rn(acc.z, v.z); acc.w = __fadd_rn(acc.w, v.w);
                         }
                         if (col < args.N) {
-                            float *dst = args.C + static_cast<int64_t>(m_lo + r4) * args.ldc + col;
-                            dst[0] = acc.x;
-                            if (r4 + 1 < rows) dst[args.ldc] = acc.y;
-                            if (r4 + 2 < rows) dst[2 * args.ldc] = acc.z;
-                            if (r4 + 3 < rows) dst[3 * args.ldc] = acc.w;
+                            emit1(args.out, m_lo + r4, col, acc.x);
+                            if (r4 + 1 < rows) emit1(args.out, m_lo + r4 + 1, col, acc.y);
+                            if (r4 + 2 < rows) emit1(args.out, m_lo + r4 + 2, col, acc.z);
+                            if (r4 + 3 < rows) emit1(args.out, m_lo + r4 + 3, col, acc.w);
                         }
                     }
                 } else {
@@ -446,7 +444,7 @@ heal_gemm_smallm_kernel(const __grid_constant__ CUtensorMap tm_x_hi, const __gri
                         float acc = src[0];
 #pragma unroll 4
                         for (int s = 1; s < args.n_seg; ++s) acc = __fadd_rn(acc, src[static_cast<size_t>(s) * seg_stride]);
-                        if (col < args.N) args.C[static_cast<int64_t>(m_lo + r) * args.ldc + col] = acc;
+                        if (col < args.N) emit1(args.out, m_lo + r, col, acc);
                     }
                 }
                 if (et == 0) HEAL_STAMP(args.trace, 9);

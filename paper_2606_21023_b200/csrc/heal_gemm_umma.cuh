@@ -15,6 +15,7 @@
 // lo.lo (those the mode keeps); segments are added in ascending order in FP32 RN.  Nothing here
 // depends on M, on the tile an element falls in, or on the SM that computes it.
 #pragma once
+#include "heal_epilogue.cuh"
 #include "heal_ptx.cuh"
 
 namespace heal {
@@ -44,8 +45,7 @@ struct GemmCfg {
 };
 
 struct GemmArgs {
-    float *C;
-    int64_t ldc;
+    OutArgs out;            // step E: FP32 C and/or hi/lo planes, optional 2^-p scale
     int M, N, K;
     int tiles_m, tiles_n;
     int *diag;
@@ -175,7 +175,7 @@ __device__ __forceinline__ void sk_wait(const uint32_t *ctr, uint32_t want, int 
 // The CTA that computed segment `seg` finishes float4 chunks [seg*NC/n_seg, (seg+1)*NC/n_seg) of every row:
 // ascending-segment FP32 RN sum of the n_seg partials, then the predicated store to C.
 template <int CPW>
-__device__ __forceinline__ void sk_finish(const float *part0, int n_seg, int seg, int etid, float *crow, int col0, int N, bool row_ok)
+__device__ __forceinline__ void sk_finish(const float *part0, int n_seg, int seg, int etid, const OutArgs &out, int64_t row, int col0, int N, bool row_ok)
 {
     constexpr int NC = CPW / 4;
     const int c_lo = seg * NC / n_seg, c_hi = (seg + 1) * NC / n_seg;
@@ -192,17 +192,7 @@ __device__ __forceinline__ void sk_finish(const float *part0, int n_seg, int seg
             acc.x = __fadd_rn(acc.x, v.x); acc.y = __fadd_rn(acc.y, v.y);
             acc.z = __fadd_rn(acc.z, v.z); acc.w = __fadd_rn(acc.w, v.w);
         }
-        if (row_ok) {
-            const int col = col0 + c4 * 4;
-            if (col + 3 < N) {
-                *reinterpret_cast<float4 *>(crow + col) = acc;
-            } else {
-                if (col < N) crow[col] = acc.x;
-                if (col + 1 < N) crow[col + 1] = acc.y;
-                if (col + 2 < N) crow[col + 2] = acc.z;
-                if (col + 3 < N) crow[col + 3] = acc.w;
-            }
-        }
+        if (row_ok) emit4(out, row, col0 + c4 * 4, acc, N);
     }
 }
 // last finisher of a (tile, rank): re-arm both counters for the next launch on this stream
@@ -460,18 +450,9 @@ heal_gemm_umma_kernel(const __grid_constant__ CUtensorMap tm_a_hi, const __grid_
             const int row = m0 + quad * 32 + lane;
             const int col0 = n0 + chalf * CPW;
             if (row < args.M) {
-                float *crow = args.C + static_cast<int64_t>(row) * args.ldc;
 #pragma unroll
-                for (int c = 0; c < CPW; c += 4) {
-                    const int col = col0 + c;
-                    if (col + 3 < args.N) {
-                        *reinterpret_cast<float4 *>(crow + col) = make_float4(run[c], run[c + 1], run[c + 2], run[c + 3]);
-                    } else {
-#pragma unroll
-                        for (int i = 0; i < 4; ++i)
-                            if (col + i < args.N) crow[col + i] = run[c + i];
-                    }
-                }
+                for (int c = 0; c < CPW; c += 4)
+                    emit4(args.out, row, col0 + c, make_float4(run[c], run[c + 1], run[c + 2], run[c + 3]), args.N);
             }
         }
         if (args.sk) {
@@ -485,7 +466,7 @@ heal_gemm_umma_kernel(const __grid_constant__ CUtensorMap tm_a_hi, const __grid_
                 sk_wait(args.cnt + 2 * tile, static_cast<uint32_t>(n_seg), etid, args.diag);
                 for (int seg = sb_seg; seg < se_seg; ++seg) {
                     sk_finish<CPW>(args.part + static_cast<size_t>(tile) * n_seg * (kBM * BN), n_seg, seg, etid,
-                                   args.C + static_cast<int64_t>(row) * args.ldc, n0 + chalf * CPW, args.N, row < args.M);
+                                   args.out, row, n0 + chalf * CPW, args.N, row < args.M);
                     sk_done(args.cnt + 2 * tile, static_cast<uint32_t>(n_seg), etid);
                 }
             }

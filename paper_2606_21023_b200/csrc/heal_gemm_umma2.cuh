@@ -273,18 +273,9 @@ heal_gemm_umma2_kernel(const __grid_constant__ CUtensorMap tm_a_hi, const __grid
             const int row = m0 + quad * 32 + lane;
             const int col0 = n0 + chalf * CPW;
             if (row < args.M) {
-                float *crow = args.C + static_cast<int64_t>(row) * args.ldc;
 #pragma unroll
-                for (int c = 0; c < CPW; c += 4) {
-                    const int col = col0 + c;
-                    if (col + 3 < args.N) {
-                        *reinterpret_cast<float4 *>(crow + col) = make_float4(run[c], run[c + 1], run[c + 2], run[c + 3]);
-                    } else {
-#pragma unroll
-                        for (int i = 0; i < 4; ++i)
-                            if (col + i < args.N) crow[col + i] = run[c + i];
-                    }
-                }
+                for (int c = 0; c < CPW; c += 4)
+                    emit4(args.out, row, col0 + c, make_float4(run[c], run[c + 1], run[c + 2], run[c + 3]), args.N);
             }
         }
         if (args.sk) {
@@ -298,7 +289,7 @@ heal_gemm_umma2_kernel(const __grid_constant__ CUtensorMap tm_a_hi, const __grid
                 sk_wait(ctr, static_cast<uint32_t>(n_seg), etid, args.diag);
                 for (int seg = sb_seg; seg < se_seg; ++seg) {
                     sk_finish<CPW>(args.part + (static_cast<size_t>(tile) * 2 + rank) * n_seg * (kBM * BN), n_seg, seg, etid,
-                                   args.C + static_cast<int64_t>(row) * args.ldc, n0 + chalf * CPW, args.N, row < args.M);
+                                   args.out, row, n0 + chalf * CPW, args.N, row < args.M);
                     sk_done(ctr, static_cast<uint32_t>(n_seg), etid);
                 }
             }

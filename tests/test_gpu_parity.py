@@ -396,6 +396,65 @@ def test_ordered_split_k_mid_m(hb, oracle, inputs, M, N, K, nprod):
     assert oracle.normwise_error(full.cpu().numpy(), oracle.gemm_f64(A, B), A, B) <= GATE
 
 
+@pytest.mark.parametrize("M,N,K,nprod", [(1, 1030, 4096, 2), (8, 130, 1024, 2), (32, 4096, 4096, 2), (64, 262, 8192, 2), (40, 128256 // 8, 512, 2),
+                                         (128, 1030, 4096, 2), (300, 522, 2056, 3), (1300, 4102, 1032, 2), (2048, 2048, 512, 1)])
+def test_extended_epilogue_scale_and_chained_planes(hb, inputs, M, N, K, nprod):
+    """heal_gemm_ex: the 2^-p output scale is exact, and the chained hi/lo planes are bit for bit heal_split() of the
+    scaled FP32 output -- through every kernel family (small-M single/cluster, single-CTA, CTA pairs, ordered split-K),
+    with ragged N, with and without the FP32 output."""
+    A = dev(inputs.activations(M, K, seed=15, outliers=True))
+    B = dev_padded(inputs.weights_f32(K, N, seed=15) if nprod >= 3 else inputs.weights_f16(K, N, seed=15), (-N) % 8)
+    ld = (N + 3) // 4 * 4
+    ref = hb.heal_gemm(A, B, nprod, C=torch.zeros((M, ld), device="cuda")[:, :N])
+    for p_exp in (0, 3, -2):
+        want = ref * (2.0 ** -p_exp)
+        C, hi, lo = hb.heal_gemm_ex(A, B, nprod, C=torch.zeros((M, ld), device="cuda")[:, :N], scale_exp=p_exp)
+        assert torch.equal(C, want)
+        wp = torch.zeros((M, ld), device="cuda")
+        wp[:, :N] = want
+        whi, wlo = hb.heal_split(wp[:, :N])
+        assert torch.equal(hi.view(torch.int16), whi.view(torch.int16)) and torch.equal(lo.view(torch.int16), wlo.view(torch.int16))
+        _, hi2, lo2 = hb.heal_gemm_ex(A, B, nprod, want_c=False, scale_exp=p_exp)          # planes only
+        assert torch.equal(hi2.view(torch.int16), whi.view(torch.int16)) and torch.equal(lo2.view(torch.int16), wlo.view(torch.int16))
+
+
+def test_chained_planes_feed_next_gemm(hb, oracle, inputs):
+    """Two compensated GEMMs back to back: the first one's epilogue emits the hi/lo planes the second consumes
+    (no FP32 round trip, no split pass).  Same bits as the unchained path; end result inside the gate vs FP64."""
+    M, K1, N1, N2 = 200, 2048, 1032, 520
+    A = inputs.activations(M, K1, seed=16, outliers=True)
+    W1 = inputs.weights_f16(K1, N1, seed=16)
+    W2 = inputs.weights_f16(N1, N2, seed=17)
+    Ad, W1d, W2d = dev(A), dev(W1), dev(W2)
+    H = hb.heal_gemm(Ad, W1d, 2)
+    want = hb.heal_gemm(H, W2d, 2)
+    _, hi, lo = hb.heal_gemm_ex(Ad, W1d, 2, want_c=False)
+    got = hb.heal_gemm_presplit(hi, lo, W2d, None, 2)
+    assert torch.equal(got, want)
+    Href = oracle.gemm_f64(A, W1).astype(np.float32)          # the FP32 hand-over is part of the method (PAPER.md:563)
+    assert oracle.normwise_error(got.cpu().numpy(), oracle.gemm_f64(H.cpu().numpy(), W2), H.cpu().numpy(), W2) <= GATE
+    assert np.abs(H.cpu().numpy() - Href).max() <= 1e-4 * np.abs(Href).max()
+
+
+def test_extended_epilogue_errors(hb):
+    A = torch.zeros((8, 64), device="cuda")
+    W = torch.zeros((64, 16), dtype=torch.float16, device="cuda")
+    C = torch.zeros((8, 16), device="cuda")
+    hi = torch.zeros((8, 16), dtype=torch.float16, device="cuda")
+    lo = torch.zeros_like(hi)
+    L = hb.lib()
+    f = lambda c, h, l, ld16, p: L.heal_gemm_ex(8, 16, 64, A.data_ptr(), 64, W.data_ptr(), 16, c, 16, h, l, ld16, p, 2, None)
+    assert f(C.data_ptr(), hi.data_ptr(), lo.data_ptr(), 16, 0) == 0
+    assert f(None, hi.data_ptr(), lo.data_ptr(), 16, 0) == 0
+    assert f(None, None, None, 0, 0) == 2                       # no output at all
+    assert f(C.data_ptr(), hi.data_ptr(), None, 16, 0) == 2     # one plane only
+    assert f(C.data_ptr(), hi.data_ptr(), lo.data_ptr(), 8, 0) == 1       # ldc16 < N
+    assert f(C.data_ptr(), hi.data_ptr(), lo.data_ptr(), 20, 0) == 3      # ldc16 % 8
+    assert f(C.data_ptr(), hi.data_ptr() + 2, lo.data_ptr(), 16, 0) == 3  # misaligned plane
+    assert f(C.data_ptr(), None, None, 0, 127) == 1             # scale exponent out of range
+    torch.cuda.synchronize()
+
+
 def test_static_weights_graph_chain(hb, inputs):
     """HEAL_B_STATIC in a captured chain of decode GEMMs (each kernel streams its weights while its predecessor
     finishes; activations and C wait): every replay reproduces the eager results bit for bit, including a chain
