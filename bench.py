@@ -128,6 +128,55 @@ def run_reference(args):
         "gpu_launches": 0}))
 
 
+def small_m_report(hb, peaks):
+    """HBM-bound shapes of BASELINE.json configs[1] (decode 4096x4096, M = 1/8/32) and configs[4] (LM head, M = 1/64):
+    achieved GB/s = (2KN + 4MK + 4MN) / t through heal_gemm (device buffers; one fused kernel for M <= 16), timed as a
+    CUDA graph of back-to-back calls rotating over enough distinct weight copies to exceed the 126 MB L2."""
+    import torch
+    out = {}
+    for tag, M, N, K in [("decode_M1", 1, 4096, 4096), ("decode_M8", 8, 4096, 4096), ("decode_M32", 32, 4096, 4096),
+                         ("lm_head_M1", 1, 128256, 4096), ("lm_head_M64", 64, 128256, 4096)]:
+        gen = torch.Generator(device="cuda")
+        gen.manual_seed(7)
+        ncopies = max(2, min(12, int(3 * 126e6 // (K * N * 2)) + 1))
+        A = torch.randn(M, K, device="cuda", generator=gen)
+        Ws = [(torch.randn(K, N, device="cuda", generator=gen) * 0.02).half() for _ in range(ncopies)]
+        C = torch.empty(M, N, device="cuda")
+        ws = torch.empty(max(256, hb.workspace_size(M, N, K, hb.MODE_2P)), dtype=torch.uint8, device="cuda")
+        hb.set_workspace(ws)
+        byt = K * N * 2 + M * K * 4 + M * N * 4
+        res = {}
+        for name, mode in (("heal_gemm", hb.MODE_2P), ("heal_gemm+B_STATIC", hb.MODE_2P | hb.B_STATIC)):
+            s = torch.cuda.Stream()
+            with torch.cuda.stream(s):
+                for W in Ws:
+                    hb.heal_gemm(A, W, mode, C=C)
+                s.synchronize()
+                g = torch.cuda.CUDAGraph()
+                reps = 2 if ncopies < 8 else 1
+                with torch.cuda.graph(g, stream=s):
+                    for _ in range(reps):
+                        for W in Ws:
+                            hb.heal_gemm(A, W, mode, C=C)
+                g.replay()
+                s.synchronize()
+                ts = []
+                for _ in range(5):
+                    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                    e0.record(s)
+                    g.replay()
+                    e1.record(s)
+                    s.synchronize()
+                    ts.append(e0.elapsed_time(e1) * 1e3 / (reps * ncopies))
+            t = sorted(ts)[2]
+            res[name] = {"us": t, "GB/s": byt / t / 1e3, "frac_of_measured_hbm_peak": byt / t / 1e3 / peaks["hbm"]}
+        out[tag] = res
+        hb.set_workspace(None)
+        del Ws
+        torch.cuda.empty_cache()
+    return out
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -233,7 +282,8 @@ def run_ours(args):
             "roofline": {"bound": "tensor", "kernel": "heal_gemm_umma2_kernel<BN=256,2P> (CTA pairs)", "achieved": achieved, "peak": peak,
                          "unit": "TFLOP/s", "frac": achieved / peak, "traffic": traffic,
                          "peak_kind": f"{peaks['src']} cuBLAS bf16 {'sustained' if long_run else 'burst'} (fp16 = bf16 rate)",
-                         "frac_of_nominal_2250": achieved / 2250.0, "avg_launch_ms": ms_gemm,
+                         "frac_of_nominal_2250": achieved / 2250.0, "frac_of_measured_burst": achieved / peaks["burst"],
+                         "frac_of_measured_sustained": achieved / peaks["sustained"], "avg_launch_ms": ms_gemm,
                          "flops_per_launch": flop_launch},
             "e2e": {"value": world * FLOP_STEP / (ms_e2e * 1e-3) / 1e12, "unit": UNIT, "h2d_bytes_per_step": h2d,
                     "d2h_bytes_per_step": d2h, "ms_per_step": ms_e2e},
@@ -247,9 +297,19 @@ def run_ours(args):
                                     "sample": f"{rows_n} evenly spaced rows of each of the two GEMMs (full N and K)"}
             import oracle
             errs = {}
-            for (name, A, W), (_, _, _, C), ref in zip(data, devs, refs):
+            contrast = {}
+            torch.backends.cuda.matmul.allow_tf32 = False
+            for (name, A, W), (_, Ad, Wd, C), ref in zip(data, devs, refs):
                 errs[name] = oracle.normwise_error(C.cpu().numpy(), ref, A, W, rows=rows)
+                # context (north_star): the same inputs through plain 16-bit GEMMs and cuBLAS SGEMM, scored the same way
+                e = lambda X: oracle.normwise_error(X.float().cpu().numpy(), ref, A, W, rows=rows)
+                contrast[name] = {"heal_2P": errs[name],
+                                  "plain_fp16_1P (heal_gemm mode 1)": e(hb.heal_gemm(Ad, Wd, hb.MODE_1P)),
+                                  "plain_bf16 (cuBLAS, bf16 out)": e(torch.matmul(Ad.bfloat16(), Wd.bfloat16())),
+                                  "sgemm_fp32 (cuBLAS, TF32 off)": e(torch.matmul(Ad, Wd.float()))}
             line["normwise_err_vs_fp64"] = errs
+            line["error_contrast_vs_fp64"] = contrast
+            line["small_m"] = small_m_report(hb, peaks)
         print(json.dumps(line))
     hb.set_workspace(None)
     if world > 1:
@@ -259,7 +319,7 @@ def run_ours(args):
 if __name__ == "__main__":
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--steps", type=int, default=1500)      # > 1 s of back-to-back GEMMs: the sustained (power-capped) regime
     ap.add_argument("--warmup", type=int, default=10)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     a = ap.parse_args()

@@ -447,12 +447,24 @@ int launch_small_cfg(int64_t M, int64_t N, int64_t K, const SmallIn &in, const v
         if (want == 1 || want == 2 || want == 4 || want == 8) cs = want <= n_seg ? want : cs;
     }
     int max_local = (n_seg + cs - 1) / cs;
-    while (max_local * Cfg::MPAD > 512 && cs * 2 <= 8 && cs * 2 <= n_seg) {
+    // One CTA per panel reading planes, and the segments would need more than 256 TMEM columns (one CTA per SM):
+    // they cycle through a ring of TMEM slots instead (256 columns, so two CTAs fit per SM and one's epilogue
+    // overlaps the other's stream) and the epilogue keeps the running sum.  Measured: LM head M = 64 227 -> 202 us;
+    // where everything fits in 256 columns anyway the plain "drain at the end" epilogue is faster (LM head M = 1
+    // 161 vs 168 us), so the ring is used only when needed.
+    const bool use_ring = cs == 1 && !Cfg::FUSED && n_seg * Cfg::MPAD > 256;
+    int ring = 0;
+    if (use_ring) {
+        ring = 256 / Cfg::MPAD;
+        if (ring > n_seg) ring = n_seg;
+        if (ring > 16) ring = 16;
+    }
+    while (!use_ring && max_local * Cfg::MPAD > 512 && cs * 2 <= 8 && cs * 2 <= n_seg) {
         cs *= 2;
         max_local = (n_seg + cs - 1) / cs;
     }
     int tmem_cols = 32;
-    while (tmem_cols < max_local * Cfg::MPAD) tmem_cols *= 2;
+    while (tmem_cols < (use_ring ? ring : max_local) * Cfg::MPAD) tmem_cols *= 2;
     if (tmem_cols > 512) return HEAL_OK;                        // leave to the large-M kernel
     const int rpr = cs > 1 ? static_cast<int>((M + cs - 1) / cs) : 0;
     const size_t red = cs > 1 ? static_cast<size_t>(n_seg) * rpr * kSmallBNW * 4 : 0;
@@ -525,6 +537,7 @@ int launch_small_cfg(int64_t M, int64_t N, int64_t K, const SmallIn &in, const v
     args.rows_per_rank = rpr;
     args.red_bytes = static_cast<int>(red);
     args.red_alias = red_alias ? 1 : 0;
+    args.ring = ring;
     static const bool no_static = std::getenv("HEAL_NO_STATIC") != nullptr;       // debug only
     args.b_static = (in.b_static && !no_static) ? 1 : 0;
     args.diag = g.diag;

@@ -49,7 +49,7 @@ struct SmallCfg {
     static constexpr int STAGE_BYTES = B_PLANES * W_TILE + A_PLANES * X_TILE_AL;
     static constexpr int W_BYTES = B_PLANES * W_TILE;
     static constexpr int TX_BYTES = W_BYTES + (FUSED ? 0 : A_PLANES * X_TILE);
-    static constexpr int BAR_BYTES = 256;
+    static constexpr int BAR_BYTES = 512;
     static constexpr int TASKS = MPAD / 16;             // FUSED: 8-float chunks per converter thread per k-tile
     static constexpr int PF = MPAD <= 32 ? 4 : 2;       // FUSED: k-tiles of activations kept in flight in registers
     static_assert(MPAD % 16 == 0 && MPAD >= 16 && MPAD <= 64, "MPAD");
@@ -69,6 +69,8 @@ struct SmallArgs {
     int red_bytes;        // CS > 1: n_seg * rows_per_rank * 128 floats of partial sums pushed by the cluster
     int red_alias;        // the pushed partial sums reuse the pipeline stages (large M * K): needs a second cluster
                           // barrier ("every rank's main loop is over") before anybody pushes
+    int ring;             // CS == 1, planes: number of TMEM slots the segments cycle through (0 = every local
+                          // segment keeps its own slot until the end)
     int b_static;         // HEAL_B_STATIC: W may be read before the stream predecessor has completed
     int *diag;
     unsigned long long *trace;   // phase stamps (HEAL_TRACE builds only), else unused
@@ -99,6 +101,9 @@ heal_gemm_smallm_kernel(const __grid_constant__ CUtensorMap tm_x_hi, const __gri
     const uint32_t done_bar = bar_base + 192u;
     const uint32_t red_bar = bar_base + 200u;
     const uint32_t tmem_slot = bar_base + 208u;
+    auto tfull_bar = [&](int j) { return bar_base + 256u + 8u * j; };      // ring: slot j holds a finished segment
+    auto tempty_bar = [&](int j) { return bar_base + 384u + 8u * j; };     // ring: slot j has been drained (4 warps)
+    const int ring = args.ring;
     volatile uint32_t *tmem_slot_ptr = reinterpret_cast<volatile uint32_t *>(smem_raw + (tmem_slot - smem_u32(smem_raw)));
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -131,6 +136,10 @@ heal_gemm_smallm_kernel(const __grid_constant__ CUtensorMap tm_x_hi, const __gri
         }
         mbar_init(done_bar, 1);
         mbar_init(red_bar, cs * 4);                      // one arrival per epilogue warp of every rank
+        for (int j = 0; j < ring; ++j) {
+            mbar_init(tfull_bar(j), 1);
+            mbar_init(tempty_bar(j), 4);
+        }
         fence_mbar_init();
     }
     if (warp == 1) {
@@ -150,7 +159,8 @@ heal_gemm_smallm_kernel(const __grid_constant__ CUtensorMap tm_x_hi, const __gri
     tc_fence_before();
     __syncthreads();
     if (threadIdx.x == 0) HEAL_STAMP(args.trace, 12);
-    if (cs > 1) cluster_arrive();                        // matched by cluster_wait() before the first remote access
+    if (cs > 1) cluster_arrive_relaxed();                // matched by cluster_wait() before the first remote access
+                                                         // (the barrier inits were published by fence.mbarrier_init)
     tc_fence_after();
     const uint32_t tmem_base = *tmem_slot_ptr;
     if (threadIdx.x == 0) HEAL_STAMP(args.trace, 1);
@@ -231,8 +241,16 @@ heal_gemm_smallm_kernel(const __grid_constant__ CUtensorMap tm_x_hi, const __gri
             uint32_t phase = 0;
             uint32_t accumulate = 0;
             for (int t = 0; t < n_t; ++t) {
-                if ((t & 7) == 0) accumulate = 0;                 // new segment -> new TMEM slot
-                const uint32_t d_tmem = tmem_base + static_cast<uint32_t>((t >> 3) * MPAD);
+                const int seg_j = t >> 3;
+                const int slot = ring ? seg_j % ring : seg_j;
+                if ((t & 7) == 0) {                               // new segment -> next TMEM slot
+                    accumulate = 0;
+                    if (ring && seg_j >= ring) {                  // the slot's previous segment must have been drained
+                        mbar_wait(tempty_bar(slot), static_cast<uint32_t>((seg_j / ring - 1) & 1), args.diag, 640 + slot);
+                        tc_fence_after();
+                    }
+                }
+                const uint32_t d_tmem = tmem_base + static_cast<uint32_t>(slot * MPAD);
                 mbar_wait(full_bar(stage), phase, args.diag, 600 + stage);
                 if (FUSED) mbar_wait(xfull_bar(stage), phase, args.diag, 620 + stage);
                 tc_fence_after();
@@ -258,6 +276,7 @@ heal_gemm_smallm_kernel(const __grid_constant__ CUtensorMap tm_x_hi, const __gri
                     if (NPROD == 4) umma_f16(d_tmem, w_lo + wo, x_lo + xo, idesc, 1);
                 }
                 umma_commit(empty_bar(stage));
+                if (ring && ((t & 7) == 7 || t == n_t - 1)) umma_commit(tfull_bar(slot));      // segment complete
                 if (++stage == STAGES) { stage = 0; phase ^= 1u; }
             }
             umma_commit(done_bar);                         // all local segments complete in TMEM
@@ -339,6 +358,49 @@ heal_gemm_smallm_kernel(const __grid_constant__ CUtensorMap tm_x_hi, const __gri
         const int quad = warp & 3;
         const int nl = quad * 32 + lane;                   // weight column within the panel = TMEM lane
         const int col = n0 + nl;
+        if (cs == 1 && ring) {
+            // single-CTA panel, ring of TMEM slots: drain each finished segment into the ascending FP32 RN running sum
+            // while the tensor core fills the next slot
+            float acc[MPAD / 16][16];
+            for (int j = 0; j < n_local; ++j) {
+                const int slot = j % ring;
+                mbar_wait(tfull_bar(slot), static_cast<uint32_t>((j / ring) & 1), args.diag, 660 + slot);
+                tc_fence_after();
+#pragma unroll
+                for (int c = 0; c < MPAD / 16; ++c) {
+                    if (c * 16 < args.M) {
+                        uint32_t v[16];
+                        tmem_ld_32x32b_x16(tmem_base + (static_cast<uint32_t>(quad * 32) << 16) + static_cast<uint32_t>(slot * MPAD + c * 16), v);
+                        tmem_ld_wait();
+                        if (j == 0) {
+#pragma unroll
+                            for (int i = 0; i < 16; ++i) acc[c][i] = __uint_as_float(v[i]);
+                        } else {
+#pragma unroll
+                            for (int i = 0; i < 16; ++i) acc[c][i] = __fadd_rn(acc[c][i], __uint_as_float(v[i]));
+                        }
+                    }
+                }
+                tc_fence_before();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(tempty_bar(slot));
+            }
+            if (et == 0) HEAL_STAMP(args.trace, 6);
+            if (col < args.N) {
+                emit_dispatch(args.out, [&](const OutArgs &po, auto has_c, auto has_p) {
+#pragma unroll
+                    for (int c = 0; c < MPAD / 16; ++c)
+#pragma unroll
+                        for (int i = 0; i < 16; ++i)
+                            if (c * 16 + i < args.M) emit1<decltype(has_c)::value, decltype(has_p)::value>(po, c * 16 + i, col, acc[c][i]);
+                });
+            }
+            if (et == 0) HEAL_STAMP(args.trace, 7);
+            mbar_wait(done_bar, 0, args.diag, 700);        // every MMA (and its commits) has retired before the CTA leaves
+            tc_fence_after();
+            tc_fence_before();
+            if (et == 0) HEAL_STAMP(args.trace, 8);
+        } else {
         mbar_wait(done_bar, 0, args.diag, 700);
         tc_fence_after();
         if (et == 0) HEAL_STAMP(args.trace, 6);
@@ -361,9 +423,11 @@ heal_gemm_smallm_kernel(const __grid_constant__ CUtensorMap tm_x_hi, const __gri
                         for (int i = 0; i < 16; ++i) acc[i] = __fadd_rn(acc[i], __uint_as_float(v[i]));
                     }
                     if (col < args.N) {
+                        emit_dispatch(args.out, [&](const OutArgs &po, auto has_c, auto has_p) {
 #pragma unroll
-                        for (int i = 0; i < 16; ++i)
-                            if (c * 16 + i < args.M) emit1(args.out, c * 16 + i, col, acc[i]);
+                            for (int i = 0; i < 16; ++i)
+                                if (c * 16 + i < args.M) emit1<decltype(has_c)::value, decltype(has_p)::value>(po, c * 16 + i, col, acc[i]);
+                        });
                     }
                 }
             }
@@ -409,9 +473,13 @@ heal_gemm_smallm_kernel(const __grid_constant__ CUtensorMap tm_x_hi, const __gri
                 }
             }
             tc_fence_before();
-            fence_acq_rel_cluster();
             __syncwarp();
-            if (lane < owners) mbar_arrive_cluster(map_to_cta(red_bar, static_cast<uint32_t>(lane)));
+            // one fence per signalling lane (cumulative over the warp's pushes, ordered by the __syncwarp) and a
+            // relaxed remote arrive: a cluster-scope release costs ~0.5 us each on this part (measured), so pay it once
+            if (lane < owners) {
+                fence_acq_rel_cluster();
+                mbar_arrive_relaxed_cluster(map_to_cta(red_bar, static_cast<uint32_t>(lane)));
+            }
             if (et == 0) HEAL_STAMP(args.trace, 7);
             if (static_cast<int>(rank) < owners) {
                 mbar_wait_cluster(red_bar, 0, args.diag, 710);
@@ -432,10 +500,13 @@ heal_gemm_smallm_kernel(const __grid_constant__ CUtensorMap tm_x_hi, const __gri
                             acc.z = __fadd_rn(acc.z, v.z); acc.w = __fadd_rn(acc.w, v.w);
                         }
                         if (col < args.N) {
-                            emit1(args.out, m_lo + r4, col, acc.x);
-                            if (r4 + 1 < rows) emit1(args.out, m_lo + r4 + 1, col, acc.y);
-                            if (r4 + 2 < rows) emit1(args.out, m_lo + r4 + 2, col, acc.z);
-                            if (r4 + 3 < rows) emit1(args.out, m_lo + r4 + 3, col, acc.w);
+                            emit_dispatch(args.out, [&](const OutArgs &po, auto has_c, auto has_p) {
+                                constexpr bool kc = decltype(has_c)::value, kp = decltype(has_p)::value;
+                                emit1<kc, kp>(po, m_lo + r4, col, acc.x);
+                                if (r4 + 1 < rows) emit1<kc, kp>(po, m_lo + r4 + 1, col, acc.y);
+                                if (r4 + 2 < rows) emit1<kc, kp>(po, m_lo + r4 + 2, col, acc.z);
+                                if (r4 + 3 < rows) emit1<kc, kp>(po, m_lo + r4 + 3, col, acc.w);
+                            });
                         }
                     }
                 } else {
@@ -444,15 +515,21 @@ heal_gemm_smallm_kernel(const __grid_constant__ CUtensorMap tm_x_hi, const __gri
                         float acc = src[0];
 #pragma unroll 4
                         for (int s = 1; s < args.n_seg; ++s) acc = __fadd_rn(acc, src[static_cast<size_t>(s) * seg_stride]);
-                        if (col < args.N) emit1(args.out, m_lo + r, col, acc);
+                        if (col < args.N) {
+                            emit_dispatch(args.out, [&](const OutArgs &po, auto has_c, auto has_p) {
+                                emit1<decltype(has_c)::value, decltype(has_p)::value>(po, m_lo + r, col, acc);
+                            });
+                        }
                     }
                 }
                 if (et == 0) HEAL_STAMP(args.trace, 9);
             }
         }
+        }
     }
 
     __syncthreads();
+    if (threadIdx.x == 64) HEAL_STAMP(args.trace, 9);
     if (warp == 1) {
         tc_fence_after();
         tmem_dealloc(tmem_base, static_cast<uint32_t>(args.tmem_cols));

@@ -89,12 +89,14 @@ def bench_shape(name, M, N, K, nprod, dist, rows):
     ws = torch.empty(max(256, hb.workspace_size(M, N, K, nprod)), dtype=torch.uint8, device="cuda")
     hb.set_workspace(ws)
     full = [(lambda b=b: hb.heal_gemm(A, b, nprod, C)) for b in Bs]
+    full_st = [(lambda b=b: hb.heal_gemm(A, b, nprod | hb.B_STATIC, C)) for b in Bs]
     ah, al = hb.heal_split(A)
     planes = [(hb.heal_split(b) if nprod >= 3 else (b, None)) for b in Bs]
     pres = [(lambda p=p: hb.heal_gemm_presplit(ah, al, p[0], p[1], nprod, C)) for p in planes]
     reps = (2 if small else 1)
     t_full = _time(full * reps, small)
     t_pre = _time(pres * reps, small)
+    t_st = _time(full_st * reps, small) if M <= 64 else None
     # context: cuBLAS on the same inputs
     torch.backends.cuda.matmul.allow_tf32 = False
     A16, Ab = A.half(), A.bfloat16()
@@ -109,7 +111,8 @@ def bench_shape(name, M, N, K, nprod, dist, rows):
     flop = 2.0 * M * N * K
     byt = K * N * 2 + M * K * 4 + M * N * 4
     burst, sust, hbm, _ = _peaks()
-    rows.append(f"| {name} | {M}x{N}x{K} | {nprod}P | {t_full[1]:.1f} | {t_pre[1]:.1f} ({t_pre[0]:.1f}) | "
+    st_col = "-" if t_st is None else f"{t_st[1]:.1f} ({byt / t_st[1] / 1e3:.0f} GB/s, {byt / t_st[1] / 1e3 / hbm * 100:.0f}%)"
+    rows.append(f"| {name} | {M}x{N}x{K} | {nprod}P | {t_full[1]:.1f} | {st_col} | {t_pre[1]:.1f} ({t_pre[0]:.1f}) | "
                 f"{flop / t_pre[1] / 1e6:.1f} | {nprod * flop / t_pre[1] / 1e6:.0f} ({nprod * flop / t_pre[1] / 1e6 / burst * 100:.0f}% / "
                 f"{nprod * flop / t_pre[1] / 1e6 / 2250 * 100:.0f}%) | {byt / t_pre[1] / 1e3:.0f} ({byt / t_pre[1] / 1e3 / hbm * 100:.0f}%) | "
                 f"{t_sgemm[1]:.1f} | {t_f16[1]:.1f} | {t_bf16[1]:.1f} | {'graph+rot%d' % ncopies if small else 'loop'} |")
@@ -125,17 +128,26 @@ def main():
     cfgs += [("cfg2 MLP up/gate", 2048, 14336, 4096, 2, "normal"), ("cfg2 MLP down", 2048, 4096, 14336, 2, "normal")]
     cfgs += [(f"cfg3 square {n}", n, n, n, 3, "uniform") for n in (1024, 2048, 4096, 8192)]
     cfgs += [(f"cfg4 LM head M={m}", m, 128256, 4096, 2, "normal") for m in (1, 64, 512)]
+    # beyond BASELINE.json: the other GEMM sites of a decoder layer at Llama-3-8B and
+    # Qwen3-14B shapes, batched decode on the down projection, and the mid-size M where HBM-bound turns MMA-bound
+    cfgs += [("L3-8B qkv", 2048, 6144, 4096, 2, "normal"), ("L3-8B o-proj", 2048, 4096, 4096, 2, "normal"),
+             ("Q3-14B up/gate", 2048, 17408, 5120, 2, "normal"), ("Q3-14B down", 2048, 5120, 17408, 2, "normal"),
+             ("Q3-14B qkv", 2048, 7168, 5120, 2, "normal")]
+    cfgs += [(f"decode down M={m}", m, 4096, 14336, 2, "normal") for m in (1, 32)]
+    cfgs += [(f"decode M={m}", m, 4096, 4096, 2, "normal") for m in (64,)]
+    cfgs += [(f"mid M={m}", m, 4096, 4096, 2, "normal") for m in (128, 256, 512, 1024)]
     for c in cfgs:
         bench_shape(*c, rows)
     name = torch.cuda.get_device_name(0)
     print(f"# HEAL compensated GEMM on {name}: all BASELINE.json configs\n")
     print(f"Peaks ({src}): cuBLAS BF16 {burst:.0f} TFLOP/s burst / {sust:.0f} sustained; HBM copy {hbm:.0f} GB/s; nominal 2250 TFLOP/s, ~8 TB/s.\n")
-    print("Times are medians in microseconds (min in brackets); `full` = heal_gemm (split + GEMM), `G+E` = heal_gemm_presplit "
+    print("Times are medians in microseconds (min in brackets); `full` = heal_gemm (split + GEMM; one fused kernel for M <= 16), "
+          "`full + HEAL_B_STATIC` = the same call with the static-weights promise (weights stream before the dependency wait), `G+E` = heal_gemm_presplit "
           "(3P: weights pre-split, the static-weight case).  `tensor` = n_prod x effective rate, as % of measured burst / nominal peak.  "
           "GB/s = (2KN + 4MK + 4MN) / t, as % of the measured copy peak.  cuBLAS columns: torch.matmul on the same inputs "
           "(SGEMM with TF32 off; FP16 and BF16 with operands rounded, 16-bit output).\n")
-    print("| config | MxNxK | mode | full us | G+E us | eff TFLOP/s | tensor TFLOP/s (% burst / % nominal) | GB/s (% peak) | cuBLAS SGEMM us | cuBLAS FP16 us | cuBLAS BF16 us | timing |")
-    print("|---|---|---|---|---|---|---|---|---|---|---|---|")
+    print("| config | MxNxK | mode | full us | full + HEAL_B_STATIC us (M <= 64) | G+E us | eff TFLOP/s | tensor TFLOP/s (% burst / % nominal) | GB/s (% peak) | cuBLAS SGEMM us | cuBLAS FP16 us | cuBLAS BF16 us | timing |")
+    print("|---|---|---|---|---|---|---|---|---|---|---|---|---|")
     print("\n".join(rows))
 
 

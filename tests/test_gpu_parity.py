@@ -455,6 +455,26 @@ def test_extended_epilogue_errors(hb):
     torch.cuda.synchronize()
 
 
+@pytest.mark.parametrize("M,N,K,nprod,b_nk", [(64, 32064, 1024, 2, False), (40, 26760, 4096, 2, False), (33, 27000, 520, 2, True),
+                                              (64, 26624, 14336, 2, False), (64, 26624, 1536, 3, False), (20, 26624, 20480, 2, False)])
+def test_small_m_single_cta_panels_tmem_ring(hb, inputs, M, N, K, nprod, b_nk):
+    """Large N (one CTA per 128-column panel, no K split): the segment partials cycle through a ring of TMEM slots and
+    the epilogue warps keep the ascending running sum in registers while the tensor core works on the next segment.
+    Same bits as rows 0..15 submitted alone (fused kernel, all segments resident) and as the large-M kernels."""
+    A = dev(inputs.activations(M, K, seed=18, outliers=True))
+    B = inputs.weights_f32(K, N, seed=18, nk=b_nk) if nprod >= 3 else inputs.weights_f16(K, N, seed=18, nk=b_nk)
+    B = dev(B)
+    mode = nprod | (hb.B_NK if b_nk else 0)
+    got = hb.heal_gemm(A, B, mode).clone()
+    assert torch.equal(got[:16], hb.heal_gemm(A[:16], B, mode))
+    assert torch.equal(got, hb.heal_gemm(A, B, mode | hb.B_STATIC))
+    try:
+        hb.debug_force_kernel(1)
+        assert torch.equal(got, hb.heal_gemm(A, B, mode))
+    finally:
+        hb.debug_force_kernel(0)
+
+
 def test_static_weights_graph_chain(hb, inputs):
     """HEAL_B_STATIC in a captured chain of decode GEMMs (each kernel streams its weights while its predecessor
     finishes; activations and C wait): every replay reproduces the eager results bit for bit, including a chain
