@@ -65,6 +65,18 @@ typedef enum {
                                   (programmatic dependent launch); everything that reads A or writes C
                                   still waits for the predecessor.  Same bits with or without the flag. */
 
+#define HEAL_LO_SHIFT 10
+#define HEAL_LO_SCALED 0x40u   /* the paper's scaled residual, Eq. 10 as printed: h = h_hi +
+                                  h_lo / 2^10 with h_lo = r16((h - h_hi) * 2^10), C = GEMM(h_hi, W) +
+                                  GEMM(h_lo / 2^10, W).  Two-product mode only.  Computed the way the paper
+                                  computes it -- two FP16 tensor-core GEMMs summed into one FP32 output
+                                  (PAPER.md:571): the h_lo GEMM stores 2^-10 times its sum (exact), the h_hi GEMM
+                                  adds its own on top in FP32 RN; each keeps the reduction order above.  Differs
+                                  from the default (s = 0, one accumulator) only where h_lo would leave FP16's
+                                  normal range, i.e. for |h| < 2^-3 (reading A1); needs the FP32 output
+                                  C (not planes only) and costs two GEMM launches.  With heal_gemm_presplit(_ex)
+                                  A_lo must hold the scaled residual (heal_split_scaled with lo_shift = 10). */
+
 /*
  * C[M x N] (FP32) = A[M x K] (FP32) . B          one pass of the whole path: split, MMAs, epilogue.
  *   A    FP32, lda >= K elements; 16-byte aligned, lda % 4 == 0.  Read-only.
@@ -93,6 +105,11 @@ int heal_gemm(int64_t M, int64_t N, int64_t K,
  */
 int heal_split(int64_t rows, int64_t cols, const void *X, int64_t ldx,
                void *hi, void *lo, int64_t ld, void *stream);
+
+/* Step S with a scaled residual: lo[r][c] = r16((X[r][c] - hi[r][c]) * 2^lo_shift), 0 <= lo_shift <= 16
+ * (PAPER.md:203 uses 10).  heal_split(...) == heal_split_scaled(..., 0, stream). */
+int heal_split_scaled(int64_t rows, int64_t cols, const void *X, int64_t ldx,
+                      void *hi, void *lo, int64_t ld, int32_t lo_shift, void *stream);
 
 /*
  * Steps G + E on pre-split planes: C = sum of the products `mode` keeps.

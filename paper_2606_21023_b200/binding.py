@@ -16,6 +16,8 @@ LIB_PATH = os.path.join(_HERE, "libheal.so")
 MODE_1P, MODE_2P, MODE_3P, MODE_4P = 1, 2, 3, 4
 B_NK = 0x10
 B_STATIC = 0x20
+LO_SCALED = 0x40
+LO_SHIFT = 10
 K_SEGMENT = 512
 
 _lib = None
@@ -40,6 +42,8 @@ def lib():
         L.heal_gemm_host.argtypes = [i64, i64, i64, vp, i64, vp, i64, vp, i64, u32, vp]
         L.heal_split.restype = ci
         L.heal_split.argtypes = [i64, i64, vp, i64, vp, vp, i64, vp]
+        L.heal_split_scaled.restype = ci
+        L.heal_split_scaled.argtypes = [i64, i64, vp, i64, vp, vp, i64, ctypes.c_int32, vp]
         L.heal_gemm_presplit.restype = ci
         L.heal_gemm_presplit.argtypes = [i64, i64, i64, vp, vp, i64, vp, vp, i64, vp, i64, u32, vp]
         i32 = ctypes.c_int32
@@ -166,8 +170,8 @@ def heal_gemm_raw(M, N, K, A_ptr, lda, B_ptr, ldb, C_ptr, ldc, mode, stream_ptr=
     return lib().heal_gemm(M, N, K, A_ptr, lda, B_ptr, ldb, C_ptr, ldc, mode, stream_ptr)
 
 
-def heal_split(X: torch.Tensor, hi: torch.Tensor | None = None, lo: torch.Tensor | None = None, stream=None):
-    """(hi, lo) fp16 planes of the fp32 matrix X (step S)."""
+def heal_split(X: torch.Tensor, hi: torch.Tensor | None = None, lo: torch.Tensor | None = None, stream=None, lo_shift: int = 0):
+    """(hi, lo) fp16 planes of the fp32 matrix X (step S); lo = r16((x - hi) * 2^lo_shift)."""
     assert X.is_cuda and X.dtype == torch.float32 and X.dim() == 2
     rows, cols = X.shape
     if hi is None:
@@ -175,7 +179,8 @@ def heal_split(X: torch.Tensor, hi: torch.Tensor | None = None, lo: torch.Tensor
         hi = torch.empty((rows, ld), dtype=torch.float16, device=X.device)[:, :cols]
         lo = torch.empty((rows, ld), dtype=torch.float16, device=X.device)[:, :cols]
     assert _ld(hi) == _ld(lo)
-    _check(lib().heal_split(rows, cols, X.data_ptr(), _ld(X), hi.data_ptr(), lo.data_ptr(), _ld(hi), _stream(stream)))
+    _check(lib().heal_split_scaled(rows, cols, X.data_ptr(), _ld(X), hi.data_ptr(), lo.data_ptr(), _ld(hi), lo_shift,
+                                   _stream(stream)))
     return hi, lo
 
 

@@ -146,7 +146,7 @@ int fill_attrs(cudaLaunchAttribute *attr, unsigned cluster_x)
 
 // ---- step S launch --------------------------------------------------------------------------
 int launch_split(int64_t rows, int64_t cols, const float *X, int64_t ldx, __half *hi, __half *lo, int64_t ld,
-                 cudaStream_t stream)
+                 cudaStream_t stream, int lo_shift = 0)
 {
     if (rows == 0 || cols == 0) return HEAL_OK;
     const int64_t vecs = rows * ((cols + 7) / 8);
@@ -160,7 +160,8 @@ int launch_split(int64_t rows, int64_t cols, const float *X, int64_t ldx, __half
     cudaLaunchAttribute attr[2];
     cfg.numAttrs = fill_attrs(attr, 1);
     cfg.attrs = attr;
-    HEAL_CUDA(cudaLaunchKernelEx(&cfg, heal_split_kernel, X, ldx, rows, cols, hi, lo, ld));
+    const float lo_scale = static_cast<float>(1u << lo_shift);                   // 2^s, s in [0, 16]
+    HEAL_CUDA(cudaLaunchKernelEx(&cfg, heal_split_kernel, X, ldx, rows, cols, hi, lo, ld, lo_scale));
     g_launches.fetch_add(1);
     return HEAL_OK;
 }
@@ -607,9 +608,10 @@ int forced_kernel()
 
 int validate_mode(uint32_t mode, int *nprod, bool *b_nk)
 {
-    if (mode & ~(HEAL_MODE_PRODUCTS_MASK | HEAL_B_NK | HEAL_B_STATIC)) return HEAL_ERR_UNSUPPORTED_MODE;
+    if (mode & ~(HEAL_MODE_PRODUCTS_MASK | HEAL_B_NK | HEAL_B_STATIC | HEAL_LO_SCALED)) return HEAL_ERR_UNSUPPORTED_MODE;
     const uint32_t p = mode & HEAL_MODE_PRODUCTS_MASK;
     if (p < 1 || p > 4) return HEAL_ERR_UNSUPPORTED_MODE;
+    if ((mode & HEAL_LO_SCALED) && p != 2) return HEAL_ERR_UNSUPPORTED_MODE;      // Eq. 10 as printed: two products only
     *nprod = static_cast<int>(p);
     *b_nk = (mode & HEAL_B_NK) != 0;
     return HEAL_OK;
@@ -696,6 +698,27 @@ int get_ws(size_t bytes, cudaStream_t stream, void **out)
     return HEAL_OK;
 }
 
+// Scaled-lo variant (HEAL_LO_SCALED; the paper's h = h_hi + h_lo / 2^10 and Eq. 10 as printed):
+// C = 2^-p (hi.W) + 2^-(p+10) (lo'.W), formed the way the paper forms it -- two FP16 tensor-core GEMMs summed into one
+// FP32 output: the lo' GEMM stores its exactly scaled sum, the hi GEMM adds its own on top (FP32 RN).
+// Each GEMM has the usual fixed reduction order, so the result is as reproducible as the one-accumulator form.
+int scaled_two_gemms(int64_t M, int64_t N, int64_t K, const void *A_hi, const void *A_lo, int64_t lda, const void *B,
+                     int64_t ldb, const OutArgs &out, int scale_exp, bool b_nk, bool b_static, cudaStream_t stream)
+{
+    if (!out.C) return HEAL_ERR_NULL_POINTER;                         // the FP32 matrix carries the first GEMM
+    if (scale_exp + HEAL_LO_SHIFT > 126) return HEAL_ERR_INVALID_VALUE;
+    OutArgs first = out;
+    first.hi = first.lo = nullptr;
+    const uint32_t bits = static_cast<uint32_t>(127 - scale_exp - HEAL_LO_SHIFT) << 23;
+    memcpy(&first.scale, &bits, 4);
+    first.accumulate = 0;
+    int st = presplit_impl(M, N, K, A_lo, nullptr, lda, B, nullptr, ldb, first, 1, b_nk, b_static, stream);
+    if (st) return st;
+    OutArgs second = out;
+    second.accumulate = 1;
+    return presplit_impl(M, N, K, A_hi, nullptr, lda, B, nullptr, ldb, second, 1, b_nk, b_static, stream);
+}
+
 }  // namespace
 
 // =============================================== C ABI ===========================================
@@ -758,6 +781,13 @@ int heal_set_workspace(void *ptr, size_t bytes)
 
 int heal_split(int64_t rows, int64_t cols, const void *X, int64_t ldx, void *hi, void *lo, int64_t ld, void *stream)
 {
+    return heal_split_scaled(rows, cols, X, ldx, hi, lo, ld, 0, stream);
+}
+
+int heal_split_scaled(int64_t rows, int64_t cols, const void *X, int64_t ldx, void *hi, void *lo, int64_t ld,
+                      int32_t lo_shift, void *stream)
+{
+    if (lo_shift < 0 || lo_shift > 16) return HEAL_ERR_INVALID_VALUE;
     if (rows < 0 || cols < 0 || ldx < cols || ld < cols) return HEAL_ERR_INVALID_VALUE;
     if (rows == 0 || cols == 0) return HEAL_OK;
     if (!X || !hi || !lo) return HEAL_ERR_NULL_POINTER;
@@ -765,7 +795,7 @@ int heal_split(int64_t rows, int64_t cols, const void *X, int64_t ldx, void *hi,
     int st = ensure_init();
     if (st) return st;
     return launch_split(rows, cols, static_cast<const float *>(X), ldx, static_cast<__half *>(hi),
-                        static_cast<__half *>(lo), ld, static_cast<cudaStream_t>(stream));
+                        static_cast<__half *>(lo), ld, static_cast<cudaStream_t>(stream), lo_shift);
 }
 
 // Output validation shared by the _ex entry points: builds the OutArgs of step E.
@@ -790,6 +820,7 @@ static int make_out(int64_t M, int64_t N, void *C, int64_t ldc, void *C_hi, void
     float sc;
     memcpy(&sc, &bits, 4);
     out->scale = sc;
+    out->accumulate = 0;
     return HEAL_OK;
 }
 
@@ -817,6 +848,9 @@ int heal_gemm_presplit_ex(int64_t M, int64_t N, int64_t K, const void *A_hi, con
     }
     st = ensure_init();
     if (st) return st;
+    if ((mode & HEAL_LO_SCALED) && K > 0)          // A_lo holds r16((x - hi) * 2^10), e.g. from heal_split_scaled(.., 10, ..)
+        return scaled_two_gemms(M, N, K, A_hi, A_lo, lda, B_hi, ldb, out, scale_exp, b_nk, (mode & HEAL_B_STATIC) != 0,
+                                static_cast<cudaStream_t>(stream));
     return presplit_impl(M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, out, nprod, b_nk, (mode & HEAL_B_STATIC) != 0,
                          static_cast<cudaStream_t>(stream));
 }
@@ -853,7 +887,8 @@ int heal_gemm_ex(int64_t M, int64_t N, int64_t K, const void *A, int64_t lda, co
     const bool b_static = (mode & HEAL_B_STATIC) != 0;
     if (K == 0) return presplit_impl(M, N, K, nullptr, nullptr, lda, nullptr, nullptr, ldb, out, nprod, b_nk, b_static, stream);
     static const bool no_fused = std::getenv("HEAL_NO_FUSED") != nullptr;          // debug only
-    if (M <= 16 && !b_f32 && !no_fused && forced_kernel() != 1) {
+    const bool lo_scaled = (mode & HEAL_LO_SCALED) != 0;
+    if (M <= 16 && !b_f32 && !no_fused && !lo_scaled && forced_kernel() != 1) {
         // decode shapes (M <= 16) with FP16 weights: step S runs inside the GEMM kernel (no planes, one launch);
         // above that the in-kernel conversion costs more than the split launch it saves (measured)
         bool handled = false;
@@ -871,8 +906,9 @@ int heal_gemm_ex(int64_t M, int64_t N, int64_t K, const void *A, int64_t lda, co
     __half *a_hi = reinterpret_cast<__half *>(w);
     __half *a_lo = reinterpret_cast<__half *>(w + p.a_plane);
     // step S on the activations; in 1P only the hi plane is consumed
-    st = launch_split(M, K, static_cast<const float *>(A), lda, a_hi, a_lo, p.lda_p, stream);
+    st = launch_split(M, K, static_cast<const float *>(A), lda, a_hi, a_lo, p.lda_p, stream, lo_scaled ? HEAL_LO_SHIFT : 0);
     if (st) return st;
+    if (lo_scaled) return scaled_two_gemms(M, N, K, a_hi, a_lo, p.lda_p, B, ldb, out, scale_exp, b_nk, b_static, stream);
     const void *b_hi = B, *b_lo = nullptr;
     int64_t ldb_eff = ldb;
     if (b_f32) {

@@ -19,6 +19,8 @@ struct OutArgs {
     __half *hi, *lo;      // FP16 M x N planes, pitch ld16 (elements, % 8 == 0); null = not requested
     int64_t ld16;
     float scale;          // 2^-p, exactly representable; 1.0f = none
+    int accumulate;       // C += scaled result (needs C): second launch of the scaled-lo variant, which forms
+                          // C = 2^-10 (lo'.W) + hi.W as the paper's two GEMMs summed into one FP32 output
 };
 
 // The output mode is uniform for the launch: pick it ONCE per store loop (a per-element test costs a dependent
@@ -33,7 +35,7 @@ struct EmitTag {
 __device__ __forceinline__ OutArgs pin_out(const OutArgs &o)
 {
     OutArgs r = o;
-    asm volatile("" : "+l"(r.C), "+l"(r.ldc), "+l"(r.hi), "+l"(r.lo), "+l"(r.ld16), "+f"(r.scale));
+    asm volatile("" : "+l"(r.C), "+l"(r.ldc), "+l"(r.hi), "+l"(r.lo), "+l"(r.ld16), "+f"(r.scale), "+r"(r.accumulate));
     return r;
 }
 template <class F>
@@ -53,6 +55,16 @@ __device__ __forceinline__ void emit4(const OutArgs &o, int64_t row, int col, fl
     const bool full = col + 3 < N;
     if (HAS_C) {
         float *c = o.C + row * o.ldc + col;
+        if (o.accumulate) {
+            if (full) {
+                const float4 old = *reinterpret_cast<const float4 *>(c);
+                v.x = __fadd_rn(old.x, v.x); v.y = __fadd_rn(old.y, v.y); v.z = __fadd_rn(old.z, v.z); v.w = __fadd_rn(old.w, v.w);
+            } else {
+                if (col < N) v.x = __fadd_rn(c[0], v.x);
+                if (col + 1 < N) v.y = __fadd_rn(c[1], v.y);
+                if (col + 2 < N) v.z = __fadd_rn(c[2], v.z);
+            }
+        }
         if (full) {
             *reinterpret_cast<float4 *>(c) = v;
         } else {
@@ -89,7 +101,10 @@ template <bool HAS_C, bool HAS_P>
 __device__ __forceinline__ void emit1(const OutArgs &o, int64_t row, int col, float v)
 {
     v *= o.scale;
-    if (HAS_C) o.C[row * o.ldc + col] = v;
+    if (HAS_C) {
+        if (o.accumulate) v = __fadd_rn(o.C[row * o.ldc + col], v);
+        o.C[row * o.ldc + col] = v;
+    }
     if (HAS_P) {
         const __half h = __float2half_rn(v);
         o.hi[row * o.ld16 + col] = h;

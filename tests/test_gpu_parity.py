@@ -475,6 +475,70 @@ def test_small_m_single_cta_panels_tmem_ring(hb, inputs, M, N, K, nprod, b_nk):
         hb.debug_force_kernel(0)
 
 
+def test_scaled_split_bit_exact(hb, oracle, inputs):
+    """heal_split_scaled(lo_shift = 10): lo = r16((x - hi) * 2^10), the paper's h = h_hi + h_lo / 2^10,
+    bit for bit against the oracle's integer split, including magnitudes where the unscaled residual underflows."""
+    X = inputs.activations(130, 1000, seed=21, outliers=True)
+    X[:40] *= 2.0 ** -12
+    X[40:60] *= 2.0 ** -20
+    X[0, :6] = [0.0, -0.0, 65504.0, 2.0 ** -24, 1 + 2.0 ** -11, -3e-6]
+    for s_ in (10, 11, 0):
+        hi, lo = hb.heal_split(dev(X), lo_shift=s_)
+        torch.cuda.synchronize()
+        ohi, olo = oracle.split(X, s=s_)
+        assert np.array_equal(hi.cpu().numpy().view(np.uint16), ohi)
+        assert np.array_equal(lo.cpu().numpy().view(np.uint16), olo)
+
+
+@pytest.mark.parametrize("M,N,K", [(8, 520, 4096), (300, 1032, 4096), (64, 264, 14336)])
+def test_lo_scaled_variant(hb, oracle, inputs, M, N, K):
+    """HEAL_LO_SCALED (Eq. 10 as printed, s = 10; two GEMMs summed into one FP32 output): against the oracle's exact
+    evaluation of the same products, inside the gate, bit-identical across M and kernel families -- and, on
+    activations small enough for the unscaled residual to underflow FP16, far closer to FP64 than the s = 0 default."""
+    A = inputs.activations(M, K, seed=22, outliers=True)
+    W = inputs.weights_f16(K, N, seed=22)
+    Ad, Wd = dev(A), dev(W)
+    mode = 2 | hb.LO_SCALED
+    got = hb.heal_gemm(Ad, Wd, mode)
+    o3 = oracle.gemm_split(A, W, 2, s=10)
+    assert np.all(np.abs(got.cpu().numpy() - o3) <= 2 * elementwise_bound(A, W, K, 2) + 1e-30)
+    assert oracle.normwise_error(got.cpu().numpy(), oracle.gemm_f64(A, W), A, W) <= GATE
+    assert torch.equal(hb.heal_gemm(Ad[:5], Wd, mode), got[:5])                  # M-invariant
+    try:
+        hb.debug_force_kernel(1)
+        assert torch.equal(hb.heal_gemm(Ad, Wd, mode), got)
+    finally:
+        hb.debug_force_kernel(0)
+    ah, al = hb.heal_split(Ad, lo_shift=hb.LO_SHIFT)
+    assert torch.equal(hb.heal_gemm_presplit(ah, al, Wd, None, mode), got)
+    C, hi, lo = hb.heal_gemm_ex(Ad, Wd, mode, scale_exp=2)                        # composes with the extended epilogue
+    assert torch.equal(C, got * 0.25)
+    whi, wlo = hb.heal_split(C)
+    assert torch.equal(hi.view(torch.int16), whi.view(torch.int16)) and torch.equal(lo.view(torch.int16), wlo.view(torch.int16))
+    # tiny activations: |x| ~ 2^-12, the s = 0 residual is an FP16 subnormal with almost no bits left
+    At = (A * np.float32(2.0 ** -12)).astype(np.float32)
+    ref = oracle.gemm_f64(At, W)
+    e0 = oracle.normwise_error(hb.heal_gemm(dev(At), Wd, 2).cpu().numpy(), ref, At, W)
+    e10 = oracle.normwise_error(hb.heal_gemm(dev(At), Wd, mode).cpu().numpy(), ref, At, W)
+    assert e10 <= GATE and e10 * 16 < e0, (e0, e10)
+
+
+def test_lo_scaled_errors(hb):
+    A = torch.zeros((8, 64), device="cuda")
+    W = torch.zeros((64, 16), dtype=torch.float16, device="cuda")
+    W32 = torch.zeros((64, 16), device="cuda")
+    C = torch.zeros((8, 16), device="cuda")
+    hi = torch.zeros((8, 16), dtype=torch.float16, device="cuda")
+    L = hb.lib()
+    raw = hb.heal_gemm_raw
+    assert raw(8, 16, 64, A.data_ptr(), 64, W32.data_ptr(), 16, C.data_ptr(), 16, 3 | hb.LO_SCALED) == 4      # 2P only
+    assert raw(8, 16, 64, A.data_ptr(), 64, W.data_ptr(), 16, C.data_ptr(), 16, 1 | hb.LO_SCALED) == 4
+    assert L.heal_gemm_ex(8, 16, 64, A.data_ptr(), 64, W.data_ptr(), 16, None, 0, hi.data_ptr(), hi.data_ptr(), 16, 0,
+                          2 | hb.LO_SCALED, None) == 2                                                           # needs C
+    assert L.heal_split_scaled(8, 64, A.data_ptr(), 64, hi.data_ptr(), hi.data_ptr(), 64, 17, None) == 1
+    torch.cuda.synchronize()
+
+
 def test_static_weights_graph_chain(hb, inputs):
     """HEAL_B_STATIC in a captured chain of decode GEMMs (each kernel streams its weights while its predecessor
     finishes; activations and C wait): every replay reproduces the eager results bit for bit, including a chain
