@@ -37,7 +37,8 @@ def test_host_side_validation_without_device(lib):
     assert raw(0, 4, 8, None, 8, None, 8, None, 4, 2) == 0           # empty: no-op
     assert raw(4, 4, 8, None, 8, None, 8, None, 4, 2) == 2           # null pointer
     assert raw(4, 4, 8, 16, 8, 16, 8, 16, 4, 9) == 4                 # unknown product count
-    assert raw(4, 4, 8, 16, 8, 16, 8, 16, 4, 0x42) == 4              # unknown flag bit (0x10 = B_NK, 0x20 = B_STATIC)
+    assert raw(4, 4, 8, 16, 8, 16, 8, 16, 4, 0x82) == 4              # unknown flag bit (0x10 B_NK, 0x20 B_STATIC, 0x40 LO_SCALED)
+    assert raw(4, 4, 8, 16, 8, 16, 8, 16, 4, 0x43) == 4              # LO_SCALED is two-product only
     assert raw(4, 4, 8, 20, 8, 16, 8, 16, 4, 2) == 3                 # misaligned A
     assert "MISALIGNED" in hb.status_string(3) and hb.status_string(0) == "HEAL_OK"
     # workspace = two FP16 planes of A (256-byte rounded); plus two planes of B in 3P
