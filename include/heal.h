@@ -11,8 +11,8 @@
  *                                                               PAPER.md:195; lo.lo dropped)
  *      1 product :  C = h_hi.W                                  the "skipped layer" / HEAL-Base GEMM
  *
- * This build uses s = 0 (BASELINE.json north_star: lo = r16(x - hi), all products into one
- * accumulator); reading A1 discusses the paper's s = 10.
+ * The default is s = 0 (BASELINE.json north_star: lo = r16(x - hi), all products into one
+ * accumulator); the paper's s = 10 is the HEAL_LO_SCALED variant below (reading A1).
  *
  * Reduction order (fixed; a function of K and mode only, never of M, N, tile shape or launch):
  *   K is cut into segments of HEAL_K_SEGMENT = 512 consecutive k.  Within a segment the tensor core

@@ -71,7 +71,7 @@ def _time(fns, graph: bool, reps: int = 7):
     return ts[0], ts[len(ts) // 2]
 
 
-def bench_shape(name, M, N, K, nprod, dist, rows):
+def bench_shape(name, M, N, K, nprod, dist, rows, flags=0):
     gen = torch.Generator(device="cuda")
     gen.manual_seed(1234)
     w_bytes = K * N * (4 if nprod >= 3 else 2)
@@ -88,11 +88,11 @@ def bench_shape(name, M, N, K, nprod, dist, rows):
     C = torch.empty(M, N, device="cuda")
     ws = torch.empty(max(256, hb.workspace_size(M, N, K, nprod)), dtype=torch.uint8, device="cuda")
     hb.set_workspace(ws)
-    full = [(lambda b=b: hb.heal_gemm(A, b, nprod, C)) for b in Bs]
-    full_st = [(lambda b=b: hb.heal_gemm(A, b, nprod | hb.B_STATIC, C)) for b in Bs]
-    ah, al = hb.heal_split(A)
+    full = [(lambda b=b: hb.heal_gemm(A, b, nprod | flags, C)) for b in Bs]
+    full_st = [(lambda b=b: hb.heal_gemm(A, b, nprod | flags | hb.B_STATIC, C)) for b in Bs]
+    ah, al = hb.heal_split(A, lo_shift=hb.LO_SHIFT if flags & hb.LO_SCALED else 0)
     planes = [(hb.heal_split(b) if nprod >= 3 else (b, None)) for b in Bs]
-    pres = [(lambda p=p: hb.heal_gemm_presplit(ah, al, p[0], p[1], nprod, C)) for p in planes]
+    pres = [(lambda p=p: hb.heal_gemm_presplit(ah, al, p[0], p[1], nprod | flags, C)) for p in planes]
     reps = (2 if small else 1)
     t_full = _time(full * reps, small)
     t_pre = _time(pres * reps, small)
@@ -138,6 +138,9 @@ def main():
     cfgs += [(f"mid M={m}", m, 4096, 4096, 2, "normal") for m in (128, 256, 512, 1024)]
     for c in cfgs:
         bench_shape(*c, rows)
+    # the paper-faithful scaled residual (HEAL_LO_SCALED, s = 10): two one-product GEMMs summed into one FP32 output
+    bench_shape("cfg2 up/gate, s=10 variant", 2048, 14336, 4096, 2, "normal", rows, flags=hb.LO_SCALED)
+    bench_shape("cfg1 decode M=8, s=10 variant", 8, 4096, 4096, 2, "normal", rows, flags=hb.LO_SCALED)
     name = torch.cuda.get_device_name(0)
     print(f"# HEAL compensated GEMM on {name}: all BASELINE.json configs\n")
     print(f"Peaks ({src}): cuBLAS BF16 {burst:.0f} TFLOP/s burst / {sust:.0f} sustained; HBM copy {hbm:.0f} GB/s; nominal 2250 TFLOP/s, ~8 TB/s.\n")
