@@ -46,7 +46,8 @@ typedef enum {
     HEAL_ERR_UNSUPPORTED_MODE = 4,   /* unknown mode bits, or B dtype/mode mismatch                */
     HEAL_ERR_CUDA = 5,               /* a CUDA call failed; see heal_last_cuda_error()             */
     HEAL_ERR_WORKSPACE = 6,          /* caller-supplied workspace too small                        */
-    HEAL_ERR_UNSUPPORTED_DEVICE = 7  /* current device is not sm_100                               */
+    HEAL_ERR_UNSUPPORTED_DEVICE = 7  /* current device is not sm_100, or differs from the device of the
+                                        process's first call (one device per process)              */
 } heal_status;
 
 #define HEAL_K_SEGMENT 512

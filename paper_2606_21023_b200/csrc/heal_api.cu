@@ -71,7 +71,13 @@ inline int cuda_fail(cudaError_t e)
 int ensure_init()
 {
     std::lock_guard<std::mutex> lk(g_mu);
-    if (g.init) return g.init_status;
+    if (g.init) {
+        // one device per process (the launch pattern of bench.py / torchrun): buffers, SM count and tensor-map entry
+        // point belong to the device of the first call
+        int cur = -1;
+        if (g.init_status == HEAL_OK && (cudaGetDevice(&cur) != cudaSuccess || cur != g.device)) return HEAL_ERR_UNSUPPORTED_DEVICE;
+        return g.init_status;
+    }
     g.init = true;
     auto fail = [&](int st) { g.init_status = st; return st; };
     int dev = 0;
@@ -757,7 +763,8 @@ const char *heal_status_string(int status)
     case HEAL_ERR_UNSUPPORTED_MODE: return "HEAL_ERR_UNSUPPORTED_MODE: unknown mode bits";
     case HEAL_ERR_CUDA: return "HEAL_ERR_CUDA: a CUDA call failed (see heal_last_cuda_error)";
     case HEAL_ERR_WORKSPACE: return "HEAL_ERR_WORKSPACE: supplied workspace too small";
-    case HEAL_ERR_UNSUPPORTED_DEVICE: return "HEAL_ERR_UNSUPPORTED_DEVICE: current device is not sm_100";
+    case HEAL_ERR_UNSUPPORTED_DEVICE:
+        return "HEAL_ERR_UNSUPPORTED_DEVICE: current device is not sm_100, or not the device of this process's first call";
     }
     return "unknown heal_status";
 }

@@ -226,7 +226,7 @@ heal_gemm_smallm_kernel(const __grid_constant__ CUtensorMap tm_x_hi, const __gri
             __syncwarp();
             mbar_wait(done_bar, 0, args.diag, 701);
             cluster_wait();
-            cluster_arrive();
+            cluster_arrive_relaxed();          // "my pipeline is dead": observed through done_bar, no data to publish
         }
     } else if (warp == 1) {
         // ================================ MMA issuer ==================================
@@ -285,7 +285,7 @@ heal_gemm_smallm_kernel(const __grid_constant__ CUtensorMap tm_x_hi, const __gri
             __syncwarp();
             mbar_wait(done_bar, 0, args.diag, 702);
             cluster_wait();
-            cluster_arrive();
+            cluster_arrive_relaxed();          // "my pipeline is dead": observed through done_bar, no data to publish
         }
     } else {
         const int et = threadIdx.x - 64;                   // 0..127 among the converter / epilogue threads
@@ -435,7 +435,7 @@ heal_gemm_smallm_kernel(const __grid_constant__ CUtensorMap tm_x_hi, const __gri
         } else {
             cluster_wait();                                // every rank's red_bar is initialised
             if (args.red_alias) {                          // ... and every rank's pipeline buffers are dead
-                cluster_arrive();
+                cluster_arrive_relaxed();
                 cluster_wait();
             }
             // push this rank's partials: token m -> rank m / rpr, float (seg * 128 + nl) * rpr + m % rpr of its

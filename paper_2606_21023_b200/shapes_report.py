@@ -120,6 +120,23 @@ def bench_shape(name, M, N, K, nprod, dist, rows, flags=0):
     torch.cuda.empty_cache()
 
 
+def products_sweep():
+    M, N, K = 2048, 14336, 4096
+    gen = torch.Generator(device="cuda")
+    gen.manual_seed(99)
+    A = torch.randn(M, K, device="cuda", generator=gen)
+    B = torch.randn(K, N, device="cuda", generator=gen) * 0.02
+    ah, al = hb.heal_split(A)
+    bh, bl = hb.heal_split(B)
+    C = torch.empty(M, N, device="cuda")
+    out = []
+    steps = (N // 256) * (M // 256) * (K // 64) / 74.0            # k-tile steps per CTA pair
+    for nprod, kb in ((1, 32), (2, 48), (3, 64), (4, 64)):
+        t = _time([lambda: hb.heal_gemm_presplit(ah, al, bh, bl, nprod, C)], False)
+        out.append(f"| {nprod}P | {t[1]:.1f} | {nprod * 2.0 * M * N * K / t[1] / 1e6:.0f} | {kb} | {kb * 1024 * steps / t[1] / 1e3:.0f} |")
+    return out
+
+
 def main():
     burst, sust, hbm, src = _peaks()
     rows = []
@@ -141,6 +158,7 @@ def main():
     # the paper-faithful scaled residual (HEAL_LO_SCALED, s = 10): two one-product GEMMs summed into one FP32 output
     bench_shape("cfg2 up/gate, s=10 variant", 2048, 14336, 4096, 2, "normal", rows, flags=hb.LO_SCALED)
     bench_shape("cfg1 decode M=8, s=10 variant", 8, 4096, 4096, 2, "normal", rows, flags=hb.LO_SCALED)
+    sweep = products_sweep()
     name = torch.cuda.get_device_name(0)
     print(f"# HEAL compensated GEMM on {name}: all BASELINE.json configs\n")
     print(f"Peaks ({src}): cuBLAS BF16 {burst:.0f} TFLOP/s burst / {sust:.0f} sustained; HBM copy {hbm:.0f} GB/s; nominal 2250 TFLOP/s, ~8 TB/s.\n")
@@ -152,6 +170,13 @@ def main():
     print("| config | MxNxK | mode | full us | full + HEAL_B_STATIC us (M <= 64) | G+E us | eff TFLOP/s | tensor TFLOP/s (% burst / % nominal) | GB/s (% peak) | cuBLAS SGEMM us | cuBLAS FP16 us | cuBLAS BF16 us | timing |")
     print("|---|---|---|---|---|---|---|---|---|---|---|---|---|")
     print("\n".join(rows))
+    print("\n## What bounds the pair kernel: tensor work per loaded byte (2048x14336x4096, pre-split planes, burst)\n")
+    print("The same kernel with 1 / 2 / 3 / 4 products per loaded k-tile (32 / 48 / 64 / 64 KB per CTA and k-tile): the tensor rate rises "
+          "with the products per byte until the fourth product makes the tensor pipe the limit, i.e. operand delivery (L2 -> SM), "
+          "not the tensor pipe, bounds the 2P kernel (DESIGN.md 7).\n")
+    print("| products | us | tensor TFLOP/s | KB per CTA and k-tile | delivery per SM GB/s |")
+    print("|---|---|---|---|---|")
+    print("\n".join(sweep))
 
 
 if __name__ == "__main__":

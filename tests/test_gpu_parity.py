@@ -539,6 +539,31 @@ def test_lo_scaled_errors(hb):
     torch.cuda.synchronize()
 
 
+def test_ordered_split_k_two_streams(hb, inputs):
+    """Ordered split-K on two streams at once (each stream has its own partial-sum area and counters), interleaved with a
+    different split-K shape on the same stream (the area is re-used and re-grown)."""
+    A1 = dev(inputs.activations(128, 4096, seed=23, outliers=True))
+    W1 = dev(inputs.weights_f16(4096, 1032, seed=23))
+    A2 = dev(inputs.activations(256, 2048, seed=24))
+    W2 = dev(inputs.weights_f16(2048, 520, seed=24))
+    r1 = hb.heal_gemm(A1, W1, 2).clone()
+    r2 = hb.heal_gemm(A2, W2, 2).clone()
+    s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+    outs = []
+    torch.cuda.synchronize()
+    for _ in range(4):
+        with torch.cuda.stream(s1):
+            a = hb.heal_gemm(A1, W1, 2)
+            b = hb.heal_gemm(A2, W2, 2)
+        with torch.cuda.stream(s2):
+            c = hb.heal_gemm(A2, W2, 2)
+            d = hb.heal_gemm(A1, W1, 2)
+        outs.append((a, b, c, d))
+    torch.cuda.synchronize()
+    for a, b, c, d in outs:
+        assert torch.equal(a, r1) and torch.equal(d, r1) and torch.equal(b, r2) and torch.equal(c, r2)
+
+
 def test_static_weights_graph_chain(hb, inputs):
     """HEAL_B_STATIC in a captured chain of decode GEMMs (each kernel streams its weights while its predecessor
     finishes; activations and C wait): every replay reproduces the eager results bit for bit, including a chain
