@@ -544,6 +544,13 @@ int launch_small_cfg(int64_t M, int64_t N, int64_t K, const SmallIn &in, const v
     args.rows_per_rank = rpr;
     args.red_bytes = static_cast<int>(red);
     args.red_alias = red_alias ? 1 : 0;
+    {
+        // pushes per thread: few -> st.async (lowest latency), many -> plain remote stores + one fence/arrive per warp
+        const int vw = (rpr & 3) == 0 ? 4 : ((rpr & 1) == 0 ? 2 : 1);
+        const int64_t pushes = cs > 1 ? static_cast<int64_t>(max_local) * ((M + vw - 1) / vw) : 0;
+        static const bool no_async = std::getenv("HEAL_NO_ASYNC_PUSH") != nullptr;        // debug only
+        args.red_async = (cs > 1 && pushes <= 8 && !no_async) ? 1 : 0;
+    }
     args.ring = ring;
     static const bool no_static = std::getenv("HEAL_NO_STATIC") != nullptr;       // debug only
     args.b_static = (in.b_static && !no_static) ? 1 : 0;

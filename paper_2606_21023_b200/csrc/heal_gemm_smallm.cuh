@@ -10,10 +10,11 @@
 //
 // Cluster of CS CTAs = one 128-column panel; CTA rank r owns segments r, r+CS, r+2CS, ... (local slot
 // j = s / CS lives in TMEM columns j*MPAD..).  Token rows are dealt to the ranks in contiguous blocks: every rank
-// PUSHES its segment partials of that row straight from its TMEM registers into the owner's shared
-// memory (st.shared::cluster) and then arrives (release.cluster) on the owner's mbarrier; the owner adds
-// the n_seg partials in ascending segment order and stores C.  No atomics, no cluster-wide barrier
-// after the main loop.
+// PUSHES its segment partials of those rows straight from its TMEM registers into the owner's shared
+// memory -- with st.async when a thread has few values to send (the bytes are counted on the owner's
+// mbarrier: no fence, no arrive), else with plain st.shared::cluster plus one fence and one relaxed
+// remote arrive per warp; the owner adds the n_seg partials in ascending segment order and stores C.
+// No atomics, no cluster-wide barrier after the main loop.
 //
 // FUSED variant (heal_gemm, B already FP16): step S runs inside the kernel -- the four epilogue warps
 // convert the FP32 activations of each k-tile to hi/lo FP16 (same arithmetic as
@@ -67,6 +68,8 @@ struct SmallArgs {
     int stages;           // pipeline depth (2..8)
     int rows_per_rank;    // ceil(M / CS): token rows finished by one rank (CS > 1)
     int red_bytes;        // CS > 1: n_seg * rows_per_rank * 128 floats of partial sums pushed by the cluster
+    int red_async;        // few pushes per thread: st.async (completion counted in bytes on the owner's mbarrier, no fence,
+                          // no arrive); many: plain remote stores + one fence and arrive per warp (higher throughput)
     int red_alias;        // the pushed partial sums reuse the pipeline stages (large M * K): needs a second cluster
                           // barrier ("every rank's main loop is over") before anybody pushes
     int ring;             // CS == 1, planes: number of TMEM slots the segments cycle through (0 = every local
@@ -135,12 +138,21 @@ heal_gemm_smallm_kernel(const __grid_constant__ CUtensorMap tm_x_hi, const __gri
             mbar_init(xfull_bar(s), 4);                  // one arrival per converter warp
         }
         mbar_init(done_bar, 1);
-        mbar_init(red_bar, cs * 4);                      // one arrival per epilogue warp of every rank
+        mbar_init(red_bar, args.red_async ? 1 : cs * 4); // async: completes when every pushed byte has landed;
+                                                         // else one arrival per epilogue warp of every rank
         for (int j = 0; j < ring; ++j) {
             mbar_init(tfull_bar(j), 1);
             mbar_init(tempty_bar(j), 4);
         }
         fence_mbar_init();
+        if (cs > 1 && args.red_async && static_cast<int>(rank) < owners) {
+            // this rank finishes rows [rank * rpr, ...): every rank pushes, per segment and column, one vector per started
+            // group of VW owned rows (VW = 4 / 2 / 1 by the divisibility of rpr)
+            const int rpr = args.rows_per_rank;
+            const int rows = min(rpr, args.M - static_cast<int>(rank) * rpr);
+            const int vw = (rpr & 3) == 0 ? 4 : ((rpr & 1) == 0 ? 2 : 1);
+            mbar_arrive_expect_tx(red_bar, static_cast<uint32_t>(args.n_seg) * kSmallBNW * static_cast<uint32_t>((rows + vw - 1) / vw * vw) * 4u);
+        }
     }
     if (warp == 1) {
         tmem_alloc(tmem_slot, static_cast<uint32_t>(args.tmem_cols));
@@ -450,13 +462,25 @@ heal_gemm_smallm_kernel(const __grid_constant__ CUtensorMap tm_x_hi, const __gri
                         uint32_t v[16];
                         tmem_ld_32x32b_x16(tmem_base + (static_cast<uint32_t>(quad * 32) << 16) + static_cast<uint32_t>(j * MPAD + c * 16), v);
                         tmem_ld_wait();
+                        const bool async = args.red_async != 0;
                         if ((rpr & 3) == 0) {
 #pragma unroll
                             for (int i = 0; i < 16; i += 4) {
                                 const int m = c * 16 + i;
                                 if (m < args.M) {         // m % 4 == 0 and rpr % 4 == 0: rows m..m+3 have one owner (rows >= M: unused zeros)
                                     const uint32_t dst = static_cast<uint32_t>(m / rpr), ml = static_cast<uint32_t>(m % rpr);
-                                    st_dsmem_v4(map_to_cta(red_base + row_off + ml * 4u, dst), v[i], v[i + 1], v[i + 2], v[i + 3]);
+                                    const uint32_t a = map_to_cta(red_base + row_off + ml * 4u, dst);
+                                    if (async) st_async_v4(a, v[i], v[i + 1], v[i + 2], v[i + 3], map_to_cta(red_bar, dst));
+                                    else       st_dsmem_v4(a, v[i], v[i + 1], v[i + 2], v[i + 3]);
+                                }
+                            }
+                        } else if ((rpr & 1) == 0 && async) {
+#pragma unroll
+                            for (int i = 0; i < 16; i += 2) {
+                                const int m = c * 16 + i;
+                                if (m < args.M) {
+                                    const uint32_t dst = static_cast<uint32_t>(m / rpr), ml = static_cast<uint32_t>(m % rpr);
+                                    st_async_v2(map_to_cta(red_base + row_off + ml * 4u, dst), v[i], v[i + 1], map_to_cta(red_bar, dst));
                                 }
                             }
                         } else {
@@ -465,7 +489,9 @@ heal_gemm_smallm_kernel(const __grid_constant__ CUtensorMap tm_x_hi, const __gri
                                 const int m = c * 16 + i;
                                 if (m < args.M) {
                                     const uint32_t dst = static_cast<uint32_t>(m / rpr), ml = static_cast<uint32_t>(m % rpr);
-                                    st_dsmem_b32(map_to_cta(red_base + row_off + ml * 4u, dst), v[i]);
+                                    const uint32_t a = map_to_cta(red_base + row_off + ml * 4u, dst);
+                                    if (async) st_async_b32(a, v[i], map_to_cta(red_bar, dst));
+                                    else       st_dsmem_b32(a, v[i]);
                                 }
                             }
                         }
@@ -473,16 +499,20 @@ heal_gemm_smallm_kernel(const __grid_constant__ CUtensorMap tm_x_hi, const __gri
                 }
             }
             tc_fence_before();
-            __syncwarp();
-            // one fence per signalling lane (cumulative over the warp's pushes, ordered by the __syncwarp) and a
-            // relaxed remote arrive: a cluster-scope release costs ~0.5 us each on this part (measured), so pay it once
-            if (lane < owners) {
-                fence_acq_rel_cluster();
-                mbar_arrive_relaxed_cluster(map_to_cta(red_bar, static_cast<uint32_t>(lane)));
+            if (!args.red_async) {
+                __syncwarp();
+                // one fence per signalling lane (cumulative over the warp's pushes, ordered by the __syncwarp) and a
+                // relaxed remote arrive: a cluster-scope release costs ~0.5 us each on this part (measured), so pay it once
+                if (lane < owners) {
+                    fence_acq_rel_cluster();
+                    mbar_arrive_relaxed_cluster(map_to_cta(red_bar, static_cast<uint32_t>(lane)));
+                }
             }
+            tc_fence_before();
             if (et == 0) HEAL_STAMP(args.trace, 7);
             if (static_cast<int>(rank) < owners) {
-                mbar_wait_cluster(red_bar, 0, args.diag, 710);
+                if (args.red_async) mbar_wait(red_bar, 0, args.diag, 710);       // every byte has landed
+                else                mbar_wait_cluster(red_bar, 0, args.diag, 710);
                 if (et == 0) HEAL_STAMP(args.trace, 8);
                 // this rank finishes rows [rank * rpr, min(M, (rank + 1) * rpr)): ascending segment order, FP32 RN
                 const float *red = reinterpret_cast<const float *>(smem_raw + (red_base - smem_u32(smem_raw)));
