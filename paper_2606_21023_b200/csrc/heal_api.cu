@@ -285,11 +285,11 @@ template <class Cfg>
 int launch_gemm_cfg(int64_t M, int64_t N, int64_t K, const void *A_hi, const void *A_lo, int64_t lda, const void *B_hi,
                     const void *B_lo, int64_t ldb, const OutArgs &out, cudaStream_t stream)
 {
-    static bool attr_set = false;
+    static std::atomic<bool> attr_set{false};          // setting the attribute twice from two threads is harmless
     auto kern = heal_gemm_umma_kernel<Cfg>;
-    if (!attr_set) {
+    if (!attr_set.load(std::memory_order_acquire)) {
         HEAL_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::SMEM_BYTES));
-        attr_set = true;
+        attr_set.store(true, std::memory_order_release);
     }
     CUtensorMap ta_hi, ta_lo, tb_hi, tb_lo;
     int st = encode_f16_2d(&ta_hi, A_hi, K, M, lda, kBK, kBM);
@@ -338,11 +338,11 @@ template <class Cfg>
 int launch_gemm2_cfg(int64_t M, int64_t N, int64_t K, const void *A_hi, const void *A_lo, int64_t lda, const void *B_hi,
                      const void *B_lo, int64_t ldb, const OutArgs &out, cudaStream_t stream)
 {
-    static bool attr_set = false;
+    static std::atomic<bool> attr_set{false};
     auto kern = heal_gemm_umma2_kernel<Cfg>;
-    if (!attr_set) {
+    if (!attr_set.load(std::memory_order_acquire)) {
         HEAL_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::SMEM_BYTES));
-        attr_set = true;
+        attr_set.store(true, std::memory_order_release);
     }
     CUtensorMap ta_hi, ta_lo, tb_hi, tb_lo;
     int st = encode_f16_2d(&ta_hi, A_hi, K, M, lda, kBK, kBM);
@@ -501,10 +501,10 @@ int launch_small_cfg(int64_t M, int64_t N, int64_t K, const SmallIn &in, const v
     // more than half of TMEM: make sure only one CTA fits per SM (two could not both allocate)
     if (tmem_cols > 256 && smem < static_cast<size_t>(kSmemLimit) / 2 + 2048) smem = static_cast<size_t>(kSmemLimit) / 2 + 2048;
     auto kern = heal_gemm_smallm_kernel<Cfg>;
-    static size_t attr_smem = 0;
-    if (smem > attr_smem) {
-        HEAL_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem)));
-        attr_smem = smem;
+    static std::atomic<size_t> attr_smem{0};           // only ever raised: a concurrent smaller request cannot lower it
+    if (smem > attr_smem.load(std::memory_order_acquire)) {
+        HEAL_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(kSmemLimit)));
+        attr_smem.store(static_cast<size_t>(kSmemLimit), std::memory_order_release);
     }
     CUtensorMap tx_hi, tx_lo, tw_hi, tw_lo;
     int st;
