@@ -23,39 +23,41 @@ struct OutArgs {
                           // C = 2^-10 (lo'.W) + hi.W as the paper's two GEMMs summed into one FP32 output
 };
 
-// The output mode is uniform for the launch: pick it ONCE per store loop (a per-element test costs a dependent
-// constant load + uniform branch, ~100 cycles each -- measured 4 us on a 64-token epilogue) and run the loop body
-// with compile-time flags.  f(out, has_c, has_planes) receives the pinned OutArgs and std::integral_constant-like tags.
+// The output mode is uniform for the launch.  The store loops of the kernels are fully unrolled, run once per CTA (cold
+// instruction cache) and sit on the latency-critical tail, so their code size matters: the common case -- FP32 output
+// only, no accumulate -- is a compile-time FAST path of one multiply and one store per element; everything else
+// (chained planes, planes only, the accumulating second launch of the scaled-lo variant) goes through one out-of-line
+// function per element.  Measured on a 64-row small-M epilogue: 4.1 us with per-element mode tests, 2.3 us with three
+// inlined variants, see DESIGN.md for the current figure.
 template <bool V>
 struct EmitTag {
     static constexpr bool value = V;
 };
 // The fields are pinned in registers first: read in place, the compiler re-loads them from the constant bank for every
-// element (LDCU -> dependent address math, ~70 cycles per store on a 64-row epilogue, measured).
+// element.
 __device__ __forceinline__ OutArgs pin_out(const OutArgs &o)
 {
     OutArgs r = o;
     asm volatile("" : "+l"(r.C), "+l"(r.ldc), "+l"(r.hi), "+l"(r.lo), "+l"(r.ld16), "+f"(r.scale), "+r"(r.accumulate));
     return r;
 }
+// f(out, fast): `fast` is EmitTag<true> when only the FP32 matrix is written and nothing is accumulated
 template <class F>
 __device__ __forceinline__ void emit_dispatch(const OutArgs &o_, F &&f)
 {
     const OutArgs o = pin_out(o_);
-    if (o.hi == nullptr) f(o, EmitTag<true>{}, EmitTag<false>{});
-    else if (o.C == nullptr) f(o, EmitTag<false>{}, EmitTag<true>{});
-    else f(o, EmitTag<true>{}, EmitTag<true>{});
+    if (o.hi == nullptr && o.accumulate == 0) f(o, EmitTag<true>{});
+    else f(o, EmitTag<false>{});
 }
 
-// four consecutive columns col..col+3 of one row (col % 4 == 0); columns >= N are not written
-template <bool HAS_C, bool HAS_P>
-__device__ __forceinline__ void emit4(const OutArgs &o, int64_t row, int col, float4 v, int N)
+// general forms, out of line, arguments by value (the caller's OutArgs stays in registers); v is already scaled
+__device__ __noinline__ void emit4_any(float *C, int64_t ldc, __half *hi, __half *lo, int64_t ld16, int accumulate,
+                                       int64_t row, int col, float4 v, int N)
 {
-    v.x *= o.scale; v.y *= o.scale; v.z *= o.scale; v.w *= o.scale;
     const bool full = col + 3 < N;
-    if (HAS_C) {
-        float *c = o.C + row * o.ldc + col;
-        if (o.accumulate) {
+    if (C) {
+        float *c = C + row * ldc + col;
+        if (accumulate) {
             if (full) {
                 const float4 old = *reinterpret_cast<const float4 *>(c);
                 v.x = __fadd_rn(old.x, v.x); v.y = __fadd_rn(old.y, v.y); v.z = __fadd_rn(old.z, v.z); v.w = __fadd_rn(old.w, v.w);
@@ -73,11 +75,11 @@ __device__ __forceinline__ void emit4(const OutArgs &o, int64_t row, int col, fl
             if (col + 2 < N) c[2] = v.z;
         }
     }
-    if (HAS_P) {
+    if (hi) {
         uint2 h, l;
         split2(v.x, v.y, h.x, l.x);
         split2(v.z, v.w, h.y, l.y);
-        __half *ph = o.hi + row * o.ld16 + col, *pl = o.lo + row * o.ld16 + col;
+        __half *ph = hi + row * ld16 + col, *pl = lo + row * ld16 + col;
         if (full) {
             *reinterpret_cast<uint2 *>(ph) = h;
             *reinterpret_cast<uint2 *>(pl) = l;
@@ -95,21 +97,47 @@ __device__ __forceinline__ void emit4(const OutArgs &o, int64_t row, int col, fl
         }
     }
 }
+__device__ __noinline__ void emit1_any(float *C, int64_t ldc, __half *hi, __half *lo, int64_t ld16, int accumulate,
+                                       int64_t row, int col, float v)
+{
+    if (C) {
+        float *c = C + row * ldc + col;
+        if (accumulate) v = __fadd_rn(*c, v);
+        *c = v;
+    }
+    if (hi) {
+        const __half h = __float2half_rn(v);
+        hi[row * ld16 + col] = h;
+        lo[row * ld16 + col] = __float2half_rn(__fsub_rn(v, __half2float(h)));
+    }
+}
+
+// four consecutive columns col..col+3 of one row (col % 4 == 0); columns >= N are not written
+template <bool FAST>
+__device__ __forceinline__ void emit4(const OutArgs &o, int64_t row, int col, float4 v, int N)
+{
+    v.x *= o.scale; v.y *= o.scale; v.z *= o.scale; v.w *= o.scale;
+    if (FAST) {
+        float *c = o.C + row * o.ldc + col;
+        if (col + 3 < N) {
+            *reinterpret_cast<float4 *>(c) = v;
+        } else {
+            if (col < N) c[0] = v.x;
+            if (col + 1 < N) c[1] = v.y;
+            if (col + 2 < N) c[2] = v.z;
+        }
+    } else {
+        emit4_any(o.C, o.ldc, o.hi, o.lo, o.ld16, o.accumulate, row, col, v, N);
+    }
+}
 
 // one element (the small-M kernel: a warp's lanes are consecutive columns of one row)
-template <bool HAS_C, bool HAS_P>
+template <bool FAST>
 __device__ __forceinline__ void emit1(const OutArgs &o, int64_t row, int col, float v)
 {
     v *= o.scale;
-    if (HAS_C) {
-        if (o.accumulate) v = __fadd_rn(o.C[row * o.ldc + col], v);
-        o.C[row * o.ldc + col] = v;
-    }
-    if (HAS_P) {
-        const __half h = __float2half_rn(v);
-        o.hi[row * o.ld16 + col] = h;
-        o.lo[row * o.ld16 + col] = __float2half_rn(__fsub_rn(v, __half2float(h)));
-    }
+    if (FAST) o.C[row * o.ldc + col] = v;
+    else emit1_any(o.C, o.ldc, o.hi, o.lo, o.ld16, o.accumulate, row, col, v);
 }
 
 }  // namespace heal

@@ -370,6 +370,8 @@ heal_gemm_smallm_kernel(const __grid_constant__ CUtensorMap tm_x_hi, const __gri
         const int quad = warp & 3;
         const int nl = quad * 32 + lane;                   // weight column within the panel = TMEM lane
         const int col = n0 + nl;
+        int Mr = args.M;                                   // kept in a register: the unrolled loops test it per element
+        asm volatile("" : "+r"(Mr));
         if (cs == 1 && ring) {
             // single-CTA panel, ring of TMEM slots: drain each finished segment into the ascending FP32 RN running sum
             // while the tensor core fills the next slot
@@ -380,7 +382,7 @@ heal_gemm_smallm_kernel(const __grid_constant__ CUtensorMap tm_x_hi, const __gri
                 tc_fence_after();
 #pragma unroll
                 for (int c = 0; c < MPAD / 16; ++c) {
-                    if (c * 16 < args.M) {
+                    if (c * 16 < Mr) {
                         uint32_t v[16];
                         tmem_ld_32x32b_x16(tmem_base + (static_cast<uint32_t>(quad * 32) << 16) + static_cast<uint32_t>(slot * MPAD + c * 16), v);
                         tmem_ld_wait();
@@ -399,12 +401,12 @@ heal_gemm_smallm_kernel(const __grid_constant__ CUtensorMap tm_x_hi, const __gri
             }
             if (et == 0) HEAL_STAMP(args.trace, 6);
             if (col < args.N) {
-                emit_dispatch(args.out, [&](const OutArgs &po, auto has_c, auto has_p) {
+                emit_dispatch(args.out, [&](const OutArgs &po, auto fast) {
 #pragma unroll
                     for (int c = 0; c < MPAD / 16; ++c)
 #pragma unroll
                         for (int i = 0; i < 16; ++i)
-                            if (c * 16 + i < args.M) emit1<decltype(has_c)::value, decltype(has_p)::value>(po, c * 16 + i, col, acc[c][i]);
+                            if (c * 16 + i < Mr) emit1<decltype(fast)::value>(po, c * 16 + i, col, acc[c][i]);
                 });
             }
             if (et == 0) HEAL_STAMP(args.trace, 7);
@@ -420,7 +422,7 @@ heal_gemm_smallm_kernel(const __grid_constant__ CUtensorMap tm_x_hi, const __gri
             // single-CTA panel: all segments are local slots; sum them in ascending order in registers
 #pragma unroll
             for (int c = 0; c < MPAD / 16; ++c) {
-                if (c * 16 < args.M) {
+                if (c * 16 < Mr) {
                     const uint32_t taddr = tmem_base + (static_cast<uint32_t>(quad * 32) << 16) + static_cast<uint32_t>(c * 16);
                     uint32_t v[16];
                     float acc[16];
@@ -435,10 +437,10 @@ heal_gemm_smallm_kernel(const __grid_constant__ CUtensorMap tm_x_hi, const __gri
                         for (int i = 0; i < 16; ++i) acc[i] = __fadd_rn(acc[i], __uint_as_float(v[i]));
                     }
                     if (col < args.N) {
-                        emit_dispatch(args.out, [&](const OutArgs &po, auto has_c, auto has_p) {
+                        emit_dispatch(args.out, [&](const OutArgs &po, auto fast) {
 #pragma unroll
                             for (int i = 0; i < 16; ++i)
-                                if (c * 16 + i < args.M) emit1<decltype(has_c)::value, decltype(has_p)::value>(po, c * 16 + i, col, acc[i]);
+                                if (c * 16 + i < Mr) emit1<decltype(fast)::value>(po, c * 16 + i, col, acc[i]);
                         });
                     }
                 }
@@ -458,41 +460,44 @@ heal_gemm_smallm_kernel(const __grid_constant__ CUtensorMap tm_x_hi, const __gri
                 const uint32_t row_off = static_cast<uint32_t>((seg * kSmallBNW + nl) * rpr) * 4u;
 #pragma unroll
                 for (int c = 0; c < MPAD / 16; ++c) {
-                    if (c * 16 < args.M) {
+                    if (c * 16 < Mr) {
                         uint32_t v[16];
                         tmem_ld_32x32b_x16(tmem_base + (static_cast<uint32_t>(quad * 32) << 16) + static_cast<uint32_t>(j * MPAD + c * 16), v);
                         tmem_ld_wait();
                         const bool async = args.red_async != 0;
+                        // owner rank and row inside its block of the first token of this chunk, then stepped along
+                        // (one division per chunk instead of one per element of the unrolled loops)
+                        uint32_t dst = static_cast<uint32_t>((c * 16) / rpr), ml = static_cast<uint32_t>((c * 16) % rpr);
+                        auto step = [&](uint32_t n) {
+                            ml += n;
+                            while (ml >= static_cast<uint32_t>(rpr)) { ml -= static_cast<uint32_t>(rpr); ++dst; }
+                        };
                         if ((rpr & 3) == 0) {
 #pragma unroll
                             for (int i = 0; i < 16; i += 4) {
-                                const int m = c * 16 + i;
-                                if (m < args.M) {         // m % 4 == 0 and rpr % 4 == 0: rows m..m+3 have one owner (rows >= M: unused zeros)
-                                    const uint32_t dst = static_cast<uint32_t>(m / rpr), ml = static_cast<uint32_t>(m % rpr);
+                                if (c * 16 + i < Mr) {    // rpr % 4 == 0: rows m..m+3 have one owner (rows >= M: unused zeros)
                                     const uint32_t a = map_to_cta(red_base + row_off + ml * 4u, dst);
                                     if (async) st_async_v4(a, v[i], v[i + 1], v[i + 2], v[i + 3], map_to_cta(red_bar, dst));
                                     else       st_dsmem_v4(a, v[i], v[i + 1], v[i + 2], v[i + 3]);
                                 }
+                                step(4);
                             }
                         } else if ((rpr & 1) == 0 && async) {
 #pragma unroll
                             for (int i = 0; i < 16; i += 2) {
-                                const int m = c * 16 + i;
-                                if (m < args.M) {
-                                    const uint32_t dst = static_cast<uint32_t>(m / rpr), ml = static_cast<uint32_t>(m % rpr);
+                                if (c * 16 + i < Mr)
                                     st_async_v2(map_to_cta(red_base + row_off + ml * 4u, dst), v[i], v[i + 1], map_to_cta(red_bar, dst));
-                                }
+                                step(2);
                             }
                         } else {
 #pragma unroll
                             for (int i = 0; i < 16; ++i) {
-                                const int m = c * 16 + i;
-                                if (m < args.M) {
-                                    const uint32_t dst = static_cast<uint32_t>(m / rpr), ml = static_cast<uint32_t>(m % rpr);
+                                if (c * 16 + i < Mr) {
                                     const uint32_t a = map_to_cta(red_base + row_off + ml * 4u, dst);
                                     if (async) st_async_b32(a, v[i], map_to_cta(red_bar, dst));
                                     else       st_dsmem_b32(a, v[i]);
                                 }
+                                step(1);
                             }
                         }
                     }
@@ -530,12 +535,12 @@ heal_gemm_smallm_kernel(const __grid_constant__ CUtensorMap tm_x_hi, const __gri
                             acc.z = __fadd_rn(acc.z, v.z); acc.w = __fadd_rn(acc.w, v.w);
                         }
                         if (col < args.N) {
-                            emit_dispatch(args.out, [&](const OutArgs &po, auto has_c, auto has_p) {
-                                constexpr bool kc = decltype(has_c)::value, kp = decltype(has_p)::value;
-                                emit1<kc, kp>(po, m_lo + r4, col, acc.x);
-                                if (r4 + 1 < rows) emit1<kc, kp>(po, m_lo + r4 + 1, col, acc.y);
-                                if (r4 + 2 < rows) emit1<kc, kp>(po, m_lo + r4 + 2, col, acc.z);
-                                if (r4 + 3 < rows) emit1<kc, kp>(po, m_lo + r4 + 3, col, acc.w);
+                            emit_dispatch(args.out, [&](const OutArgs &po, auto fast) {
+                                constexpr bool kf = decltype(fast)::value;
+                                emit1<kf>(po, m_lo + r4, col, acc.x);
+                                if (r4 + 1 < rows) emit1<kf>(po, m_lo + r4 + 1, col, acc.y);
+                                if (r4 + 2 < rows) emit1<kf>(po, m_lo + r4 + 2, col, acc.z);
+                                if (r4 + 3 < rows) emit1<kf>(po, m_lo + r4 + 3, col, acc.w);
                             });
                         }
                     }
@@ -546,8 +551,8 @@ heal_gemm_smallm_kernel(const __grid_constant__ CUtensorMap tm_x_hi, const __gri
 #pragma unroll 4
                         for (int s = 1; s < args.n_seg; ++s) acc = __fadd_rn(acc, src[static_cast<size_t>(s) * seg_stride]);
                         if (col < args.N) {
-                            emit_dispatch(args.out, [&](const OutArgs &po, auto has_c, auto has_p) {
-                                emit1<decltype(has_c)::value, decltype(has_p)::value>(po, m_lo + r, col, acc);
+                            emit_dispatch(args.out, [&](const OutArgs &po, auto fast) {
+                                emit1<decltype(fast)::value>(po, m_lo + r, col, acc);
                             });
                         }
                     }

@@ -273,10 +273,10 @@ heal_gemm_umma2_kernel(const __grid_constant__ CUtensorMap tm_a_hi, const __grid
             const int row = m0 + quad * 32 + lane;
             const int col0 = n0 + chalf * CPW;
             if (row < args.M) {
-                emit_dispatch(args.out, [&](const OutArgs &po, auto has_c, auto has_p) {
+                emit_dispatch(args.out, [&](const OutArgs &po, auto fast) {
 #pragma unroll
                     for (int c = 0; c < CPW; c += 4)
-                        emit4<decltype(has_c)::value, decltype(has_p)::value>(po, row, col0 + c,
+                        emit4<decltype(fast)::value>(po, row, col0 + c,
                                                                               make_float4(run[c], run[c + 1], run[c + 2], run[c + 3]), args.N);
                 });
             }

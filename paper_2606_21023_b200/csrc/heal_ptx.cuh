@@ -73,9 +73,10 @@ __device__ __forceinline__ uint32_t mbar_try_wait(uint32_t bar, uint32_t parity)
         : "memory");
     return ok;
 }
-__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity, int *diag, int code)
+// The slow path (spin + watchdog) is kept out of line: inlined at every wait site it multiplies the code size, and these
+// kernels run most of their code exactly once per CTA, i.e. from a cold instruction cache.
+__device__ __noinline__ void mbar_wait_slow(uint32_t bar, uint32_t parity, int *diag, int code)
 {
-    if (mbar_try_wait(bar, parity)) return;
     const uint64_t t0 = globaltimer_ns();
     uint32_t spins = 0;
     while (!mbar_try_wait(bar, parity)) {
@@ -89,6 +90,11 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity, int *di
             __trap();
         }
     }
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity, int *diag, int code)
+{
+    if (mbar_try_wait(bar, parity)) return;
+    mbar_wait_slow(bar, parity, diag, code);
 }
 
 // ---- TMA -----------------------------------------------------------------------------------
@@ -287,20 +293,23 @@ __device__ __forceinline__ void fence_acq_rel_cluster() { asm volatile("fence.ac
 // generic-proxy shared-memory writes -> visible to the async proxy (TMA / tcgen05 operand reads)
 __device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 // wait with cluster-scope acquire: pairs with mbar_arrive_cluster (release.cluster) from other CTAs
-__device__ __forceinline__ void mbar_wait_cluster(uint32_t bar, uint32_t parity, int *diag, int code)
+__device__ __forceinline__ uint32_t mbar_try_wait_cluster(uint32_t bar, uint32_t parity)
+{
+    uint32_t ok;
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(ok)
+        : "r"(bar), "r"(parity)
+        : "memory");
+    return ok;
+}
+__device__ __noinline__ void mbar_wait_cluster(uint32_t bar, uint32_t parity, int *diag, int code)
 {
     const uint64_t t0 = globaltimer_ns();
     uint32_t spins = 0;
-    for (;;) {
-        uint32_t ok;
-        asm volatile(
-            "{\n\t.reg .pred p;\n\t"
-            "mbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 p, [%1], %2;\n\t"
-            "selp.u32 %0, 1, 0, p;\n\t}"
-            : "=r"(ok)
-            : "r"(bar), "r"(parity)
-            : "memory");
-        if (ok) return;
+    while (!mbar_try_wait_cluster(bar, parity)) {
         if ((++spins & 0x3ffu) == 0 && globaltimer_ns() - t0 > 4000000000ull) {
             if (diag) {
                 diag[0] = code;
