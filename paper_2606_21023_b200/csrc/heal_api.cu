@@ -240,7 +240,18 @@ bool bind_xfer(GemmArgs &args, cudaStream_t stream, size_t part_bytes = 0)
 //  * tiles >= G_max: full waves stay tile-granular; the ragged remainder (plus one full wave when the remainder
 //    alone would leave less than half a tile per CTA) is cut at K-segment granularity.
 //  * tiles < G_max (mid-size M, small N): ordered split-K, see below.
-int64_t set_balance(GemmArgs &args, int64_t tiles, int64_t n_seg, int64_t G_max, int ctas_per_tile, int bn, cudaStream_t stream)
+// the ordered split-K rule of set_balance(), without side effects: decides which kernel instantiation to launch
+bool wants_split_k(int64_t tiles, int64_t n_seg, int64_t G_max, int ctas_per_tile, int bn)
+{
+    if (tiles >= G_max || n_seg <= 1 || std::getenv("HEAL_NO_BALANCE")) return false;
+    const int64_t units = tiles * n_seg;
+    const int64_t G = units < G_max ? units : G_max;
+    const size_t part_bytes = static_cast<size_t>(units) * ctas_per_tile * kBM * bn * sizeof(float);
+    return G > tiles && 12 * ((units + G - 1) / G) < 5 * n_seg && part_bytes <= (static_cast<size_t>(128) << 20);
+}
+
+int64_t set_balance(GemmArgs &args, int64_t tiles, int64_t n_seg, int64_t G_max, int ctas_per_tile, int bn, bool full_kernel,
+                    cudaStream_t stream)
 {
     args.xfer = nullptr;
     args.flags = nullptr;
@@ -259,7 +270,7 @@ int64_t set_balance(GemmArgs &args, int64_t tiles, int64_t n_seg, int64_t G_max,
         // Worth it only while a CTA gets few units: parking and re-reading a partial costs about 1.4 segments of
         // L2 traffic (measured: a parked unit takes 2.4x a plain segment), whole tiles cost n_seg segments.
         const int64_t units_per_cta = (units + G - 1) / G;
-        if (!no_balance && n_seg > 1 && G > tiles && 12 * units_per_cta < 5 * n_seg &&
+        if (full_kernel && !no_balance && n_seg > 1 && G > tiles && 12 * units_per_cta < 5 * n_seg &&
             part_bytes <= (static_cast<size_t>(128) << 20) && bind_xfer(args, stream, part_bytes)) {
             args.balance = 1;
             args.sk = 1;
@@ -319,7 +330,7 @@ int launch_gemm_cfg(int64_t M, int64_t N, int64_t K, const void *A_hi, const voi
     args.tiles_n = static_cast<int>((N + Cfg::BN - 1) / Cfg::BN);
     args.diag = g.diag;
     const int64_t tiles = static_cast<int64_t>(args.tiles_m) * args.tiles_n;
-    const unsigned grid = static_cast<unsigned>(set_balance(args, tiles, (K + kKSeg - 1) / kKSeg, g.num_sms, 1, Cfg::BN, stream));
+    const unsigned grid = static_cast<unsigned>(set_balance(args, tiles, (K + kKSeg - 1) / kKSeg, g.num_sms, 1, Cfg::BN, Cfg::FULL, stream));
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(grid);
     cfg.blockDim = dim3(kGemmThreads);
@@ -372,7 +383,7 @@ int launch_gemm2_cfg(int64_t M, int64_t N, int64_t K, const void *A_hi, const vo
     args.tiles_n = static_cast<int>((N + Cfg::BN - 1) / Cfg::BN);
     args.diag = g.diag;
     const int64_t tiles = static_cast<int64_t>(args.tiles_m) * args.tiles_n;
-    const int64_t G = set_balance(args, tiles, (K + kKSeg - 1) / kKSeg, g.num_sms / 2, 2, Cfg::BN, stream);
+    const int64_t G = set_balance(args, tiles, (K + kKSeg - 1) / kKSeg, g.num_sms / 2, 2, Cfg::BN, Cfg::FULL, stream);
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(static_cast<unsigned>(2 * G));
     cfg.blockDim = dim3(kGemmThreads);
@@ -386,10 +397,22 @@ int launch_gemm2_cfg(int64_t M, int64_t N, int64_t K, const void *A_hi, const vo
     return HEAL_OK;
 }
 
+inline bool needs_ext(const OutArgs &out) { return out.hi != nullptr || out.accumulate != 0 || out.scale != 1.0f || out.C == nullptr; }
+
 template <bool B_MN>
 int launch_gemm2_np(int nprod, int64_t M, int64_t N, int64_t K, const void *A_hi, const void *A_lo, int64_t lda,
                     const void *B_hi, const void *B_lo, int64_t ldb, const OutArgs &out, cudaStream_t s)
 {
+    const int64_t tiles = ((M + 2 * kBM - 1) / (2 * kBM)) * ((N + 255) / 256);
+    if (needs_ext(out) || wants_split_k(tiles, (K + kKSeg - 1) / kKSeg, g.num_sms / 2, 2, 256)) {
+        switch (nprod) {
+        case 1: return launch_gemm2_cfg<Gemm2Cfg<256, 1, B_MN, true>>(M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, out, s);
+        case 2: return launch_gemm2_cfg<Gemm2Cfg<256, 2, B_MN, true>>(M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, out, s);
+        case 3: return launch_gemm2_cfg<Gemm2Cfg<256, 3, B_MN, true>>(M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, out, s);
+        case 4: return launch_gemm2_cfg<Gemm2Cfg<256, 4, B_MN, true>>(M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, out, s);
+        }
+        return HEAL_ERR_UNSUPPORTED_MODE;
+    }
     switch (nprod) {
     case 1: return launch_gemm2_cfg<Gemm2Cfg<256, 1, B_MN>>(M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, out, s);
     case 2: return launch_gemm2_cfg<Gemm2Cfg<256, 2, B_MN>>(M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, out, s);
@@ -403,6 +426,16 @@ template <int BN, bool B_MN>
 int launch_gemm_np(int nprod, int64_t M, int64_t N, int64_t K, const void *A_hi, const void *A_lo, int64_t lda,
                    const void *B_hi, const void *B_lo, int64_t ldb, const OutArgs &out, cudaStream_t s)
 {
+    const int64_t tiles = ((M + kBM - 1) / kBM) * ((N + BN - 1) / BN);
+    if (needs_ext(out) || wants_split_k(tiles, (K + kKSeg - 1) / kKSeg, g.num_sms, 1, BN)) {
+        switch (nprod) {
+        case 1: return launch_gemm_cfg<GemmCfg<BN, 1, B_MN, true>>(M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, out, s);
+        case 2: return launch_gemm_cfg<GemmCfg<BN, 2, B_MN, true>>(M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, out, s);
+        case 3: return launch_gemm_cfg<GemmCfg<BN, 3, B_MN, true>>(M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, out, s);
+        case 4: return launch_gemm_cfg<GemmCfg<BN, 4, B_MN, true>>(M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, out, s);
+        }
+        return HEAL_ERR_UNSUPPORTED_MODE;
+    }
     switch (nprod) {
     case 1: return launch_gemm_cfg<GemmCfg<BN, 1, B_MN>>(M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, out, s);
     case 2: return launch_gemm_cfg<GemmCfg<BN, 2, B_MN>>(M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, out, s);

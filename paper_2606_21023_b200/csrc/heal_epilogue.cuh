@@ -112,6 +112,18 @@ __device__ __noinline__ void emit1_any(float *C, int64_t ldc, __half *hi, __half
     }
 }
 
+// plain FP32 store of four columns (no scale): the kernels' default instantiation
+__device__ __forceinline__ void emit4_plain(float *crow, int col, float4 v, int N)
+{
+    if (col + 3 < N) {
+        *reinterpret_cast<float4 *>(crow + col) = v;
+    } else {
+        if (col < N) crow[col] = v.x;
+        if (col + 1 < N) crow[col + 1] = v.y;
+        if (col + 2 < N) crow[col + 2] = v.z;
+    }
+}
+
 // four consecutive columns col..col+3 of one row (col % 4 == 0); columns >= N are not written
 template <bool FAST>
 __device__ __forceinline__ void emit4(const OutArgs &o, int64_t row, int col, float4 v, int N)

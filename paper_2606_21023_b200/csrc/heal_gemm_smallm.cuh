@@ -224,7 +224,7 @@ heal_gemm_smallm_kernel(const __grid_constant__ CUtensorMap tm_x_hi, const __gri
                 if (pre == STAGES) phase = 1u; else stage = pre;
             }
             for (; t < n_t; ++t) {
-                mbar_wait(empty_bar(stage), phase ^ 1u, args.diag, 500 + stage);
+                mbar_wait_ool(empty_bar(stage), phase ^ 1u, args.diag, 500 + stage);
                 const uint32_t sb = smem_base + stage * Cfg::STAGE_BYTES;
                 const uint32_t fb = full_bar(stage);
                 mbar_arrive_expect_tx(fb, Cfg::TX_BYTES);
@@ -236,7 +236,7 @@ heal_gemm_smallm_kernel(const __grid_constant__ CUtensorMap tm_x_hi, const __gri
         }
         if (cs > 1 && args.red_alias) {
             __syncwarp();
-            mbar_wait(done_bar, 0, args.diag, 701);
+            mbar_wait_ool(done_bar, 0, args.diag, 701);
             cluster_wait();
             cluster_arrive_relaxed();          // "my pipeline is dead": observed through done_bar, no data to publish
         }
@@ -258,13 +258,13 @@ heal_gemm_smallm_kernel(const __grid_constant__ CUtensorMap tm_x_hi, const __gri
                 if ((t & 7) == 0) {                               // new segment -> next TMEM slot
                     accumulate = 0;
                     if (ring && seg_j >= ring) {                  // the slot's previous segment must have been drained
-                        mbar_wait(tempty_bar(slot), static_cast<uint32_t>((seg_j / ring - 1) & 1), args.diag, 640 + slot);
+                        mbar_wait_ool(tempty_bar(slot), static_cast<uint32_t>((seg_j / ring - 1) & 1), args.diag, 640 + slot);
                         tc_fence_after();
                     }
                 }
                 const uint32_t d_tmem = tmem_base + static_cast<uint32_t>(slot * MPAD);
-                mbar_wait(full_bar(stage), phase, args.diag, 600 + stage);
-                if (FUSED) mbar_wait(xfull_bar(stage), phase, args.diag, 620 + stage);
+                mbar_wait_ool(full_bar(stage), phase, args.diag, 600 + stage);
+                if (FUSED) mbar_wait_ool(xfull_bar(stage), phase, args.diag, 620 + stage);
                 tc_fence_after();
                 if (t == 0) HEAL_STAMP(args.trace, 4);
                 if (t == n_t - 1) HEAL_STAMP(args.trace, 5);
@@ -295,7 +295,7 @@ heal_gemm_smallm_kernel(const __grid_constant__ CUtensorMap tm_x_hi, const __gri
         }
         if (cs > 1 && args.red_alias) {
             __syncwarp();
-            mbar_wait(done_bar, 0, args.diag, 702);
+            mbar_wait_ool(done_bar, 0, args.diag, 702);
             cluster_wait();
             cluster_arrive_relaxed();          // "my pipeline is dead": observed through done_bar, no data to publish
         }
@@ -340,7 +340,7 @@ heal_gemm_smallm_kernel(const __grid_constant__ CUtensorMap tm_x_hi, const __gri
                 for (int p = 0; p < PF; ++p) {
                     const int t = t0 + p;
                     if (t < n_t) {
-                        mbar_wait(empty_bar(stage), phase ^ 1u, args.diag, 540 + stage);
+                        mbar_wait_ool(empty_bar(stage), phase ^ 1u, args.diag, 540 + stage);
                         const uint32_t sx = smem_base + stage * Cfg::STAGE_BYTES + Cfg::W_BYTES;
 #pragma unroll
                         for (int q = 0; q < TASKS; ++q) {
@@ -378,7 +378,7 @@ heal_gemm_smallm_kernel(const __grid_constant__ CUtensorMap tm_x_hi, const __gri
             float acc[MPAD / 16][16];
             for (int j = 0; j < n_local; ++j) {
                 const int slot = j % ring;
-                mbar_wait(tfull_bar(slot), static_cast<uint32_t>((j / ring) & 1), args.diag, 660 + slot);
+                mbar_wait_ool(tfull_bar(slot), static_cast<uint32_t>((j / ring) & 1), args.diag, 660 + slot);
                 tc_fence_after();
 #pragma unroll
                 for (int c = 0; c < MPAD / 16; ++c) {
@@ -410,12 +410,12 @@ heal_gemm_smallm_kernel(const __grid_constant__ CUtensorMap tm_x_hi, const __gri
                 });
             }
             if (et == 0) HEAL_STAMP(args.trace, 7);
-            mbar_wait(done_bar, 0, args.diag, 700);        // every MMA (and its commits) has retired before the CTA leaves
+            mbar_wait_ool(done_bar, 0, args.diag, 700);        // every MMA (and its commits) has retired before the CTA leaves
             tc_fence_after();
             tc_fence_before();
             if (et == 0) HEAL_STAMP(args.trace, 8);
         } else {
-        mbar_wait(done_bar, 0, args.diag, 700);
+        mbar_wait_ool(done_bar, 0, args.diag, 700);
         tc_fence_after();
         if (et == 0) HEAL_STAMP(args.trace, 6);
         if (cs == 1) {
@@ -516,7 +516,7 @@ heal_gemm_smallm_kernel(const __grid_constant__ CUtensorMap tm_x_hi, const __gri
             tc_fence_before();
             if (et == 0) HEAL_STAMP(args.trace, 7);
             if (static_cast<int>(rank) < owners) {
-                if (args.red_async) mbar_wait(red_bar, 0, args.diag, 710);       // every byte has landed
+                if (args.red_async) mbar_wait_ool(red_bar, 0, args.diag, 710);       // every byte has landed
                 else                mbar_wait_cluster(red_bar, 0, args.diag, 710);
                 if (et == 0) HEAL_STAMP(args.trace, 8);
                 // this rank finishes rows [rank * rpr, min(M, (rank + 1) * rpr)): ascending segment order, FP32 RN

@@ -91,10 +91,29 @@ __device__ __noinline__ void mbar_wait_slow(uint32_t bar, uint32_t parity, int *
         }
     }
 }
-__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity, int *diag, int code)
+// out-of-line slow path: the small-M kernel (many wait sites, all of them run once per CTA from a cold instruction cache)
+__device__ __forceinline__ void mbar_wait_ool(uint32_t bar, uint32_t parity, int *diag, int code)
 {
     if (mbar_try_wait(bar, parity)) return;
     mbar_wait_slow(bar, parity, diag, code);
+}
+// fully inline: the large-M kernels' steady-state loops (a call there costs register spills around it)
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity, int *diag, int code)
+{
+    if (mbar_try_wait(bar, parity)) return;
+    const uint64_t t0 = globaltimer_ns();
+    uint32_t spins = 0;
+    while (!mbar_try_wait(bar, parity)) {
+        if ((++spins & 0x3ffu) == 0 && globaltimer_ns() - t0 > 4000000000ull) {
+            if (diag) {
+                diag[0] = code;
+                diag[1] = static_cast<int>(blockIdx.x);
+                diag[2] = static_cast<int>(parity);
+            }
+            __threadfence_system();
+            __trap();
+        }
+    }
 }
 
 // ---- TMA -----------------------------------------------------------------------------------
