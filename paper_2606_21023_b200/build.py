@@ -22,7 +22,7 @@ def _sources():
 
 
 def _deps():
-    return _sources() + glob.glob(os.path.join(_CSRC, "*.cuh")) + \
+    return _sources() + glob.glob(os.path.join(_CSRC, "*.cuh")) + glob.glob(os.path.join(_CSRC, "*.h")) + \
         [os.path.join(_HERE, "..", "include", "heal.h")]
 
 

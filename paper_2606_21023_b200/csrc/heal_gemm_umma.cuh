@@ -17,6 +17,7 @@
 #pragma once
 #include "heal_epilogue.cuh"
 #include "heal_ptx.cuh"
+#include "heal_sched.h"
 
 namespace heal {
 
@@ -62,77 +63,6 @@ struct GemmArgs {
     int sk;
     float *part;            // [(tile * R + rank) * n_seg + seg] x (kBM * BN) floats, R = CTAs per tile
     uint32_t *cnt;          // [(tile * R + rank) * 2]: partials written, shares finished (both back to 0 at the end)
-};
-
-// Work distribution.  The unit of work is (tile, K segment).  The first `dp_tiles` tiles (a multiple of
-// gridDim.x) are dealt round-robin, whole tiles, so the CTAs of a wave walk K in lockstep and share W / A
-// panels in L2.  With `balance`, the remaining tiles (the ragged last wave) are cut at segment granularity
-// into gridDim.x contiguous, equal ranges, so a tile may be shared by neighbouring CTAs: CTA c computes
-// the first segments of a tile and hands the FP32 running sum to CTA c+1, which adds the following ones --
-// the same ascending-segment sum, copied, never re-associated, so the result is bit-identical to the
-// unbalanced schedule.  Within its range a CTA processes its "head" (the part it hands on) first and its
-// "tail" (the part that needs a neighbour's prefix) last, so the prefix is almost never waited for.
-struct TileSched {
-    int n_seg, n_dp, n_sk, dp_tiles;
-    int t_first, t_last, s_first, s_last_end, has_head, has_tail;
-    int n_chunks, bid, G;
-    // bid / G_: index of this CTA (or CTA pair) and number of CTAs (pairs) sharing the work
-    __device__ __forceinline__ void init(const GemmArgs &a, int n_seg_, int bid_, int G_)
-    {
-        n_seg = n_seg_;
-        bid = bid_;
-        G = G_;
-        const int num_tiles = a.tiles_m * a.tiles_n;
-        dp_tiles = a.balance ? a.dp_tiles : num_tiles;
-        n_dp = (dp_tiles > bid) ? (dp_tiles - 1 - bid) / G + 1 : 0;
-        n_sk = 0;
-        has_head = has_tail = 0;
-        t_first = t_last = s_first = s_last_end = 0;
-        if (a.balance) {
-            const long long total = static_cast<long long>(num_tiles - dp_tiles) * n_seg;
-            const long long u0 = total * bid / G, u1 = total * (bid + 1) / G;
-            if (u1 > u0) {
-                t_first = static_cast<int>(u0 / n_seg);
-                s_first = static_cast<int>(u0 % n_seg);
-                t_last = static_cast<int>((u1 - 1) / n_seg);
-                s_last_end = static_cast<int>((u1 - 1) % n_seg) + 1;
-                n_sk = t_last - t_first + 1;
-                if (n_sk > 1) {
-                    has_head = (s_last_end < n_seg) ? 1 : 0;
-                    has_tail = (s_first > 0) ? 1 : 0;
-                }
-            }
-        }
-        n_chunks = n_dp + n_sk;
-    }
-    // i-th chunk in processing order: tile index and its segment range [sb, se)
-    __device__ __forceinline__ void get(int i, int &tile, int &sb, int &se) const
-    {
-        if (i < n_dp) {
-            tile = bid + i * G;
-            sb = 0;
-            se = n_seg;
-            return;
-        }
-        i -= n_dp;
-        if (n_sk == 1) {                       // one (possibly partial, possibly interior) piece of a tile
-            tile = dp_tiles + t_first;
-            sb = s_first;
-            se = s_last_end;
-        } else if (has_head && i == 0) {
-            tile = dp_tiles + t_last;
-            sb = 0;
-            se = s_last_end;
-        } else if (has_tail && i == n_sk - 1) {
-            tile = dp_tiles + t_first;
-            sb = s_first;
-            se = n_seg;
-        } else {
-            tile = dp_tiles + t_first + has_tail + (i - has_head);
-            sb = 0;
-            se = n_seg;
-        }
-    }
 };
 
 // ---- ordered split-K helpers (256 epilogue threads, etid = 0..255; thread owns row quad*32+lane, CPW columns) ----
@@ -243,7 +173,7 @@ heal_gemm_umma_kernel(const __grid_constant__ CUtensorMap tm_a_hi, const __grid_
     const int k_tiles = (args.K + kBK - 1) / kBK;
     const int n_seg = (k_tiles + kTilesPerSeg - 1) / kTilesPerSeg;
     TileSched sched;
-    sched.init(args, n_seg, static_cast<int>(blockIdx.x), static_cast<int>(gridDim.x));
+    sched.init(args.tiles_m * args.tiles_n, args.balance, args.dp_tiles, n_seg, static_cast<int>(blockIdx.x), static_cast<int>(gridDim.x));
 
     if (warp == 0 && lane == 0) {
         tma_prefetch_desc(&tm_a_hi);

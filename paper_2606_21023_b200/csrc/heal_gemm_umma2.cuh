@@ -63,7 +63,7 @@ heal_gemm_umma2_kernel(const __grid_constant__ CUtensorMap tm_a_hi, const __grid
     const int k_tiles = (args.K + kBK - 1) / kBK;
     const int n_seg = (k_tiles + kTilesPerSeg - 1) / kTilesPerSeg;
     TileSched sched;
-    sched.init(args, n_seg, static_cast<int>(blockIdx.x >> 1), static_cast<int>(gridDim.x >> 1));
+    sched.init(args.tiles_m * args.tiles_n, args.balance, args.dp_tiles, n_seg, static_cast<int>(blockIdx.x >> 1), static_cast<int>(gridDim.x >> 1));
 
     if (warp == 0 && lane == 0) {
         tma_prefetch_desc(&tm_a_hi);

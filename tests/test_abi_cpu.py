@@ -64,3 +64,15 @@ def test_product_does_not_import_oracle():
     osrc = open(os.path.join(ROOT, "oracle", "__init__.py")).read() + open(os.path.join(ROOT, "oracle", "heal_oracle.c")).read()
     assert "import paper_2606_21023_b200" not in osrc and "from paper_2606_21023_b200" not in osrc
     assert "#include <cuda" not in osrc and "import torch" not in osrc
+
+
+def test_tile_schedule_covers_every_unit_once(tmp_path):
+    """Host logic of the large-M kernels (csrc/heal_sched.h, plain C++): for thousands of (tiles, K segments, CTAs)
+    combinations of the plain, balanced and ordered split-K schedules every (tile, segment) unit is computed exactly
+    once and a tile's pieces form consecutive ranges in ascending CTA order (tests/sched_check.cpp)."""
+    import subprocess
+    exe = tmp_path / "sched_check"
+    subprocess.check_call(["g++", "-O2", "-std=c++17", "-o", str(exe), os.path.join(ROOT, "tests", "sched_check.cpp")])
+    out = subprocess.run([str(exe)], capture_output=True, text=True)
+    assert out.returncode == 0, out.stdout[-2000:]
+    assert ", 0 failures" in out.stdout
