@@ -157,7 +157,9 @@ int heal_gemm_presplit_ex(int64_t M, int64_t N, int64_t K,
  * HOST-buffer variant of heal_gemm: A, B, C are HOST pointers (ideally pinned).  Copies A and B to
  * the device, runs the path, copies C back and synchronises `stream` before returning.  Same
  * layout rules as heal_gemm except that alignment applies to the internal device copies only.
- * Staging buffers are library-owned and reused between calls.
+ * Staging buffers are library-owned and reused between calls.  Large problems are pipelined over blocks of
+ * weight columns on two library-owned copy streams (weights in while the previous block computes and the one
+ * before travels out), with bit-identical results; calls are serialised inside the library.
  */
 int heal_gemm_host(int64_t M, int64_t N, int64_t K,
                    const void *A_host, int64_t lda,

@@ -26,6 +26,7 @@ std::atomic<int> g_last_cuda_error{0};
 std::atomic<uint64_t> g_launches{0};
 std::mutex g_mu;
 std::mutex g_xf_mu;
+std::mutex g_host_mu;
 
 struct State {
     bool init = false;
@@ -53,6 +54,8 @@ struct State {
     // host-variant staging
     void *stage = nullptr;
     size_t stage_bytes = 0;
+    cudaStream_t copy_in = nullptr, copy_out = nullptr;      // host variant: one stream per PCIe direction
+    cudaEvent_t ev_in[8] = {}, ev_done[8] = {}, ev_start = nullptr;
     PFN_cuTensorMapEncodeTiled_v12000 encode = nullptr;
 };
 State g;
@@ -1010,14 +1013,59 @@ int heal_gemm_host(int64_t M, int64_t N, int64_t K, const void *A_host, int64_t 
         }
     }
     char *dA = static_cast<char *>(g.stage), *dB = dA + a_bytes, *dC = dB + b_bytes;
-    if (K > 0) {
-        HEAL_CUDA(cudaMemcpy2DAsync(dA, dlda * 4, A_host, lda * 4, K * 4, M, cudaMemcpyHostToDevice, stream));
-        HEAL_CUDA(cudaMemcpy2DAsync(dB, dldb * b_es, B_host, ldb * b_es, bcols * b_es, brows, cudaMemcpyHostToDevice,
-                                    stream));
+    // Large problems are pipelined over blocks of weight columns: block b's weights travel host -> device on one copy
+    // stream while block b-1 is computed and block b-2's results travel device -> host on another, so the two PCIe
+    // directions work at the same time.  The per-element reduction order does not depend on the tile or block an
+    // element falls in, so the result is bit-identical to the one-shot path.
+    const int64_t kBlockCols = 2048;
+    const int64_t nb = (K > 0 && N > kBlockCols && static_cast<size_t>(K) * N * b_es >= (static_cast<size_t>(32) << 20)) ? (N + kBlockCols - 1) / kBlockCols : 1;
+    if (nb == 1) {
+        if (K > 0) {
+            HEAL_CUDA(cudaMemcpy2DAsync(dA, dlda * 4, A_host, lda * 4, K * 4, M, cudaMemcpyHostToDevice, stream));
+            HEAL_CUDA(cudaMemcpy2DAsync(dB, dldb * b_es, B_host, ldb * b_es, bcols * b_es, brows, cudaMemcpyHostToDevice,
+                                        stream));
+        }
+        st = heal_gemm(M, N, K, dA, dlda, dB, dldb, dC, dldc, mode, stream_);
+        if (st) return st;
+        HEAL_CUDA(cudaMemcpy2DAsync(C_host, ldc * 4, dC, dldc * 4, N * 4, M, cudaMemcpyDeviceToHost, stream));
+        HEAL_CUDA(cudaStreamSynchronize(stream));
+        return HEAL_OK;
     }
-    st = heal_gemm(M, N, K, dA, dlda, dB, dldb, dC, dldc, mode, stream_);
-    if (st) return st;
-    HEAL_CUDA(cudaMemcpy2DAsync(C_host, ldc * 4, dC, dldc * 4, N * 4, M, cudaMemcpyDeviceToHost, stream));
+    std::lock_guard<std::mutex> lk(g_host_mu);                  // the copy streams and events below are shared
+    if (!g.copy_in) {
+        HEAL_CUDA(cudaStreamCreateWithFlags(&g.copy_in, cudaStreamNonBlocking));
+        HEAL_CUDA(cudaStreamCreateWithFlags(&g.copy_out, cudaStreamNonBlocking));
+        for (auto &e : g.ev_in) HEAL_CUDA(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+        for (auto &e : g.ev_done) HEAL_CUDA(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+        HEAL_CUDA(cudaEventCreateWithFlags(&g.ev_start, cudaEventDisableTiming));
+    }
+    constexpr int kEv = 8;                                       // events are recycled round-robin; a block's events are
+                                                                 // re-recorded only after the stream that waits on them got there
+    HEAL_CUDA(cudaEventRecord(g.ev_start, stream));              // staging buffers are free once earlier work on `stream` is done
+    HEAL_CUDA(cudaStreamWaitEvent(g.copy_in, g.ev_start, 0));
+    HEAL_CUDA(cudaStreamWaitEvent(g.copy_out, g.ev_start, 0));
+    HEAL_CUDA(cudaMemcpy2DAsync(dA, dlda * 4, A_host, lda * 4, K * 4, M, cudaMemcpyHostToDevice, g.copy_in));
+    const char *Bh = static_cast<const char *>(B_host);
+    for (int64_t b = 0; b < nb; ++b) {
+        const int64_t c0 = b * kBlockCols, cw = (N - c0 < kBlockCols) ? N - c0 : kBlockCols;
+        if (b >= kEv) HEAL_CUDA(cudaEventSynchronize(g.ev_done[b % kEv]));       // block b - kEv fully consumed: its events are free
+        // weights of this block: columns c0.. (K x N storage) or rows c0.. (N x K storage)
+        if (b_nk)
+            HEAL_CUDA(cudaMemcpy2DAsync(dB + c0 * dldb * b_es, dldb * b_es, Bh + c0 * ldb * b_es, ldb * b_es, K * b_es, cw,
+                                        cudaMemcpyHostToDevice, g.copy_in));
+        else
+            HEAL_CUDA(cudaMemcpy2DAsync(dB + c0 * b_es, dldb * b_es, Bh + c0 * b_es, ldb * b_es, cw * b_es, K,
+                                        cudaMemcpyHostToDevice, g.copy_in));
+        HEAL_CUDA(cudaEventRecord(g.ev_in[b % kEv], g.copy_in));
+        HEAL_CUDA(cudaStreamWaitEvent(stream, g.ev_in[b % kEv], 0));
+        st = heal_gemm(M, cw, K, dA, dlda, b_nk ? dB + c0 * dldb * b_es : dB + c0 * b_es, dldb, dC + c0 * 4, dldc, mode, stream_);
+        if (st) return st;
+        HEAL_CUDA(cudaEventRecord(g.ev_done[b % kEv], stream));
+        HEAL_CUDA(cudaStreamWaitEvent(g.copy_out, g.ev_done[b % kEv], 0));
+        HEAL_CUDA(cudaMemcpy2DAsync(static_cast<char *>(C_host) + c0 * 4, ldc * 4, dC + c0 * 4, dldc * 4, cw * 4, M,
+                                    cudaMemcpyDeviceToHost, g.copy_out));
+    }
+    HEAL_CUDA(cudaStreamSynchronize(g.copy_out));
     HEAL_CUDA(cudaStreamSynchronize(stream));
     return HEAL_OK;
 }

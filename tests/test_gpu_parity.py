@@ -639,6 +639,26 @@ def test_presplit_and_host_variants_match(hb, inputs):
 
 # --------------------------------------------------------------------------------- edges / contract
 
+@pytest.mark.parametrize("b_nk", [False, True])
+def test_host_variant_pipelined_blocks(hb, inputs, b_nk):
+    """heal_gemm_host on a problem large enough to be pipelined over blocks of weight columns (weights in, results out
+    on separate copy streams): bit-identical to the device call, ragged last block, padded host leading dimensions."""
+    M, K, N = 70, 4096, 4104
+    A = inputs.activations(M, K, seed=25, outliers=True)
+    W = inputs.weights_f16(K, N, seed=25, nk=b_nk)
+    mode = 2 | (hb.B_NK if b_nk else 0)
+    want = hb.heal_gemm(dev(A), dev(W), mode).cpu()
+    Ah = torch.zeros((M, K + 4)).pin_memory()
+    Ah[:, :K] = torch.from_numpy(A)
+    Wh = torch.zeros((W.shape[0], W.shape[1] + 8), dtype=torch.float16).pin_memory()
+    Wh[:, :W.shape[1]] = torch.from_numpy(W)
+    Ch = torch.full((M, N + 4), 7.0).pin_memory()
+    for _ in range(2):
+        hb.heal_gemm_host(Ah[:, :K], Wh[:, :W.shape[1]], mode, C=Ch[:, :N])
+        assert torch.equal(Ch[:, :N], want)
+        assert torch.all(Ch[:, N:] == 7.0)
+
+
 def test_empty_and_k0(hb):
     A = torch.zeros((0, 64), device="cuda")
     W = torch.zeros((64, 16), dtype=torch.float16, device="cuda")
