@@ -64,7 +64,8 @@ typedef enum {
                                   operations enqueued on `stream` just before this call.  The kernel may
                                   then start streaming B while its stream predecessor is still finishing
                                   (programmatic dependent launch); everything that reads A or writes C
-                                  still waits for the predecessor.  Same bits with or without the flag. */
+                                  still waits for the predecessor.  Same bits with or without the flag.  Ignored by
+                                  heal_gemm in the FP32-B modes (3P/4P), whose B planes are produced on the fly. */
 
 #define HEAL_LO_SHIFT 10
 #define HEAL_LO_SCALED 0x40u   /* the paper's scaled residual, Eq. 10 as printed: h = h_hi +
@@ -86,9 +87,12 @@ typedef enum {
  *   C    FP32, ldc >= N, 16-byte aligned, ldc % 4 == 0.  Overwritten (no beta).  Must not alias A/B.
  *   M == 0 or N == 0: no-op, HEAL_OK.  K == 0: C is zero-filled.
  * Ownership: the caller owns A, B, C and keeps them alive until `stream` has passed the call.  The
- * hi/lo planes live in a library-owned workspace (see heal_set_workspace) which this call may
- * grow with stream-ordered allocation; calls that share a workspace must be issued on one stream
- * at a time.  Numerical contract: finite inputs with |x| <= 65504 (activations
+ * hi/lo planes live in a library-owned workspace -- one per stream (up to 8 streams; beyond that the
+ * least recently used one is recycled after a device synchronise), grown on first use, so calls on
+ * different streams may run concurrently.  A caller-supplied workspace (heal_set_workspace) is
+ * shared by all streams: calls that use it must be issued on one stream at a time.  During stream
+ * capture the library does not allocate: run the call once eagerly on that stream first (or supply
+ * a workspace), else HEAL_ERR_WORKSPACE.  Numerical contract: finite inputs with |x| <= 65504 (activations
  * observed < 1024); anything larger, Inf or NaN propagates to Inf/NaN in the affected rows/columns.
  */
 int heal_gemm(int64_t M, int64_t N, int64_t K,

@@ -41,6 +41,8 @@ struct State {
         float *xfer = nullptr;     // per-CTA running-sum slots (128 x 256 floats each)
         uint32_t *flags = nullptr; // per-CTA flag: 1 = slot written, reset by the consumer
         uint64_t last_use = 0;     // for recycling the least recently used slot when all 8 are taken
+        void *ws = nullptr;        // library-owned hi/lo plane workspace of this stream, grown on demand
+        size_t ws_bytes = 0;
         float *part = nullptr;     // ordered split-K: segment partials, grown on demand (never while capturing)
         size_t part_bytes = 0;
         uint32_t *cnt = nullptr;   // ordered split-K: two counters per (tile, rank), all zero between launches
@@ -49,8 +51,6 @@ struct State {
     // workspace
     void *user_ws = nullptr;
     size_t user_ws_bytes = 0;
-    void *own_ws = nullptr;
-    size_t own_ws_bytes = 0;
     // host-variant staging
     void *stage = nullptr;
     size_t stage_bytes = 0;
@@ -175,34 +175,48 @@ int launch_split(int64_t rows, int64_t cols, const float *X, int64_t ldx, __half
     return HEAL_OK;
 }
 
-// Hand-off buffers for `stream`: created on first use (19 MB per stream + the split-K partial area, grown on
-// demand); 8 slots, the least recently used one is recycled (after a device synchronise) when a ninth stream
-// shows up.  During stream capture nothing is allocated: an unbound stream runs the unbalanced schedule (same bits).
-bool bind_xfer(GemmArgs &args, cudaStream_t stream, size_t part_bytes = 0)
+// Per-stream resources (hi/lo plane workspace, balanced-schedule hand-off buffers, split-K partial area): 8 slots, one
+// per stream that has called into the library, so calls on different streams never share scratch memory.  The least
+// recently used slot is recycled (after a device synchronise; it keeps its buffers) when a ninth stream shows up.
+// During stream capture nothing is allocated: what a captured call needs must exist from an earlier eager call on the
+// same stream (else: unbalanced schedule for the GEMM, HEAL_ERR_WORKSPACE for the planes).  Call with g_xf_mu held.
+State::Xfer *acquire_slot(cudaStream_t stream, bool capturing)
 {
-    std::lock_guard<std::mutex> lk(g_xf_mu);
+    static uint64_t tick = 0;
     State::Xfer *slot = nullptr;
     for (auto &x : g.xf)
         if (x.used && x.stream == stream) { slot = &x; break; }
-    cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
-    const bool capturing = cudaStreamIsCapturing(stream, &cap) != cudaSuccess || cap != cudaStreamCaptureStatusNone;
-    static uint64_t tick = 0;
     if (!slot && !capturing) {
-        // all slots taken (streams come and go): recycle the least recently used one once the device is idle
-        bool any_free = false;
-        for (auto &x : g.xf) any_free = any_free || !x.used;
-        if (!any_free && cudaDeviceSynchronize() == cudaSuccess) {
-            State::Xfer *lru = &g.xf[0];
-            for (auto &x : g.xf)
-                if (x.last_use < lru->last_use) lru = &x;
-            lru->stream = stream;
-            slot = lru;
-        }
-    }
-    if (!slot) {
         for (auto &x : g.xf)
             if (!x.used) { slot = &x; break; }
-        if (!slot || capturing) return false;
+        if (!slot && cudaDeviceSynchronize() == cudaSuccess) {
+            slot = &g.xf[0];
+            for (auto &x : g.xf)
+                if (x.last_use < slot->last_use) slot = &x;
+        }
+        if (slot) {
+            slot->stream = stream;
+            slot->used = true;
+        }
+    }
+    if (slot) slot->last_use = ++tick;
+    return slot;
+}
+
+bool stream_capturing(cudaStream_t stream)
+{
+    cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+    return cudaStreamIsCapturing(stream, &cap) != cudaSuccess || cap != cudaStreamCaptureStatusNone;
+}
+
+bool bind_xfer(GemmArgs &args, cudaStream_t stream, size_t part_bytes = 0)
+{
+    std::lock_guard<std::mutex> lk(g_xf_mu);
+    const bool capturing = stream_capturing(stream);
+    State::Xfer *slot = acquire_slot(stream, capturing);
+    if (!slot) return false;
+    if (!slot->xfer) {                                   // 19 MB of hand-off slots + flags + split-K counters, first use only
+        if (capturing) return false;
         float *xf = nullptr;
         uint32_t *fl = nullptr, *cn = nullptr;
         const size_t cnt_bytes = static_cast<size_t>(g.num_sms) * 4 * sizeof(uint32_t);
@@ -215,8 +229,6 @@ bool bind_xfer(GemmArgs &args, cudaStream_t stream, size_t part_bytes = 0)
             if (cn) cudaFree(cn);
             return false;
         }
-        slot->stream = stream;
-        slot->used = true;
         slot->xfer = xf;
         slot->flags = fl;
         slot->cnt = cn;
@@ -230,7 +242,6 @@ bool bind_xfer(GemmArgs &args, cudaStream_t stream, size_t part_bytes = 0)
         if (cudaMalloc(&slot->part, part_bytes) != cudaSuccess) return false;
         slot->part_bytes = part_bytes;
     }
-    slot->last_use = ++tick;
     args.xfer = slot->xfer;
     args.flags = slot->flags;
     args.part = slot->part;
@@ -731,19 +742,25 @@ WsPlan plan_ws(int64_t M, int64_t N, int64_t K, int nprod, bool b_nk)
 
 int get_ws(size_t bytes, cudaStream_t stream, void **out)
 {
-    if (g.user_ws) {
+    if (g.user_ws) {                                     // caller-owned: shared by all streams, the caller serialises
         if (bytes > g.user_ws_bytes) return HEAL_ERR_WORKSPACE;
         *out = g.user_ws;
         return HEAL_OK;
     }
-    if (bytes > g.own_ws_bytes) {
-        if (g.own_ws) HEAL_CUDA(cudaFreeAsync(g.own_ws, stream));
-        g.own_ws = nullptr;
-        g.own_ws_bytes = 0;
-        HEAL_CUDA(cudaMallocAsync(&g.own_ws, bytes, stream));
-        g.own_ws_bytes = bytes;
+    std::lock_guard<std::mutex> lk(g_xf_mu);
+    const bool capturing = stream_capturing(stream);
+    State::Xfer *slot = acquire_slot(stream, capturing);
+    if (!slot) return HEAL_ERR_WORKSPACE;                // capturing on a stream the library has never seen
+    if (bytes > slot->ws_bytes) {
+        if (capturing) return HEAL_ERR_WORKSPACE;        // run the call once eagerly, or supply a workspace
+        HEAL_CUDA(cudaStreamSynchronize(stream));        // earlier calls on this stream may still read the old planes
+        if (slot->ws) HEAL_CUDA(cudaFree(slot->ws));
+        slot->ws = nullptr;
+        slot->ws_bytes = 0;
+        HEAL_CUDA(cudaMalloc(&slot->ws, bytes));
+        slot->ws_bytes = bytes;
     }
-    *out = g.own_ws;
+    *out = slot->ws;
     return HEAL_OK;
 }
 
@@ -971,7 +988,9 @@ int heal_gemm_ex(int64_t M, int64_t N, int64_t K, const void *A, int64_t lda, co
         b_lo = bl;
         ldb_eff = p.ldb_p;
     }
-    return presplit_impl(M, N, K, a_hi, a_lo, p.lda_p, b_hi, b_lo, ldb_eff, out, nprod, b_nk, b_static, stream);
+    // FP32 B: its planes were written by the split kernel just launched on this stream, so the static-weights
+    // promise cannot be passed on (the GEMM would prefetch them before that kernel has finished)
+    return presplit_impl(M, N, K, a_hi, a_lo, p.lda_p, b_hi, b_lo, ldb_eff, out, nprod, b_nk, b_static && !b_f32, stream);
 }
 
 int heal_gemm(int64_t M, int64_t N, int64_t K, const void *A, int64_t lda, const void *B, int64_t ldb, void *C,

@@ -564,6 +564,37 @@ def test_ordered_split_k_two_streams(hb, inputs):
         assert torch.equal(a, r1) and torch.equal(d, r1) and torch.equal(b, r2) and torch.equal(c, r2)
 
 
+def test_static_flag_with_on_the_fly_weight_split(hb, inputs):
+    """HEAL_B_STATIC on a three-product heal_gemm: the B planes are written by the library's own split kernel right
+    before the GEMM, so the flag must not let the GEMM prefetch them early (found by a soak run: stale planes of the
+    previous call).  Alternate two different problems that share the workspace."""
+    A1 = dev(inputs.activations(64, 256, seed=26)); B1 = dev(inputs.weights_f32(256, 256, seed=26, dist="normal"))
+    A2 = dev(inputs.activations(48, 512, seed=27)); B2 = dev(inputs.weights_f32(512, 264, seed=27, dist="normal"))
+    r1 = hb.heal_gemm(A1, B1, 3).clone()
+    r2 = hb.heal_gemm(A2, B2, 3).clone()
+    for _ in range(50):
+        c1 = hb.heal_gemm(A1, B1, 3 | hb.B_STATIC)
+        c2 = hb.heal_gemm(A2, B2, 3 | hb.B_STATIC)
+        assert torch.equal(c1, r1) and torch.equal(c2, r2)
+
+
+def test_concurrent_streams_have_their_own_workspace(hb, inputs):
+    """Calls on different streams run concurrently with library-owned hi/lo planes: one workspace per stream."""
+    A1 = dev(inputs.activations(300, 2056, seed=28)); W1 = dev(inputs.weights_f16(2056, 520, seed=28))
+    A2 = dev(inputs.activations(64, 4096, seed=29)); W2 = dev(inputs.weights_f16(4096, 1032, seed=29))
+    r1 = hb.heal_gemm(A1, W1, 2).clone()
+    r2 = hb.heal_gemm(A2, W2, 2).clone()
+    s1, s2, s3 = torch.cuda.Stream(), torch.cuda.Stream(), torch.cuda.Stream()
+    outs = []
+    torch.cuda.synchronize()
+    for _ in range(40):
+        for s, (A, W, r) in ((s1, (A1, W1, r1)), (s2, (A2, W2, r2)), (s3, (A1, W1, r1)), (s1, (A2, W2, r2))):
+            with torch.cuda.stream(s):
+                outs.append((hb.heal_gemm(A, W, 2), r))
+    torch.cuda.synchronize()
+    assert all(torch.equal(c, r) for c, r in outs)
+
+
 def test_static_weights_graph_chain(hb, inputs):
     """HEAL_B_STATIC in a captured chain of decode GEMMs (each kernel streams its weights while its predecessor
     finishes; activations and C wait): every replay reproduces the eager results bit for bit, including a chain
