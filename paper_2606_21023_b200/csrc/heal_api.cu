@@ -955,9 +955,10 @@ int heal_gemm_ex(int64_t M, int64_t N, int64_t K, const void *A, int64_t lda, co
     if (K == 0) return presplit_impl(M, N, K, nullptr, nullptr, lda, nullptr, nullptr, ldb, out, nprod, b_nk, b_static, stream);
     static const bool no_fused = std::getenv("HEAL_NO_FUSED") != nullptr;          // debug only
     const bool lo_scaled = (mode & HEAL_LO_SCALED) != 0;
-    if (M <= 16 && !b_f32 && !no_fused && !lo_scaled && forced_kernel() != 1) {
+    if (M <= 16 && K <= 8192 && !b_f32 && !no_fused && !lo_scaled && forced_kernel() != 1) {
         // decode shapes (M <= 16) with FP16 weights: step S runs inside the GEMM kernel (no planes, one launch);
-        // above that the in-kernel conversion costs more than the split launch it saves (measured)
+        // above that -- and for long K, where a CTA converts many k-tiles -- the in-kernel conversion costs more
+        // than the split launch it saves (measured: M = 1, K = 14336 31 vs 28 us)
         bool handled = false;
         st = presplit_impl(M, N, K, nullptr, nullptr, 0, B, nullptr, ldb, out, nprod, b_nk, b_static, stream,
                            static_cast<const float *>(A), lda, &handled);

@@ -151,6 +151,8 @@ def main():
              ("Q3-14B up/gate", 2048, 17408, 5120, 2, "normal"), ("Q3-14B down", 2048, 5120, 17408, 2, "normal"),
              ("Q3-14B qkv", 2048, 7168, 5120, 2, "normal")]
     cfgs += [(f"decode down M={m}", m, 4096, 14336, 2, "normal") for m in (1, 32)]
+    cfgs += [(f"decode gate+up M={m}", m, 28672, 4096, 2, "normal") for m in (1, 32)]
+    cfgs += [("decode qkv M=1", 1, 6144, 4096, 2, "normal")]
     cfgs += [(f"decode M={m}", m, 4096, 4096, 2, "normal") for m in (64,)]
     cfgs += [(f"mid M={m}", m, 4096, 4096, 2, "normal") for m in (128, 256, 512, 1024)]
     for c in cfgs:

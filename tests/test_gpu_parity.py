@@ -320,7 +320,7 @@ def test_kernel_families_bit_identical(hb, inputs, M, N, K, nprod, b_nk):
     assert torch.equal(outs[0], outs[1]) and torch.equal(outs[0], outs[2])
 
 
-@pytest.mark.parametrize("M,N,K,b_nk", [(1, 4096, 4096, False), (8, 1032, 4096, False), (16, 520, 14336, False), (13, 264, 1000, True),
+@pytest.mark.parametrize("M,N,K,b_nk", [(1, 4096, 4096, False), (8, 1032, 4096, False), (16, 520, 8192, False), (13, 264, 1000, True),
                                         (5, 4096, 520, True), (16, 128, 8192, False)])
 def test_fused_split_small_m_bit_identical(hb, oracle, inputs, M, N, K, b_nk):
     """M <= 16 with FP16 weights: heal_gemm splits the activations inside the GEMM kernel (no planes, one launch).
