@@ -485,6 +485,11 @@ struct SmallIn {
     bool b_static;
 };
 
+// st.async pushes (lowest latency) pay off while a thread sends few values: up to 8 of any width, or up to 32 8-byte
+// vectors (the plain path has no 8-byte form and falls back to 4-byte remote stores, which are slow; measured: M = 16,
+// K = 6144 21.7 -> 15.7 us, K = 14336 36.9 -> 26.9 us).
+inline bool async_push_ok(int64_t pushes, int64_t vw) { return pushes <= 8 || (vw == 2 && pushes <= 32); }
+
 template <class Cfg>
 int launch_small_cfg(int64_t M, int64_t N, int64_t K, const SmallIn &in, const void *B_hi, const void *B_lo, int64_t ldb,
                      const OutArgs &out, cudaStream_t stream, bool *handled)
@@ -496,9 +501,25 @@ int launch_small_cfg(int64_t M, int64_t N, int64_t K, const SmallIn &in, const v
     // and at most n_seg.  Purely a performance choice: the result does not depend on it (segment sums are exact copies).
     int cs = 1;
     while (cs * 2 <= 8 && cs * 2 <= n_seg && panels * cs * 5 < 7 * g.num_sms) cs *= 2;
+    // The doubling above ignores balance: with n_seg = 28 (K = 14336) a cluster of 8 leaves four ranks with 4 segments
+    // and four with 3.  For few tokens (cheap reduction) take instead the smallest cluster, down to cs/2 + 1, that keeps
+    // the longest rank as short, as long as about 1.2 CTAs per SM remain (measured: K = 14336 M = 1 26.1 -> 23.6 us with
+    // 7 ranks, K = 6144 M = 8 16.5 -> 13.3 us with 6).
+    if (cs > 2 && M <= 16) {
+        const int longest = (n_seg + cs - 1) / cs;
+        for (int c = cs / 2 + 1; c < cs; ++c) {
+            int64_t r = (M + c - 1) / c;                                        // rows per rank (rounded as below), pushes per thread
+            if (r >= 3) r = (r + 3) / 4 * 4;
+            const int64_t vw = (r & 3) == 0 ? 4 : ((r & 1) == 0 ? 2 : 1);
+            if ((n_seg + c - 1) / c == longest && panels * c * 5 >= 6 * g.num_sms && async_push_ok(longest * ((M + vw - 1) / vw), vw)) {
+                cs = c;                                                          // (only while the pushes stay st.async)
+                break;
+            }
+        }
+    }
     if (const char *e = std::getenv("HEAL_SMALL_CS")) {                          // debug only
         const int want = std::atoi(e);
-        if (want == 1 || want == 2 || want == 4 || want == 8) cs = want <= n_seg ? want : cs;
+        if (want >= 1 && want <= 8) cs = want <= n_seg ? want : cs;
     }
     int max_local = (n_seg + cs - 1) / cs;
     // One CTA per panel reading planes, and the segments would need more than 256 TMEM columns (one CTA per SM):
@@ -520,7 +541,10 @@ int launch_small_cfg(int64_t M, int64_t N, int64_t K, const SmallIn &in, const v
     int tmem_cols = 32;
     while (tmem_cols < (use_ring ? ring : max_local) * Cfg::MPAD) tmem_cols *= 2;
     if (tmem_cols > 512) return HEAL_OK;                        // leave to the large-M kernel
-    const int rpr = cs > 1 ? static_cast<int>((M + cs - 1) / cs) : 0;
+    // token rows finished by one rank; 3 or more are rounded up to a multiple of 4 so that the pushes are 16-byte vectors
+    // (fewer ranks then own rows; measured: M = 24 decode 16.5 us with 4-byte pushes vs 9.9 us at M = 32)
+    int rpr = cs > 1 ? static_cast<int>((M + cs - 1) / cs) : 0;
+    if (rpr >= 3) rpr = (rpr + 3) / 4 * 4;
     const size_t red = cs > 1 ? static_cast<size_t>(n_seg) * rpr * kSmallBNW * 4 : 0;
     // Shared memory.  Measured on B200 (decode 4096 x 4096, LM head): what matters is how many CTAs are resident
     // -- the next kernel's CTAs run their prologue (and with HEAL_B_STATIC prefetch W) beside this kernel's --
@@ -596,7 +620,7 @@ int launch_small_cfg(int64_t M, int64_t N, int64_t K, const SmallIn &in, const v
         const int vw = (rpr & 3) == 0 ? 4 : ((rpr & 1) == 0 ? 2 : 1);
         const int64_t pushes = cs > 1 ? static_cast<int64_t>(max_local) * ((M + vw - 1) / vw) : 0;
         static const bool no_async = std::getenv("HEAL_NO_ASYNC_PUSH") != nullptr;        // debug only
-        args.red_async = (cs > 1 && pushes <= 8 && !no_async) ? 1 : 0;
+        args.red_async = (cs > 1 && async_push_ok(pushes, vw) && !no_async) ? 1 : 0;
     }
     args.ring = ring;
     static const bool no_static = std::getenv("HEAL_NO_STATIC") != nullptr;       // debug only
