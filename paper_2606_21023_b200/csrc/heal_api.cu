@@ -552,7 +552,8 @@ int launch_small_cfg(int64_t M, int64_t N, int64_t K, const SmallIn &in, const v
     // one when the CTA needs more than half of TMEM), at least 2 stages, at most 8 and no more than the CTA
     // has k-tiles.
     // Partial sums pushed by the cluster: a dedicated area when small (decode), else overlaid on the pipeline.
-    const bool red_alias = red > static_cast<size_t>(16 * 1024);
+    static const size_t alias_min = std::getenv("HEAL_RED_ALIAS_MIN") ? static_cast<size_t>(std::atol(std::getenv("HEAL_RED_ALIAS_MIN"))) : 16 * 1024;   // debug only
+    const bool red_alias = red > alias_min;
     const size_t fixed = 1024 + (red_alias ? 0 : red) + Cfg::BAR_BYTES;
     size_t budget = tmem_cols > 256 ? static_cast<size_t>(kSmemLimit)
                     : (Cfg::STAGE_BYTES <= 24 * 1024 && cs > 1 ? static_cast<size_t>(74 * 1024) : static_cast<size_t>(112 * 1024));
