@@ -92,8 +92,10 @@ typedef enum {
  * different streams may run concurrently.  A caller-supplied workspace (heal_set_workspace) is
  * shared by all streams: calls that use it must be issued on one stream at a time.  During stream
  * capture the library does not allocate: run the call once eagerly on that stream first (or supply
- * a workspace), else HEAL_ERR_WORKSPACE.  Numerical contract: finite inputs with |x| <= 65504 (activations
- * observed < 1024); anything larger, Inf or NaN propagates to Inf/NaN in the affected rows/columns.
+ * a workspace), else HEAL_ERR_WORKSPACE.  With FP16 weights, M <= 16 and K <= 8192 the split runs
+ * inside the GEMM kernel: one launch, no workspace.
+ * Numerical contract: finite inputs with |x| <= 65504 (activations observed
+ * < 1024); anything larger, Inf or NaN propagates to Inf/NaN in the affected rows/columns.
  */
 int heal_gemm(int64_t M, int64_t N, int64_t K,
               const void *A, int64_t lda,
