@@ -500,7 +500,7 @@ int launch_small_cfg(int64_t M, int64_t N, int64_t K, const SmallIn &in, const v
     // Cluster size: the smallest that gives about 1.4 CTAs per SM (measured: enough to saturate HBM), at most 8
     // and at most n_seg.  Purely a performance choice: the result does not depend on it (segment sums are exact copies).
     int cs = 1;
-    while (cs * 2 <= 8 && cs * 2 <= n_seg && panels * cs * 5 < 7 * g.num_sms) cs *= 2;
+    while (!Cfg::PAIR && cs * 2 <= 8 && cs * 2 <= n_seg && panels * cs * 5 < 7 * g.num_sms) cs *= 2;
     // The doubling above ignores balance: with n_seg = 28 (K = 14336) a cluster of 8 leaves four ranks with 4 segments
     // and four with 3.  For few tokens (cheap reduction) take instead the smallest cluster, down to cs/2 + 1, that keeps
     // the longest rank as short, as long as about 1.2 CTAs per SM remain (measured: K = 14336 M = 1 26.1 -> 23.6 us with
@@ -519,7 +519,7 @@ int launch_small_cfg(int64_t M, int64_t N, int64_t K, const SmallIn &in, const v
     }
     if (const char *e = std::getenv("HEAL_SMALL_CS")) {                          // debug only
         const int want = std::atoi(e);
-        if (want >= 1 && want <= 8) cs = want <= n_seg ? want : cs;
+        if (!Cfg::PAIR && want >= 1 && want <= 8) cs = want <= n_seg ? want : cs;
     }
     int max_local = (n_seg + cs - 1) / cs;
     // One CTA per panel reading planes, and the segments would need more than 256 TMEM columns (one CTA per SM):
@@ -593,10 +593,10 @@ int launch_small_cfg(int64_t M, int64_t N, int64_t K, const SmallIn &in, const v
     if (Cfg::FUSED) {
         tx_hi = tx_lo = tw_hi;                                  // unused by the fused kernel
     } else {
-        st = encode_f16_2d(&tx_hi, in.A_hi, K, M, in.lda, kBK, Cfg::MPAD);
+        st = encode_f16_2d(&tx_hi, in.A_hi, K, M, in.lda, kBK, Cfg::XROWS);
         if (st) return st;
         if (Cfg::A_PLANES == 2) {
-            st = encode_f16_2d(&tx_lo, in.A_lo, K, M, in.lda, kBK, Cfg::MPAD);
+            st = encode_f16_2d(&tx_lo, in.A_lo, K, M, in.lda, kBK, Cfg::XROWS);
             if (st) return st;
         } else {
             tx_lo = tx_hi;
@@ -635,12 +635,12 @@ int launch_small_cfg(int64_t M, int64_t N, int64_t K, const SmallIn &in, const v
     }
 #endif
     cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = dim3(static_cast<unsigned>(panels * cs));
+    cfg.gridDim = dim3(static_cast<unsigned>(Cfg::PAIR ? (panels + 1) / 2 * 2 : panels * cs));
     cfg.blockDim = dim3(kSmallThreads);
     cfg.dynamicSmemBytes = smem;
     cfg.stream = stream;
     cudaLaunchAttribute attr[2];
-    cfg.numAttrs = fill_attrs(attr, static_cast<unsigned>(cs));
+    cfg.numAttrs = fill_attrs(attr, Cfg::PAIR ? 2u : static_cast<unsigned>(cs));
     cfg.attrs = attr;
     HEAL_CUDA(cudaLaunchKernelEx(&cfg, kern, tx_hi, tx_lo, tw_hi, tw_lo, args));
     g_launches.fetch_add(1);
@@ -658,6 +658,21 @@ int launch_small_np(int nprod, int64_t M, int64_t N, int64_t K, const SmallIn &i
         case 2: return launch_small_cfg<SmallCfg<MPAD, 2, B_MN, true>>(M, N, K, in, B_hi, B_lo, ldb, out, s, handled);
         }
         return HEAL_ERR_UNSUPPORTED_MODE;
+    }
+    // Large N (no K split) and more than 32 tokens: pairs of panels share one cta_group::2 MMA, so each CTA receives only
+    // half of the token tile (at MPAD = 64 it is as large as the weight tile, and the unpaired kernel runs into the
+    // L2 -> SM delivery cap).  Same bits.
+    if constexpr (MPAD == 64) {
+        static const bool no_pair = std::getenv("HEAL_NO_PAIR") != nullptr;      // debug only
+        const int64_t panels = (N + kSmallBNW - 1) / kSmallBNW;
+        if (!no_pair && panels * 5 >= 7 * g.num_sms) {
+            switch (nprod) {
+            case 1: return launch_small_cfg<SmallCfg<MPAD, 1, B_MN, false, true>>(M, N, K, in, B_hi, B_lo, ldb, out, s, handled);
+            case 2: return launch_small_cfg<SmallCfg<MPAD, 2, B_MN, false, true>>(M, N, K, in, B_hi, B_lo, ldb, out, s, handled);
+            case 3: return launch_small_cfg<SmallCfg<MPAD, 3, B_MN, false, true>>(M, N, K, in, B_hi, B_lo, ldb, out, s, handled);
+            case 4: return launch_small_cfg<SmallCfg<MPAD, 4, B_MN, false, true>>(M, N, K, in, B_hi, B_lo, ldb, out, s, handled);
+            }
+        }
     }
     switch (nprod) {
     case 1: return launch_small_cfg<SmallCfg<MPAD, 1, B_MN, false>>(M, N, K, in, B_hi, B_lo, ldb, out, s, handled);

@@ -24,6 +24,10 @@
 // Static weights (HEAL_B_STATIC): the producer starts streaming W before griddepcontrol.wait, i.e. while
 // the previous kernel on the stream is still in its tail; everything that touches activations or C waits.
 //
+// PAIR variant (M > 32, large N, one CTA per panel): two adjacent panels form a CTA pair under one cta_group::2 MMA
+// (UMMA M = 256), each CTA staging its own weight panel and HALF of the token tile; barriers as in heal_gemm_umma2.cuh
+// (full in the leader, empty / slot-full / done by multicast commit, slot-empty in the leader).
+//
 // Roles per CTA (192 threads): warp 0 TMA producer, warp 1 MMA issuer + TMEM allocator, warps 2-5
 // converter (FUSED) and epilogue (warp w owns TMEM lanes 32*(w%4)..+31).
 #pragma once
@@ -36,16 +40,21 @@ constexpr int kSmallThreads = 192;
 constexpr int kSmallBNW = 128;          // weight columns per panel (UMMA M)
 constexpr int kSmallMaxStages = 8;
 
-template <int MPAD_, int NPROD_, bool B_MN_, bool FUSED_>
+template <int MPAD_, int NPROD_, bool B_MN_, bool FUSED_, bool PAIR_ = false>
 struct SmallCfg {
     static constexpr int MPAD = MPAD_;                  // UMMA N: padded token count
     static constexpr int NPROD = NPROD_;
     static constexpr bool B_MN = B_MN_;                 // weights stored K x N (N contiguous)
     static constexpr bool FUSED = FUSED_;               // split the FP32 activations in the kernel
+    static constexpr bool PAIR = PAIR_;                 // large N, no K split, many tokens: two adjacent panels share one
+                                                        // cta_group::2 MMA and each CTA stages only HALF of the token tile
+                                                        // (at MPAD = 64 the token tile is as large as the weight tile and
+                                                        // the L2 -> SM delivery cap, not HBM, bounds the unpaired kernel)
+    static constexpr int XROWS = PAIR ? MPAD / 2 : MPAD;// token rows this CTA stages per k-tile
     static constexpr int A_PLANES = NPROD >= 2 ? 2 : 1; // activation planes
     static constexpr int B_PLANES = NPROD >= 3 ? 2 : 1; // weight planes
     static constexpr int W_TILE = kSmallBNW * kBK * 2;  // 16 KB
-    static constexpr int X_TILE = MPAD * kBK * 2;
+    static constexpr int X_TILE = XROWS * kBK * 2;
     static constexpr int X_TILE_AL = (X_TILE + 1023) / 1024 * 1024;
     static constexpr int STAGE_BYTES = B_PLANES * W_TILE + A_PLANES * X_TILE_AL;
     static constexpr int W_BYTES = B_PLANES * W_TILE;
@@ -55,6 +64,7 @@ struct SmallCfg {
     static constexpr int PF = MPAD <= 32 ? 4 : 2;       // FUSED: k-tiles of activations kept in flight in registers
     static_assert(MPAD % 16 == 0 && MPAD >= 16 && MPAD <= 64, "MPAD");
     static_assert(!FUSED || NPROD <= 2, "the fused split needs FP16 weights");
+    static_assert(!PAIR || (!FUSED && MPAD >= 32), "pairs: planes only, UMMA N >= 32 across the pair");
 };
 
 struct SmallArgs {
@@ -92,8 +102,11 @@ heal_gemm_smallm_kernel(const __grid_constant__ CUtensorMap tm_x_hi, const __gri
     // layout: [pipeline stages][partial sums pushed by the cluster][barriers]; with red_alias the partial sums
     // overlay the pipeline stages instead
     const int STAGES = args.stages;
-    const uint32_t cs = cluster_nctarank();
-    const uint32_t rank = cluster_ctarank();
+    constexpr bool PAIR = Cfg::PAIR;
+    // cluster = the CS ranks that split K of one panel, or (PAIR) the two panels of one cta_group::2 MMA
+    const uint32_t cs = PAIR ? 1u : cluster_nctarank();
+    const uint32_t rank = PAIR ? 0u : cluster_ctarank();
+    const uint32_t prank = PAIR ? cluster_ctarank() : 0u;          // 0 = leader of the pair
     const uint32_t pipe_bytes = static_cast<uint32_t>(STAGES) * Cfg::STAGE_BYTES;
     const uint32_t red_base = args.red_alias ? smem_base : smem_base + pipe_bytes;
     const uint32_t bar_base = args.red_alias ? smem_base + max(pipe_bytes, static_cast<uint32_t>(args.red_bytes))
@@ -111,7 +124,7 @@ heal_gemm_smallm_kernel(const __grid_constant__ CUtensorMap tm_x_hi, const __gri
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     if (threadIdx.x == 0) HEAL_STAMP(args.trace, 0);
-    const int panel = blockIdx.x / cs;
+    const int panel = PAIR ? static_cast<int>(blockIdx.x) : static_cast<int>(blockIdx.x / cs);
     const int n0 = panel * kSmallBNW;
     const int k_tiles = (args.K + kBK - 1) / kBK;
     const int n_local = (args.n_seg > static_cast<int>(rank)) ? (args.n_seg - 1 - static_cast<int>(rank)) / static_cast<int>(cs) + 1 : 0;
@@ -133,7 +146,7 @@ heal_gemm_smallm_kernel(const __grid_constant__ CUtensorMap tm_x_hi, const __gri
         tma_prefetch_desc(&tm_w_hi);
         if (Cfg::B_PLANES == 2) tma_prefetch_desc(&tm_w_lo);
         for (int s = 0; s < STAGES; ++s) {
-            mbar_init(full_bar(s), 1);
+            mbar_init(full_bar(s), PAIR ? 2 : 1);        // PAIR: lives in the leader, one arrive.expect_tx per producer
             mbar_init(empty_bar(s), 1);
             mbar_init(xfull_bar(s), 4);                  // one arrival per converter warp
         }
@@ -142,7 +155,7 @@ heal_gemm_smallm_kernel(const __grid_constant__ CUtensorMap tm_x_hi, const __gri
                                                          // else one arrival per epilogue warp of every rank
         for (int j = 0; j < ring; ++j) {
             mbar_init(tfull_bar(j), 1);
-            mbar_init(tempty_bar(j), 4);
+            mbar_init(tempty_bar(j), PAIR ? 8 : 4);      // PAIR: lives in the leader, 4 epilogue warps of each CTA
         }
         fence_mbar_init();
         if (cs > 1 && args.red_async && static_cast<int>(rank) < owners) {
@@ -155,8 +168,13 @@ heal_gemm_smallm_kernel(const __grid_constant__ CUtensorMap tm_x_hi, const __gri
         }
     }
     if (warp == 1) {
-        tmem_alloc(tmem_slot, static_cast<uint32_t>(args.tmem_cols));
-        tmem_relinquish();
+        if (PAIR) {
+            tmem_alloc_2cta(tmem_slot, static_cast<uint32_t>(args.tmem_cols));
+            tmem_relinquish_2cta();
+        } else {
+            tmem_alloc(tmem_slot, static_cast<uint32_t>(args.tmem_cols));
+            tmem_relinquish();
+        }
         if (lane == 0) HEAL_STAMP(args.trace, 13);
     }
     if (FUSED) {
@@ -171,6 +189,7 @@ heal_gemm_smallm_kernel(const __grid_constant__ CUtensorMap tm_x_hi, const __gri
     tc_fence_before();
     __syncthreads();
     if (threadIdx.x == 0) HEAL_STAMP(args.trace, 12);
+    if (PAIR) cluster_sync_all();                        // the peer's barriers exist before any remote arrive / commit
     if (cs > 1) cluster_arrive_relaxed();                // matched by cluster_wait() before the first remote access
                                                          // (the barrier inits were published by fence.mbarrier_init)
     tc_fence_after();
@@ -187,25 +206,39 @@ heal_gemm_smallm_kernel(const __grid_constant__ CUtensorMap tm_x_hi, const __gri
         // ================================ TMA producer ================================
         if (lane == 0) {
             const uint64_t pol_w = l2_policy_evict_first();      // weights are streamed once
+            // one TMA box; PAIR: the completion barrier is the leader's (cta_group::2 form of the copy)
+            auto ld_w = [&](uint32_t dst, const CUtensorMap *m, uint32_t fb, int x, int y) {
+                if (PAIR) tma_load_2d_2cta_hint(dst, m, fb, x, y, pol_w);
+                else      tma_load_2d_hint(dst, m, fb, x, y, pol_w);
+            };
+            auto ld_x = [&](uint32_t dst, const CUtensorMap *m, uint32_t fb, int x, int y) {
+                if (PAIR) tma_load_2d_2cta(dst, m, fb, x, y);
+                else      tma_load_2d(dst, m, fb, x, y);
+            };
+            auto expect = [&](uint32_t fb) {
+                if (PAIR) mbar_arrive_expect_tx_cluster(fb, Cfg::TX_BYTES);
+                else      mbar_arrive_expect_tx(fb, Cfg::TX_BYTES);
+            };
+            auto fbar = [&](int st) { return PAIR ? leader_addr(full_bar(st)) : full_bar(st); };
             auto load_w = [&](int t, uint32_t sb, uint32_t fb) {
                 const int k0 = ((static_cast<int>(rank) + (t >> 3) * static_cast<int>(cs)) * kTilesPerSeg + (t & 7)) * kBK;
                 if (Cfg::B_MN) {
 #pragma unroll
                     for (int c = 0; c < 2; ++c) {
-                        tma_load_2d_hint(sb + c * 8192, &tm_w_hi, fb, n0 + c * 64, k0, pol_w);
-                        if (Cfg::B_PLANES == 2)
-                            tma_load_2d_hint(sb + Cfg::W_TILE + c * 8192, &tm_w_lo, fb, n0 + c * 64, k0, pol_w);
+                        ld_w(sb + c * 8192, &tm_w_hi, fb, n0 + c * 64, k0);
+                        if (Cfg::B_PLANES == 2) ld_w(sb + Cfg::W_TILE + c * 8192, &tm_w_lo, fb, n0 + c * 64, k0);
                     }
                 } else {
-                    tma_load_2d_hint(sb, &tm_w_hi, fb, k0, n0, pol_w);
-                    if (Cfg::B_PLANES == 2) tma_load_2d_hint(sb + Cfg::W_TILE, &tm_w_lo, fb, k0, n0, pol_w);
+                    ld_w(sb, &tm_w_hi, fb, k0, n0);
+                    if (Cfg::B_PLANES == 2) ld_w(sb + Cfg::W_TILE, &tm_w_lo, fb, k0, n0);
                 }
             };
             auto load_x = [&](int t, uint32_t sb, uint32_t fb) {
                 const int k0 = ((static_cast<int>(rank) + (t >> 3) * static_cast<int>(cs)) * kTilesPerSeg + (t & 7)) * kBK;
                 const uint32_t sx = sb + Cfg::W_BYTES;
-                tma_load_2d(sx, &tm_x_hi, fb, k0, 0);
-                if (Cfg::A_PLANES == 2) tma_load_2d(sx + Cfg::X_TILE_AL, &tm_x_lo, fb, k0, 0);
+                const int m_first = static_cast<int>(prank) * Cfg::XROWS;          // PAIR: this CTA's half of the tokens
+                ld_x(sx, &tm_x_hi, fb, k0, m_first);
+                if (Cfg::A_PLANES == 2) ld_x(sx + Cfg::X_TILE_AL, &tm_x_lo, fb, k0, m_first);
             };
             int stage = 0, t = 0;
             uint32_t phase = 0;
@@ -214,20 +247,20 @@ heal_gemm_smallm_kernel(const __grid_constant__ CUtensorMap tm_x_hi, const __gri
                 // stream predecessor (which may have produced them) has completed
                 const int pre = min(STAGES, n_t);
                 for (int s = 0; s < pre; ++s) {
-                    mbar_arrive_expect_tx(full_bar(s), Cfg::TX_BYTES);
-                    load_w(s, smem_base + s * Cfg::STAGE_BYTES, full_bar(s));
+                    expect(fbar(s));
+                    load_w(s, smem_base + s * Cfg::STAGE_BYTES, fbar(s));
                 }
                 HEAL_STAMP(args.trace, 3);
                 pdl_wait();
-                for (int s = 0; s < pre; ++s) load_x(s, smem_base + s * Cfg::STAGE_BYTES, full_bar(s));
+                for (int s = 0; s < pre; ++s) load_x(s, smem_base + s * Cfg::STAGE_BYTES, fbar(s));
                 t = pre;
                 if (pre == STAGES) phase = 1u; else stage = pre;
             }
             for (; t < n_t; ++t) {
                 mbar_wait_ool(empty_bar(stage), phase ^ 1u, args.diag, 500 + stage);
                 const uint32_t sb = smem_base + stage * Cfg::STAGE_BYTES;
-                const uint32_t fb = full_bar(stage);
-                mbar_arrive_expect_tx(fb, Cfg::TX_BYTES);
+                const uint32_t fb = fbar(stage);
+                expect(fb);
                 load_w(t, sb, fb);
                 if (!FUSED) load_x(t, sb, fb);
                 if (t == 0) HEAL_STAMP(args.trace, 3);
@@ -242,9 +275,18 @@ heal_gemm_smallm_kernel(const __grid_constant__ CUtensorMap tm_x_hi, const __gri
         }
     } else if (warp == 1) {
         // ================================ MMA issuer ==================================
-        if (lane == 0) {
-            // D[n][m] = sum_k W[k][n] * X[m][k]: UMMA A = weights (128 rows), UMMA B = tokens (N = MPAD)
-            constexpr uint32_t idesc = umma_idesc_f16_f32(kSmallBNW, MPAD, Cfg::B_MN ? 1u : 0u, 0u);
+        if (lane == 0 && prank == 0) {
+            // D[n][m] = sum_k W[k][n] * X[m][k]: UMMA A = weights (128 rows per CTA), UMMA B = tokens (N = MPAD;
+            // PAIR: 256 weight rows over the two CTAs, each holding half of the token rows)
+            constexpr uint32_t idesc = umma_idesc_f16_f32(PAIR ? 2 * kSmallBNW : kSmallBNW, MPAD, Cfg::B_MN ? 1u : 0u, 0u);
+            auto mma = [&](uint32_t d, uint64_t a, uint64_t b, uint32_t acc) {
+                if (PAIR) umma_f16_2cta(d, a, b, idesc, acc);
+                else      umma_f16(d, a, b, idesc, acc);
+            };
+            auto commit = [&](uint32_t bar) {                  // PAIR: the barrier at this offset in both CTAs
+                if (PAIR) umma_commit_2cta(bar, 3);
+                else      umma_commit(bar);
+            };
             constexpr uint64_t kdesc0 = umma_smem_desc_sw128(0, 16, 1024);                 // K-major SW128
             constexpr uint64_t wdesc0 = Cfg::B_MN ? umma_smem_desc_sw128(0, kBK * 128, 1024) : kdesc0;
             constexpr uint32_t w_step = (Cfg::B_MN ? 16 * 128 : 32) >> 4;
@@ -278,20 +320,20 @@ heal_gemm_smallm_kernel(const __grid_constant__ CUtensorMap tm_x_hi, const __gri
                 for (int q = 0; q < kBK / 16; ++q) {
                     const uint64_t wo = static_cast<uint64_t>(q * w_step), xo = static_cast<uint64_t>(q * x_step);
                     // product order as in the large-M kernel: a_hi.b_hi, a_hi.b_lo, a_lo.b_hi, a_lo.b_lo
-                    umma_f16(d_tmem, w_hi + wo, x_hi + xo, idesc, accumulate);
+                    mma(d_tmem, w_hi + wo, x_hi + xo, accumulate);
                     accumulate = 1;
-                    if (NPROD == 2) umma_f16(d_tmem, w_hi + wo, x_lo + xo, idesc, 1);
+                    if (NPROD == 2) mma(d_tmem, w_hi + wo, x_lo + xo, 1);
                     if (NPROD >= 3) {
-                        umma_f16(d_tmem, w_lo + wo, x_hi + xo, idesc, 1);
-                        umma_f16(d_tmem, w_hi + wo, x_lo + xo, idesc, 1);
+                        mma(d_tmem, w_lo + wo, x_hi + xo, 1);
+                        mma(d_tmem, w_hi + wo, x_lo + xo, 1);
                     }
-                    if (NPROD == 4) umma_f16(d_tmem, w_lo + wo, x_lo + xo, idesc, 1);
+                    if (NPROD == 4) mma(d_tmem, w_lo + wo, x_lo + xo, 1);
                 }
-                umma_commit(empty_bar(stage));
-                if (ring && ((t & 7) == 7 || t == n_t - 1)) umma_commit(tfull_bar(slot));      // segment complete
+                commit(empty_bar(stage));
+                if (ring && ((t & 7) == 7 || t == n_t - 1)) commit(tfull_bar(slot));           // segment complete
                 if (++stage == STAGES) { stage = 0; phase ^= 1u; }
             }
-            umma_commit(done_bar);                         // all local segments complete in TMEM
+            commit(done_bar);                              // all local segments complete in TMEM
         }
         if (cs > 1 && args.red_alias) {
             __syncwarp();
@@ -397,7 +439,10 @@ heal_gemm_smallm_kernel(const __grid_constant__ CUtensorMap tm_x_hi, const __gri
                 }
                 tc_fence_before();
                 __syncwarp();
-                if (lane == 0) mbar_arrive(tempty_bar(slot));
+                if (lane == 0) {
+                    if (PAIR) mbar_arrive_cluster(leader_addr(tempty_bar(slot)));
+                    else      mbar_arrive(tempty_bar(slot));
+                }
             }
             if (et == 0) HEAL_STAMP(args.trace, 6);
             if (col < args.N) {
@@ -564,10 +609,12 @@ heal_gemm_smallm_kernel(const __grid_constant__ CUtensorMap tm_x_hi, const __gri
     }
 
     __syncthreads();
+    if (PAIR) cluster_sync_all();                          // the peer may still read this CTA's smem / signal its barriers
     if (threadIdx.x == 64) HEAL_STAMP(args.trace, 9);
     if (warp == 1) {
         tc_fence_after();
-        tmem_dealloc(tmem_base, static_cast<uint32_t>(args.tmem_cols));
+        if (PAIR) tmem_dealloc_2cta(tmem_base, static_cast<uint32_t>(args.tmem_cols));
+        else      tmem_dealloc(tmem_base, static_cast<uint32_t>(args.tmem_cols));
         if (lane == 0) HEAL_STAMP(args.trace, 11);
     }
 }

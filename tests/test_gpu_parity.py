@@ -459,7 +459,8 @@ def test_extended_epilogue_errors(hb):
                                               (64, 26624, 14336, 2, False), (64, 26624, 1536, 3, False), (20, 26624, 20480, 2, False)])
 def test_small_m_single_cta_panels_tmem_ring(hb, inputs, M, N, K, nprod, b_nk):
     """Large N (one CTA per 128-column panel, no K split): the segment partials cycle through a ring of TMEM slots and
-    the epilogue warps keep the ascending running sum in registers while the tensor core works on the next segment.
+    the epilogue warps keep the ascending running sum in registers while the tensor core works on the next segment;
+    above 32 tokens two panels share one cta_group::2 MMA (odd panel counts leave the last pair half empty).
     Same bits as rows 0..15 submitted alone (fused kernel, all segments resident) and as the large-M kernels."""
     A = dev(inputs.activations(M, K, seed=18, outliers=True))
     B = inputs.weights_f32(K, N, seed=18, nk=b_nk) if nprod >= 3 else inputs.weights_f16(K, N, seed=18, nk=b_nk)
