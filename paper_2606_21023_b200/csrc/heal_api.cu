@@ -554,7 +554,7 @@ int launch_small_cfg(int64_t M, int64_t N, int64_t K, const SmallIn &in, const v
     // Partial sums pushed by the cluster: a dedicated area when small (decode), else overlaid on the pipeline.
     static const size_t alias_min = std::getenv("HEAL_RED_ALIAS_MIN") ? static_cast<size_t>(std::atol(std::getenv("HEAL_RED_ALIAS_MIN"))) : 16 * 1024;   // debug only
     const bool red_alias = red > alias_min;
-    const size_t fixed = 1024 + (red_alias ? 0 : red) + Cfg::BAR_BYTES;
+    const size_t fixed = (red_alias ? 0 : red) + Cfg::BAR_BYTES;          // no alignment slack: see the kernel
     size_t budget = tmem_cols > 256 ? static_cast<size_t>(kSmemLimit)
                     : (Cfg::STAGE_BYTES <= 24 * 1024 && cs > 1 ? static_cast<size_t>(74 * 1024) : static_cast<size_t>(112 * 1024));
     if (budget < fixed + 3 * static_cast<size_t>(Cfg::STAGE_BYTES) && budget < static_cast<size_t>(112 * 1024)) budget = static_cast<size_t>(112 * 1024);
@@ -568,27 +568,8 @@ int launch_small_cfg(int64_t M, int64_t N, int64_t K, const SmallIn &in, const v
         const int want = std::atoi(e);
         if (want >= 2 && want <= kSmallMaxStages && fixed + static_cast<size_t>(want) * Cfg::STAGE_BYTES <= static_cast<size_t>(kSmemLimit)) stages = want;
     }
-    // Reduction transport (cs > 1): st.async while a thread sends few values; else, if a staging copy of the partials fits
-    // beside what the CTA already needs, bulk shared-memory copies; else plain remote stores.
-    const int vw_push = (rpr & 3) == 0 ? 4 : ((rpr & 1) == 0 ? 2 : 1);
-    const int64_t pushes = cs > 1 ? static_cast<int64_t>(max_local) * ((M + vw_push - 1) / vw_push) : 0;
-    static const bool no_async = std::getenv("HEAL_NO_ASYNC_PUSH") != nullptr;        // debug only
-    static const bool no_bulk = std::getenv("HEAL_NO_BULK_PUSH") != nullptr;          // debug only
-    const bool red_async = cs > 1 && async_push_ok(pushes, vw_push) && !no_async;
-    const size_t pipe = static_cast<size_t>(stages) * Cfg::STAGE_BYTES;
-    const size_t owners = cs > 1 ? static_cast<size_t>((M + rpr - 1) / rpr) : 0;
-    const size_t stg = owners * max_local * kSmallBNW * rpr * 4;
-    size_t region = red_alias ? (pipe > red ? pipe : red) : pipe;
-    bool red_bulk = false;
-    if (cs > 1 && !red_async && !no_bulk) {
-        const size_t need = red_alias ? stg + red : stg;
-        const size_t cap = (tmem_cols <= 256 ? static_cast<size_t>(112 * 1024) : static_cast<size_t>(kSmemLimit)) - fixed;
-        if (need <= (pipe > cap ? pipe : cap)) {
-            red_bulk = true;
-            if (need > region) region = need;
-        }
-    }
-    size_t smem = fixed + region;
+    size_t smem = fixed + static_cast<size_t>(stages) * Cfg::STAGE_BYTES;
+    if (red_alias && smem < fixed + red) smem = fixed + red;
     // more than half of TMEM: make sure only one CTA fits per SM (two could not both allocate)
     if (tmem_cols > 256 && smem < static_cast<size_t>(kSmemLimit) / 2 + 2048) smem = static_cast<size_t>(kSmemLimit) / 2 + 2048;
     auto kern = heal_gemm_smallm_kernel<Cfg>;
@@ -635,10 +616,13 @@ int launch_small_cfg(int64_t M, int64_t N, int64_t K, const SmallIn &in, const v
     args.rows_per_rank = rpr;
     args.red_bytes = static_cast<int>(red);
     args.red_alias = red_alias ? 1 : 0;
-    args.red_async = red_async ? 1 : 0;
-    args.red_bulk = red_bulk ? 1 : 0;
-    args.stg_bytes = red_bulk ? static_cast<int>(stg) : 0;
-    args.region_bytes = static_cast<int>(region);
+    {
+        // pushes per thread: few -> st.async (lowest latency), many -> plain remote stores + one fence/arrive per warp
+        const int vw = (rpr & 3) == 0 ? 4 : ((rpr & 1) == 0 ? 2 : 1);
+        const int64_t pushes = cs > 1 ? static_cast<int64_t>(max_local) * ((M + vw - 1) / vw) : 0;
+        static const bool no_async = std::getenv("HEAL_NO_ASYNC_PUSH") != nullptr;        // debug only
+        args.red_async = (cs > 1 && async_push_ok(pushes, vw) && !no_async) ? 1 : 0;
+    }
     args.ring = ring;
     static const bool no_static = std::getenv("HEAL_NO_STATIC") != nullptr;       // debug only
     args.b_static = (in.b_static && !no_static) ? 1 : 0;

@@ -12,8 +12,8 @@
 // j = s / CS lives in TMEM columns j*MPAD..).  Token rows are dealt to the ranks in contiguous blocks: every rank
 // PUSHES its segment partials of those rows straight from its TMEM registers into the owner's shared
 // memory -- with st.async when a thread has few values to send (the bytes are counted on the owner's
-// mbarrier: no fence, no arrive), else staged locally and sent with bulk shared-memory copies counted on
-// the same mbarrier, else with plain st.shared::cluster plus one fence and one relaxed remote arrive per warp; the owner adds the n_seg partials in ascending segment order and stores C.
+// mbarrier: no fence, no arrive), else with plain st.shared::cluster plus one fence and one relaxed
+// remote arrive per warp; the owner adds the n_seg partials in ascending segment order and stores C.
 // No atomics, no cluster-wide barrier after the main loop.
 //
 // FUSED variant (heal_gemm, B already FP16): step S runs inside the kernel -- the four epilogue warps
@@ -80,11 +80,6 @@ struct SmallArgs {
     int red_bytes;        // CS > 1: n_seg * rows_per_rank * 128 floats of partial sums pushed by the cluster
     int red_async;        // few pushes per thread: st.async (completion counted in bytes on the owner's mbarrier, no fence,
                           // no arrive); many: plain remote stores + one fence and arrive per warp (higher throughput)
-    int red_bulk;         // many values per thread and room for a staging copy: the partials are staged in this CTA's (dead)
-                          // pipeline buffers and sent with one bulk shared-memory copy per (owner, segment), counted on
-                          // the owner's mbarrier like the st.async pushes; a cluster barrier before exit keeps the source alive
-    int stg_bytes;        // size of that staging area (at the start of the pipeline region)
-    int region_bytes;     // pipeline region: max(stages, staging [+ aliased partial sums])
     int red_alias;        // the pushed partial sums reuse the pipeline stages (large M * K): needs a second cluster
                           // barrier ("every rank's main loop is over") before anybody pushes
     int ring;             // CS == 1, planes: number of TMEM slots the segments cycle through (0 = every local
@@ -102,8 +97,18 @@ heal_gemm_smallm_kernel(const __grid_constant__ CUtensorMap tm_x_hi, const __gri
 {
     constexpr int MPAD = Cfg::MPAD, NPROD = Cfg::NPROD;
     constexpr bool FUSED = Cfg::FUSED;
-    extern __shared__ uint8_t smem_raw[];
-    const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
+    // 128B-swizzled tiles need a 1024-byte aligned base.  The dynamic shared memory window of a kernel without static
+    // shared memory starts 1024-aligned; the host therefore reserves no slack (which keeps two of the largest CTAs on
+    // one SM: M = 64, K = 14336 decode 79 -> 51 us), and a launch that ever got a misaligned base fails loudly.
+    extern __shared__ __align__(1024) uint8_t smem_raw[];
+    const uint32_t smem_base = smem_u32(smem_raw);
+    if ((smem_base & 1023u) != 0u) {
+        if (threadIdx.x == 0 && args.diag) {
+            args.diag[0] = 900;
+            args.diag[1] = static_cast<int>(smem_base);
+        }
+        __trap();
+    }
     // layout: [pipeline stages][partial sums pushed by the cluster][barriers]; with red_alias the partial sums
     // overlay the pipeline stages instead
     const int STAGES = args.stages;
@@ -113,9 +118,9 @@ heal_gemm_smallm_kernel(const __grid_constant__ CUtensorMap tm_x_hi, const __gri
     const uint32_t rank = PAIR ? 0u : cluster_ctarank();
     const uint32_t prank = PAIR ? cluster_ctarank() : 0u;          // 0 = leader of the pair
     const uint32_t pipe_bytes = static_cast<uint32_t>(STAGES) * Cfg::STAGE_BYTES;
-    const uint32_t region = max(pipe_bytes, static_cast<uint32_t>(args.region_bytes));
-    const uint32_t red_base = args.red_alias ? smem_base + static_cast<uint32_t>(args.stg_bytes) : smem_base + region;
-    const uint32_t bar_base = args.red_alias ? smem_base + region : red_base + static_cast<uint32_t>(args.red_bytes);
+    const uint32_t red_base = args.red_alias ? smem_base : smem_base + pipe_bytes;
+    const uint32_t bar_base = args.red_alias ? smem_base + max(pipe_bytes, static_cast<uint32_t>(args.red_bytes))
+                                             : red_base + static_cast<uint32_t>(args.red_bytes);
     auto full_bar = [&](int s) { return bar_base + 8u * s; };
     auto empty_bar = [&](int s) { return bar_base + 64u + 8u * s; };
     auto xfull_bar = [&](int s) { return bar_base + 128u + 8u * s; };
@@ -156,17 +161,13 @@ heal_gemm_smallm_kernel(const __grid_constant__ CUtensorMap tm_x_hi, const __gri
             mbar_init(xfull_bar(s), 4);                  // one arrival per converter warp
         }
         mbar_init(done_bar, 1);
-        mbar_init(red_bar, (args.red_async || args.red_bulk) ? 1 : cs * 4);   // async / bulk: completes when every pushed
-                                                         // byte has landed; else one arrival per epilogue warp of every rank
+        mbar_init(red_bar, args.red_async ? 1 : cs * 4); // async: completes when every pushed byte has landed;
+                                                         // else one arrival per epilogue warp of every rank
         for (int j = 0; j < ring; ++j) {
             mbar_init(tfull_bar(j), 1);
             mbar_init(tempty_bar(j), PAIR ? 8 : 4);      // PAIR: lives in the leader, 4 epilogue warps of each CTA
         }
         fence_mbar_init();
-        if (cs > 1 && args.red_bulk && static_cast<int>(rank) < owners) {
-            // bulk: every rank sends one full block of rows_per_rank x 128 floats per segment
-            mbar_arrive_expect_tx(red_bar, static_cast<uint32_t>(args.n_seg) * kSmallBNW * static_cast<uint32_t>(args.rows_per_rank) * 4u);
-        }
         if (cs > 1 && args.red_async && static_cast<int>(rank) < owners) {
             // this rank finishes rows [rank * rpr, ...): every rank pushes, per segment and column, one vector per started
             // group of VW owned rows (VW = 4 / 2 / 1 by the divisibility of rpr)
@@ -519,19 +520,6 @@ heal_gemm_smallm_kernel(const __grid_constant__ CUtensorMap tm_x_hi, const __gri
                         tmem_ld_32x32b_x16(tmem_base + (static_cast<uint32_t>(quad * 32) << 16) + static_cast<uint32_t>(j * MPAD + c * 16), v);
                         tmem_ld_wait();
                         const bool async = args.red_async != 0;
-                        if (args.red_bulk) {
-                            // stage locally: block (owner d, slot j) = 128 x rpr floats, same layout as the owner's area
-                            uint32_t d = static_cast<uint32_t>((c * 16) / rpr), r = static_cast<uint32_t>((c * 16) % rpr);
-#pragma unroll
-                            for (int i = 0; i < 16; ++i) {
-                                const uint32_t a = smem_base + (((d * static_cast<uint32_t>(n_local) + static_cast<uint32_t>(j)) * kSmallBNW +
-                                                                 static_cast<uint32_t>(nl)) * static_cast<uint32_t>(rpr) + r) * 4u;
-                                if (c * 16 + i < static_cast<int>(owners) * rpr)
-                                    asm volatile("st.shared.b32 [%0], %1;" ::"r"(a), "r"(v[i]) : "memory");
-                                if (++r == static_cast<uint32_t>(rpr)) { r = 0; ++d; }
-                            }
-                            continue;
-                        }
                         // owner rank and row inside its block of the first token of this chunk, then stepped along
                         // (one division per chunk instead of one per element of the unrolled loops)
                         uint32_t dst = static_cast<uint32_t>((c * 16) / rpr), ml = static_cast<uint32_t>((c * 16) % rpr);
@@ -571,16 +559,7 @@ heal_gemm_smallm_kernel(const __grid_constant__ CUtensorMap tm_x_hi, const __gri
                 }
             }
             tc_fence_before();
-            if (args.red_bulk) {
-                fence_proxy_async_smem();                  // staged values -> visible to the bulk-copy engine
-                asm volatile("bar.sync 1, 128;" ::: "memory");
-                if (et < owners * n_local) {
-                    const uint32_t d = static_cast<uint32_t>(et / n_local), j = static_cast<uint32_t>(et % n_local);
-                    const uint32_t seg = rank + j * cs, blk = kSmallBNW * static_cast<uint32_t>(rpr) * 4u;
-                    bulk_copy_to_peer(map_to_cta(red_base + seg * blk, d), smem_base + (d * static_cast<uint32_t>(n_local) + j) * blk, blk,
-                                      map_to_cta(red_bar, d));
-                }
-            } else if (!args.red_async) {
+            if (!args.red_async) {
                 __syncwarp();
                 // one fence per signalling lane (cumulative over the warp's pushes, ordered by the __syncwarp) and a
                 // relaxed remote arrive: a cluster-scope release costs ~0.5 us each on this part (measured), so pay it once
@@ -592,7 +571,7 @@ heal_gemm_smallm_kernel(const __grid_constant__ CUtensorMap tm_x_hi, const __gri
             tc_fence_before();
             if (et == 0) HEAL_STAMP(args.trace, 7);
             if (static_cast<int>(rank) < owners) {
-                if (args.red_async || args.red_bulk) mbar_wait_ool(red_bar, 0, args.diag, 710);       // every byte has landed
+                if (args.red_async) mbar_wait_ool(red_bar, 0, args.diag, 710);       // every byte has landed
                 else                mbar_wait_cluster(red_bar, 0, args.diag, 710);
                 if (et == 0) HEAL_STAMP(args.trace, 8);
                 // this rank finishes rows [rank * rpr, min(M, (rank + 1) * rpr)): ascending segment order, FP32 RN
@@ -639,13 +618,6 @@ heal_gemm_smallm_kernel(const __grid_constant__ CUtensorMap tm_x_hi, const __gri
         }
     }
 
-    if (cs > 1 && args.red_bulk) {
-        // the bulk copies read this CTA's shared memory asynchronously: nobody leaves before every owner has received its
-        // bytes (owners get here after their red_bar wait).  Warps 0 and 1 still owe the wait of their last arrive.
-        if (warp < 2) cluster_wait();
-        cluster_arrive_relaxed();
-        cluster_wait();
-    }
     __syncthreads();
     if (PAIR) cluster_sync_all();                          // the peer may still read this CTA's smem / signal its barriers
     if (threadIdx.x == 64) HEAL_STAMP(args.trace, 9);
