@@ -784,3 +784,47 @@ def test_segment_order_is_fp32_rn_ascending(hb):
     assert torch.all(hb.heal_gemm(A, W, 2).cpu() == 2.0 ** 24)
     A[0, 1025] = 1.0          # s2 = 2: fl(2^24 + 2) is exact
     assert torch.all(hb.heal_gemm(A, W, 2).cpu() == 2.0 ** 24 + 2)
+
+
+def test_soak_random_shapes_streams_and_flags(hb):
+    """Short soak (a longer run of the same loop found two real bugs in round 1: hi/lo planes shared between streams,
+    and HEAL_B_STATIC prefetching weight planes the library itself had just written): random shapes of every kernel
+    family on three streams, random HEAL_B_STATIC / extended-epilogue use, every result compared bit for bit with the
+    large-M kernels' result for the same inputs."""
+    import random
+    import time
+    rnd = random.Random(1)
+    torch.manual_seed(1)
+    shapes = [(1, 4096, 4096, 2), (8, 4096, 4096, 2), (16, 1032, 8192, 2), (32, 4096, 4096, 2), (64, 4096, 4096, 2), (40, 520, 14336, 2),
+              (64, 32064, 4096, 2), (5, 26624, 2048, 2), (128, 4096, 4096, 2), (256, 1032, 4096, 2), (300, 520, 2056, 3), (700, 4104, 1032, 2),
+              (2048, 2048, 512, 2), (64, 256, 256, 3), (33, 264, 30000 // 8 * 8, 2)]
+    cases = []
+    try:
+        hb.debug_force_kernel(1)
+        for (M, N, K, nprod) in shapes:
+            A = torch.randn(M, K, device="cuda")
+            B = torch.randn(K, N, device="cuda") * 0.02
+            if nprod < 3:
+                B = B.half()
+            cases.append((A, B, nprod, hb.heal_gemm(A, B, nprod).clone()))
+    finally:
+        hb.debug_force_kernel(0)
+    streams = [torch.cuda.Stream() for _ in range(3)]
+    torch.cuda.synchronize()
+    t0, n = time.time(), 0
+    while time.time() - t0 < 8.0:
+        outs = []
+        for _ in range(12):
+            A, B, nprod, ref = rnd.choice(cases)
+            flag = rnd.choice([0, hb.B_STATIC])
+            with torch.cuda.stream(rnd.choice(streams)):
+                if rnd.random() < 0.3:
+                    C, _, _ = hb.heal_gemm_ex(A, B, nprod | flag, scale_exp=1)
+                    outs.append((C * 2.0, ref))
+                else:
+                    outs.append((hb.heal_gemm(A, B, nprod | flag), ref))
+        torch.cuda.synchronize()
+        for c, r in outs:
+            n += 1
+            assert torch.equal(c, r), (tuple(c.shape), n)
+    assert n > 100
