@@ -317,3 +317,45 @@ def test_metric_definition(oracle):
     C = np.array([[11.5]], np.float32)
     assert abs(oracle.normwise_error(C, Cref, A, B) - 0.5 / (5 * np.sqrt(5))) < 1e-15
     assert abs(oracle.normwise_error(C, Cref, A, B.astype(np.float16)) - 0.5 / (5 * np.sqrt(5))) < 1e-15
+
+
+def test_metric_rows_list_and_padded_operands_vs_numpy(oracle):
+    """The sampled-row form of the acceptance metric -- the one every full-size gate (configs[2], [3], [4], bench.py's
+    normwise_err_vs_fp64) goes through: a `rows` list in non-ascending order with a repeat, C inside a buffer with
+    ldc > N, FP16 B inside a buffer with ld > cols, FP32 A with lda > K.  Pinned against numpy.linalg.norm in float64
+    (an independent evaluation of e = ||C_S - Cref||_F / (||A_S||_F ||B||_F), BASELINE.json north_star); a dropped
+    row index, a row/column stride mix-up or padding leaking into a norm changes the value by far more than 1e-14."""
+    rng = np.random.default_rng(5)
+    M, N, K = 23, 24, 40
+    Abuf = rng.standard_normal((M, K + 4)).astype(np.float32)
+    A = Abuf[:, :K]
+    Bbuf = (rng.standard_normal((K, N + 8)) * 0.02).astype(np.float16)
+    Bbuf[:, N:] = np.float16(7.0)                               # padding must not enter ||B||_F
+    B = Bbuf[:, :N]
+    Cbuf = np.full((M, N + 5), 1e3, np.float32)                 # padding must not enter the difference
+    C = Cbuf[:, :N]
+    exact = A.astype(np.float64) @ B.astype(np.float64)
+    C[:] = (exact + 1e-3 * rng.standard_normal((M, N))).astype(np.float32)
+    rows = [17, 3, 22, 0, 9, 3, 11]
+    ref = oracle.gemm_f64(A, B, rows=rows)
+    assert np.allclose(ref, exact[rows], rtol=1e-13, atol=1e-13)
+    want = np.linalg.norm(C[rows].astype(np.float64) - exact[rows]) / (
+        np.linalg.norm(A[rows].astype(np.float64)) * np.linalg.norm(B.astype(np.float64)))
+    got = oracle.normwise_error(C, ref, A, B, rows=rows)
+    assert abs(got - want) <= 1e-14 * want, (got, want)
+    # the same through the FP32-B form (three-product configs) and with the full-matrix call
+    B32buf = rng.uniform(-1, 1, (K, N + 4)).astype(np.float32)
+    B32 = B32buf[:, :N]
+    ex32 = A.astype(np.float64) @ B32.astype(np.float64)
+    C[:] = (ex32 * (1 + 1e-5)).astype(np.float32)
+    want = np.linalg.norm(C[rows].astype(np.float64) - ex32[rows]) / (
+        np.linalg.norm(A[rows].astype(np.float64)) * np.linalg.norm(B32.astype(np.float64)))
+    got = oracle.normwise_error(C, oracle.gemm_f64(A, B32, rows=rows), A, B32, rows=rows)
+    assert abs(got - want) <= 1e-14 * want, (got, want)
+    want = np.linalg.norm(C.astype(np.float64) - ex32) / (np.linalg.norm(A.astype(np.float64)) * np.linalg.norm(B32.astype(np.float64)))
+    got = oracle.normwise_error(C, oracle.gemm_f64(A, B32), A, B32)
+    assert abs(got - want) <= 1e-14 * want, (got, want)
+    # the raw C routines on strided data
+    L = oracle.lib()
+    assert abs(L.oracle_sumsq_f16(K, N, Bbuf.ctypes.data, N + 8) - float((B.astype(np.float64) ** 2).sum())) <= 1e-14 * float((B.astype(np.float64) ** 2).sum())
+    assert abs(L.oracle_sumsq_f32(M, K, Abuf.ctypes.data, K + 4) - float((A.astype(np.float64) ** 2).sum())) <= 1e-13 * float((A.astype(np.float64) ** 2).sum())
