@@ -9,9 +9,12 @@
 #include <cuda_runtime.h>
 
 #include <atomic>
+#include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <deque>
 #include <mutex>
+#include <vector>
 
 #include "heal_gemm_smallm.cuh"
 #include "heal_gemm_umma.cuh"
@@ -34,20 +37,23 @@ struct State {
     int device = -1;
     int num_sms = 0;
     int *diag = nullptr;
-    // hand-off buffers of the balanced schedule, one set per stream (concurrent streams must not share them)
+    // Per-stream resources: hand-off buffers of the balanced schedule, hi/lo plane workspace, split-K partial area (concurrent
+    // streams must not share them).  A slot that was ever used while its stream was being captured is PINNED: its buffers may
+    // be baked into a CUDA graph, so they are never freed, shrunk, moved or handed to another stream (see acquire_slot).
     struct Xfer {
         cudaStream_t stream = nullptr;
         bool used = false;
+        bool pinned = false;       // used during stream capture at least once
         float *xfer = nullptr;     // per-CTA running-sum slots (128 x 256 floats each)
         uint32_t *flags = nullptr; // per-CTA flag: 1 = slot written, reset by the consumer
-        uint64_t last_use = 0;     // for recycling the least recently used slot when all 8 are taken
+        uint64_t last_use = 0;     // for recycling the least recently used un-pinned slot
         void *ws = nullptr;        // library-owned hi/lo plane workspace of this stream, grown on demand
         size_t ws_bytes = 0;
         float *part = nullptr;     // ordered split-K: segment partials, grown on demand (never while capturing)
         size_t part_bytes = 0;
-        uint32_t *cnt = nullptr;   // ordered split-K: two counters per (tile, rank), all zero between launches
     };
-    Xfer xf[8];
+    std::deque<Xfer> xf;           // grows when every slot is pinned or busy; addresses of elements stay valid
+    std::vector<void *> retired;   // buffers replaced while their slot was pinned: kept alive for the graphs that hold them
     // workspace
     void *user_ws = nullptr;
     size_t user_ws_bytes = 0;
@@ -110,21 +116,69 @@ inline int64_t round_up(int64_t x, int64_t m) { return (x + m - 1) / m * m; }
 
 // 2-D FP16 tensor map, 128-byte swizzle, out-of-bounds elements read as zero (K/M/N tails).
 //   inner/outer: extents in elements; ld: row pitch in elements; box: {inner, outer} elements.
-int encode_f16_2d(CUtensorMap *tm, const void *base, int64_t inner, int64_t outer, int64_t ld, uint32_t box_inner,
-                  uint32_t box_outer)
+// Encoded maps are cached (direct-mapped, keyed on everything that enters the encoding): an inference loop calls with
+// the same few (pointer, shape) combinations over and over, and four driver encodes per launch are a measurable part
+// of the host-side cost of a 9 us decode GEMM.  A map holds only the address and geometry, never data, so a stale
+// entry for a freed-and-reused pointer is still a correct encoding of the same arguments.
+struct MapKey {
+    const void *base;
+    int64_t inner, outer, ld;
+    uint32_t box_inner, box_outer, kind;
+    bool operator==(const MapKey &o) const
+    {
+        return base == o.base && inner == o.inner && outer == o.outer && ld == o.ld && box_inner == o.box_inner &&
+               box_outer == o.box_outer && kind == o.kind;
+    }
+};
+struct MapEntry {
+    MapKey key;
+    bool valid = false;
+    CUtensorMap map;
+};
+constexpr int kMapCache = 256;
+MapEntry g_maps[kMapCache];
+std::mutex g_map_mu;
+
+// kind 0: FP16, 128-byte swizzle (MMA operand tiles); kind 1: FP32, no swizzle (activation tiles the kernel converts itself)
+int encode_2d(CUtensorMap *tm, const void *base, int64_t inner, int64_t outer, int64_t ld, uint32_t box_inner,
+              uint32_t box_outer, uint32_t kind)
 {
+    const MapKey key{base, inner, outer, ld, box_inner, box_outer, kind};
+    uint64_t h = reinterpret_cast<uintptr_t>(base) >> 4;
+    h = (h ^ static_cast<uint64_t>(inner) * 0x9E3779B97F4A7C15ull) + static_cast<uint64_t>(outer) * 0xC2B2AE3D27D4EB4Full;
+    h ^= static_cast<uint64_t>(ld) * 0x165667B19E3779F9ull + box_inner * 131u + box_outer * 31u + kind;
+    h ^= h >> 29;
+    MapEntry &e = g_maps[h % kMapCache];
+    {
+        std::lock_guard<std::mutex> lk(g_map_mu);
+        if (e.valid && e.key == key) {
+            *tm = e.map;
+            return HEAL_OK;
+        }
+    }
+    const size_t es = kind == 1 ? 4 : 2;
     cuuint64_t dims[2] = {static_cast<cuuint64_t>(inner), static_cast<cuuint64_t>(outer)};
-    cuuint64_t strides[1] = {static_cast<cuuint64_t>(ld) * 2};
+    cuuint64_t strides[1] = {static_cast<cuuint64_t>(ld) * es};
     cuuint32_t box[2] = {box_inner, box_outer};
     cuuint32_t estr[2] = {1, 1};
-    CUresult r = g.encode(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 2, const_cast<void *>(base), dims, strides, box, estr,
-                          CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
-                          CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    CUresult r = g.encode(tm, kind == 1 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 2,
+                          const_cast<void *>(base), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                          kind == 1 ? CU_TENSOR_MAP_SWIZZLE_NONE : CU_TENSOR_MAP_SWIZZLE_128B,
+                          CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) {
         g_last_cuda_error.store(static_cast<int>(cudaErrorInvalidValue));
         return HEAL_ERR_CUDA;
     }
+    std::lock_guard<std::mutex> lk(g_map_mu);
+    e.key = key;
+    e.map = *tm;
+    e.valid = true;
     return HEAL_OK;
+}
+inline int encode_f16_2d(CUtensorMap *tm, const void *base, int64_t inner, int64_t outer, int64_t ld, uint32_t box_inner,
+                         uint32_t box_outer)
+{
+    return encode_2d(tm, base, inner, outer, ld, box_inner, box_outer, 0);
 }
 
 }  // namespace
@@ -134,7 +188,7 @@ namespace {
 // Launch attributes: optional cluster dimension + programmatic stream serialization (PDL), which lets the
 // kernel's prologue (barrier init, TMEM allocation, descriptor prefetch) overlap the previous kernel's tail;
 // every kernel calls griddepcontrol.wait before its first global-memory access.
-int fill_attrs(cudaLaunchAttribute *attr, unsigned cluster_x)
+int fill_attrs(cudaLaunchAttribute *attr, unsigned cluster_x, int cooperative = 0)
 {
     static const bool no_pdl = std::getenv("HEAL_NO_PDL") != nullptr;          // debug only
     int n = 0;
@@ -145,7 +199,12 @@ int fill_attrs(cudaLaunchAttribute *attr, unsigned cluster_x)
         attr[n].val.clusterDim.z = 1;
         ++n;
     }
-    if (!no_pdl) {
+    if (cooperative) {                   // all CTAs co-resident or the launch waits: see epi_take_prefix
+        attr[n].id = cudaLaunchAttributeCooperative;
+        attr[n].val.cooperative = 1;
+        ++n;
+    }
+    if (!no_pdl && cooperative != 1) {
         attr[n].id = cudaLaunchAttributeProgrammaticStreamSerialization;
         attr[n].val.programmaticStreamSerializationAllowed = 1;
         ++n;
@@ -166,7 +225,7 @@ int launch_split(int64_t rows, int64_t cols, const float *X, int64_t ldx, __half
     cfg.gridDim = dim3(static_cast<unsigned>(blocks));
     cfg.blockDim = dim3(256);
     cfg.stream = stream;
-    cudaLaunchAttribute attr[2];
+    cudaLaunchAttribute attr[3];
     cfg.numAttrs = fill_attrs(attr, 1);
     cfg.attrs = attr;
     const float lo_scale = static_cast<float>(1u << lo_shift);                   // 2^s, s in [0, 16]
@@ -175,11 +234,13 @@ int launch_split(int64_t rows, int64_t cols, const float *X, int64_t ldx, __half
     return HEAL_OK;
 }
 
-// Per-stream resources (hi/lo plane workspace, balanced-schedule hand-off buffers, split-K partial area): 8 slots, one
-// per stream that has called into the library, so calls on different streams never share scratch memory.  The least
-// recently used slot is recycled (after a device synchronise; it keeps its buffers) when a ninth stream shows up.
-// During stream capture nothing is allocated: what a captured call needs must exist from an earlier eager call on the
-// same stream (else: unbalanced schedule for the GEMM, HEAL_ERR_WORKSPACE for the planes).  Call with g_xf_mu held.
+// Per-stream resources (hi/lo plane workspace, balanced-schedule hand-off buffers, split-K partial area): one slot per
+// stream that has called into the library, so calls on different streams never share scratch memory.  Up to 8 slots are
+// kept for streams that were never captured: when a ninth such stream shows up the least recently used un-pinned slot is
+// recycled (after a device synchronise; it keeps its buffers).  Pinned slots (used under stream capture: their buffers
+// may live on in graphs) are never recycled; the deque simply grows.  During stream capture nothing is allocated: what a
+// captured call needs must exist from an earlier eager call on the same stream (else: unbalanced schedule for the GEMM,
+// HEAL_ERR_WORKSPACE for the planes).  Call with g_xf_mu held.
 State::Xfer *acquire_slot(cudaStream_t stream, bool capturing)
 {
     static uint64_t tick = 0;
@@ -189,18 +250,46 @@ State::Xfer *acquire_slot(cudaStream_t stream, bool capturing)
     if (!slot && !capturing) {
         for (auto &x : g.xf)
             if (!x.used) { slot = &x; break; }
-        if (!slot && cudaDeviceSynchronize() == cudaSuccess) {
-            slot = &g.xf[0];
-            for (auto &x : g.xf)
-                if (x.last_use < slot->last_use) slot = &x;
+        if (!slot) {
+            int unpinned = 0;
+            for (auto &x : g.xf) unpinned += x.pinned ? 0 : 1;
+            if (unpinned >= 8 && cudaDeviceSynchronize() == cudaSuccess) {
+                for (auto &x : g.xf)
+                    if (!x.pinned && (!slot || x.last_use < slot->last_use)) slot = &x;
+            }
+            if (!slot) {
+                g.xf.emplace_back();
+                slot = &g.xf.back();
+            }
         }
-        if (slot) {
-            slot->stream = stream;
-            slot->used = true;
+        slot->stream = stream;
+        slot->used = true;
+    }
+    if (slot) {
+        slot->last_use = ++tick;
+        if (capturing) slot->pinned = true;
+    }
+    return slot;
+}
+
+// Replace a slot buffer by a larger one.  An un-pinned slot: wait for the stream (earlier calls may still use the old
+// buffer) and free it.  A pinned slot: a captured graph may replay the old address at any time, so it stays allocated for
+// the life of the process (g.retired) and only new calls use the new one.
+int grow_buffer(State::Xfer *slot, cudaStream_t stream, void **buf, size_t *have, size_t want)
+{
+    if (*buf) {
+        if (slot->pinned) {
+            g.retired.push_back(*buf);
+        } else {
+            HEAL_CUDA(cudaStreamSynchronize(stream));
+            HEAL_CUDA(cudaFree(*buf));
         }
     }
-    if (slot) slot->last_use = ++tick;
-    return slot;
+    *buf = nullptr;
+    *have = 0;
+    HEAL_CUDA(cudaMalloc(buf, want));
+    *have = want;
+    return HEAL_OK;
 }
 
 bool stream_capturing(cudaStream_t stream)
@@ -215,37 +304,30 @@ bool bind_xfer(GemmArgs &args, cudaStream_t stream, size_t part_bytes = 0)
     const bool capturing = stream_capturing(stream);
     State::Xfer *slot = acquire_slot(stream, capturing);
     if (!slot) return false;
-    if (!slot->xfer) {                                   // 19 MB of hand-off slots + flags + split-K counters, first use only
+    if (!slot->xfer) {                                   // 19 MB of hand-off slots + flags, first use only
         if (capturing) return false;
         float *xf = nullptr;
-        uint32_t *fl = nullptr, *cn = nullptr;
-        const size_t cnt_bytes = static_cast<size_t>(g.num_sms) * 4 * sizeof(uint32_t);
+        uint32_t *fl = nullptr;
         if (cudaMalloc(&xf, static_cast<size_t>(g.num_sms) * kBM * 256 * sizeof(float)) != cudaSuccess) return false;
         if (cudaMalloc(&fl, static_cast<size_t>(g.num_sms) * sizeof(uint32_t)) != cudaSuccess ||
-            cudaMemset(fl, 0, static_cast<size_t>(g.num_sms) * sizeof(uint32_t)) != cudaSuccess ||
-            cudaMalloc(&cn, cnt_bytes) != cudaSuccess || cudaMemset(cn, 0, cnt_bytes) != cudaSuccess) {
+            cudaMemset(fl, 0, static_cast<size_t>(g.num_sms) * sizeof(uint32_t)) != cudaSuccess) {
             cudaFree(xf);
             if (fl) cudaFree(fl);
-            if (cn) cudaFree(cn);
             return false;
         }
         slot->xfer = xf;
         slot->flags = fl;
-        slot->cnt = cn;
     }
     if (part_bytes > slot->part_bytes) {
-        // grow the partial-sum area: the stream may still be using the old one, so wait for it first
-        if (capturing || cudaStreamSynchronize(stream) != cudaSuccess) return false;
-        if (slot->part) cudaFree(slot->part);
-        slot->part = nullptr;
-        slot->part_bytes = 0;
-        if (cudaMalloc(&slot->part, part_bytes) != cudaSuccess) return false;
-        slot->part_bytes = part_bytes;
+        if (capturing) return false;
+        void *p = slot->part;
+        const int st = grow_buffer(slot, stream, &p, &slot->part_bytes, part_bytes);
+        slot->part = static_cast<float *>(p);
+        if (st) return false;
     }
     args.xfer = slot->xfer;
     args.flags = slot->flags;
     args.part = slot->part;
-    args.cnt = slot->cnt;
     return true;
 }
 
@@ -255,13 +337,30 @@ bool bind_xfer(GemmArgs &args, cudaStream_t stream, size_t part_bytes = 0)
 //    alone would leave less than half a tile per CTA) is cut at K-segment granularity.
 //  * tiles < G_max (mid-size M, small N): ordered split-K, see below.
 // the ordered split-K rule of set_balance(), without side effects: decides which kernel instantiation to launch
+// Ordered split-K pays while a CTA gets few units: a parked unit costs about `a/b` plain segments more than a unit of a
+// whole tile (its partial travels to L2 and back through the reduce kernel), whole tiles cost n_seg segments per CTA.
+// HEAL_SK_RULE="a,b" overrides the measured default (debug / tuning).
+bool sk_rule(int64_t units_per_cta, int64_t n_seg)
+{
+    static int a = 12, b = 5;
+    static const bool init = [] {
+        if (const char *e = std::getenv("HEAL_SK_RULE")) {
+            int x = 0, y = 0;
+            if (std::sscanf(e, "%d,%d", &x, &y) == 2 && x > 0 && y > 0) { a = x; b = y; }
+        }
+        return true;
+    }();
+    (void)init;
+    return a * units_per_cta < b * n_seg;
+}
+
 bool wants_split_k(int64_t tiles, int64_t n_seg, int64_t G_max, int ctas_per_tile, int bn)
 {
     if (tiles >= G_max || n_seg <= 1 || std::getenv("HEAL_NO_BALANCE")) return false;
     const int64_t units = tiles * n_seg;
     const int64_t G = units < G_max ? units : G_max;
     const size_t part_bytes = static_cast<size_t>(units) * ctas_per_tile * kBM * bn * sizeof(float);
-    return G > tiles && 12 * ((units + G - 1) / G) < 5 * n_seg && part_bytes <= (static_cast<size_t>(128) << 20);
+    return G > tiles && sk_rule((units + G - 1) / G, n_seg) && part_bytes <= (static_cast<size_t>(128) << 20);
 }
 
 int64_t set_balance(GemmArgs &args, int64_t tiles, int64_t n_seg, int64_t G_max, int ctas_per_tile, int bn, bool full_kernel,
@@ -270,7 +369,6 @@ int64_t set_balance(GemmArgs &args, int64_t tiles, int64_t n_seg, int64_t G_max,
     args.xfer = nullptr;
     args.flags = nullptr;
     args.part = nullptr;
-    args.cnt = nullptr;
     args.sk = 0;
     static const bool no_balance = std::getenv("HEAL_NO_BALANCE") != nullptr;      // debug only
     args.balance = 0;
@@ -284,7 +382,7 @@ int64_t set_balance(GemmArgs &args, int64_t tiles, int64_t n_seg, int64_t G_max,
         // Worth it only while a CTA gets few units: parking and re-reading a partial costs about 1.4 segments of
         // L2 traffic (measured: a parked unit takes 2.4x a plain segment), whole tiles cost n_seg segments.
         const int64_t units_per_cta = (units + G - 1) / G;
-        if (full_kernel && !no_balance && n_seg > 1 && G > tiles && 12 * units_per_cta < 5 * n_seg &&
+        if (full_kernel && !no_balance && n_seg > 1 && G > tiles && sk_rule(units_per_cta, n_seg) &&
             part_bytes <= (static_cast<size_t>(128) << 20) && bind_xfer(args, stream, part_bytes)) {
             args.balance = 1;
             args.sk = 1;
@@ -303,6 +401,40 @@ int64_t set_balance(GemmArgs &args, int64_t tiles, int64_t n_seg, int64_t G_max,
         }
     }
     return G_max;
+}
+
+// Balanced-schedule launches spin on a flag written by a lower-indexed CTA (epi_take_prefix).  0 = plain launch (relies on
+// in-order block dispatch), 1 = cooperative launch instead of PDL, 2 = cooperative + PDL.  HEAL_COOP overrides (debug).
+int coop_mode()
+{
+    static const int mode = [] {
+        const char *e = std::getenv("HEAL_COOP");
+        return e ? std::atoi(e) : 0;
+    }();
+    return mode;
+}
+
+// second half of the ordered split-K schedule: ascending-segment FP32 RN sums of the parked partials + step E
+template <int BN>
+int launch_sk_reduce(const GemmArgs &args, int ctas_per_tile, int64_t tiles, cudaStream_t stream)
+{
+    const int n_seg = (args.K + kKSeg - 1) / kKSeg;
+    const int64_t units = tiles * ctas_per_tile;
+    constexpr int NC = BN / 8;                                    // float4 chunks per thread
+    int64_t shares = (2 * static_cast<int64_t>(g.num_sms) + units - 1) / units;     // about two waves of 256-thread CTAs
+    if (shares > NC) shares = NC;
+    if (shares < 1) shares = 1;
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(static_cast<unsigned>(units * shares));
+    cfg.blockDim = dim3(256);
+    cfg.stream = stream;
+    cudaLaunchAttribute attr[3];
+    cfg.numAttrs = fill_attrs(attr, 1);
+    cfg.attrs = attr;
+    HEAL_CUDA(cudaLaunchKernelEx(&cfg, heal_splitk_reduce_kernel<BN>, static_cast<const float *>(args.part), n_seg, ctas_per_tile,
+                                 args.tiles_m, static_cast<int>(shares), args.out, args.M, args.N));
+    g_launches.fetch_add(1);
+    return HEAL_OK;
 }
 
 // ---- steps G + E launch -----------------------------------------------------------------------
@@ -350,11 +482,12 @@ int launch_gemm_cfg(int64_t M, int64_t N, int64_t K, const void *A_hi, const voi
     cfg.blockDim = dim3(kGemmThreads);
     cfg.dynamicSmemBytes = Cfg::SMEM_BYTES;
     cfg.stream = stream;
-    cudaLaunchAttribute attr[2];
-    cfg.numAttrs = fill_attrs(attr, 1);
+    cudaLaunchAttribute attr[3];
+    cfg.numAttrs = fill_attrs(attr, 1, (args.balance && !args.sk) ? coop_mode() : 0);
     cfg.attrs = attr;
     HEAL_CUDA(cudaLaunchKernelEx(&cfg, kern, ta_hi, ta_lo, tb_hi, tb_lo, args));
     g_launches.fetch_add(1);
+    if (args.sk) return launch_sk_reduce<Cfg::BN>(args, 1, tiles, stream);
     return HEAL_OK;
 }
 
@@ -403,11 +536,12 @@ int launch_gemm2_cfg(int64_t M, int64_t N, int64_t K, const void *A_hi, const vo
     cfg.blockDim = dim3(kGemmThreads);
     cfg.dynamicSmemBytes = Cfg::SMEM_BYTES;
     cfg.stream = stream;
-    cudaLaunchAttribute attr[2];
-    cfg.numAttrs = fill_attrs(attr, 2);
+    cudaLaunchAttribute attr[3];
+    cfg.numAttrs = fill_attrs(attr, 2, (args.balance && !args.sk) ? coop_mode() : 0);
     cfg.attrs = attr;
     HEAL_CUDA(cudaLaunchKernelEx(&cfg, kern, ta_hi, ta_lo, tb_hi, tb_lo, args));
     g_launches.fetch_add(1);
+    if (args.sk) return launch_sk_reduce<Cfg::BN>(args, 2, tiles, stream);
     return HEAL_OK;
 }
 
@@ -431,7 +565,7 @@ int launch_gemm2_np(int nprod, int64_t M, int64_t N, int64_t K, const void *A_hi
     case 1: return launch_gemm2_cfg<Gemm2Cfg<256, 1, B_MN>>(M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, out, s);
     case 2: return launch_gemm2_cfg<Gemm2Cfg<256, 2, B_MN>>(M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, out, s);
     case 3: return launch_gemm2_cfg<Gemm2Cfg<256, 3, B_MN>>(M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, out, s);
-    case 4: return launch_gemm2_cfg<Gemm2Cfg<256, 4, B_MN>>(M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, out, s);
+    case 4: return launch_gemm2_cfg<Gemm2Cfg<256, 4, B_MN, true>>(M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, out, s);   // diagnostic mode: one instantiation
     }
     return HEAL_ERR_UNSUPPORTED_MODE;
 }
@@ -454,7 +588,7 @@ int launch_gemm_np(int nprod, int64_t M, int64_t N, int64_t K, const void *A_hi,
     case 1: return launch_gemm_cfg<GemmCfg<BN, 1, B_MN>>(M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, out, s);
     case 2: return launch_gemm_cfg<GemmCfg<BN, 2, B_MN>>(M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, out, s);
     case 3: return launch_gemm_cfg<GemmCfg<BN, 3, B_MN>>(M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, out, s);
-    case 4: return launch_gemm_cfg<GemmCfg<BN, 4, B_MN>>(M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, out, s);
+    case 4: return launch_gemm_cfg<GemmCfg<BN, 4, B_MN, true>>(M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, out, s);      // diagnostic mode: one instantiation
     }
     return HEAL_ERR_UNSUPPORTED_MODE;
 }
@@ -570,8 +704,16 @@ int launch_small_cfg(int64_t M, int64_t N, int64_t K, const SmallIn &in, const v
     }
     size_t smem = fixed + static_cast<size_t>(stages) * Cfg::STAGE_BYTES;
     if (red_alias && smem < fixed + red) smem = fixed + red;
-    // more than half of TMEM: make sure only one CTA fits per SM (two could not both allocate)
-    if (tmem_cols > 256 && smem < static_cast<size_t>(kSmemLimit) / 2 + 2048) smem = static_cast<size_t>(kSmemLimit) / 2 + 2048;
+    // TMEM must never be oversubscribed by the CTAs an SM can hold: a CTA blocked in tcgen05.alloc has not yet arrived at
+    // its cluster barrier, its peers hold TMEM elsewhere while they wait for it, and a cycle of such waits across clusters
+    // (or across kernels on concurrent streams) would hang.  Every kernel of the library therefore takes at least the
+    // same fraction of an SM's shared memory (228 KB, 1 KB reserved per CTA) as of its 512 TMEM columns, so whatever mix
+    // of the library's CTAs fits into an SM's shared memory also fits into its TMEM.
+    {
+        const size_t need = (static_cast<size_t>(tmem_cols) * (228 * 1024) + 511) / 512;
+        if (smem + 1024 < need) smem = need - 1024;
+        if (smem > static_cast<size_t>(kSmemLimit)) smem = static_cast<size_t>(kSmemLimit);
+    }
     auto kern = heal_gemm_smallm_kernel<Cfg>;
     static std::atomic<size_t> attr_smem{0};           // only ever raised: a concurrent smaller request cannot lower it
     if (smem > attr_smem.load(std::memory_order_acquire)) {
@@ -639,7 +781,7 @@ int launch_small_cfg(int64_t M, int64_t N, int64_t K, const SmallIn &in, const v
     cfg.blockDim = dim3(kSmallThreads);
     cfg.dynamicSmemBytes = smem;
     cfg.stream = stream;
-    cudaLaunchAttribute attr[2];
+    cudaLaunchAttribute attr[3];
     cfg.numAttrs = fill_attrs(attr, Cfg::PAIR ? 2u : static_cast<unsigned>(cs));
     cfg.attrs = attr;
     HEAL_CUDA(cudaLaunchKernelEx(&cfg, kern, tx_hi, tx_lo, tw_hi, tw_lo, args));
@@ -782,10 +924,13 @@ WsPlan plan_ws(int64_t M, int64_t N, int64_t K, int nprod, bool b_nk)
 
 int get_ws(size_t bytes, cudaStream_t stream, void **out)
 {
-    if (g.user_ws) {                                     // caller-owned: shared by all streams, the caller serialises
-        if (bytes > g.user_ws_bytes) return HEAL_ERR_WORKSPACE;
-        *out = g.user_ws;
-        return HEAL_OK;
+    {
+        std::lock_guard<std::mutex> lk(g_mu);            // (held for this lookup only, never across a launch)
+        if (g.user_ws) {                                 // caller-owned: shared by all streams, the caller serialises
+            if (bytes > g.user_ws_bytes) return HEAL_ERR_WORKSPACE;
+            *out = g.user_ws;
+            return HEAL_OK;
+        }
     }
     std::lock_guard<std::mutex> lk(g_xf_mu);
     const bool capturing = stream_capturing(stream);
@@ -793,12 +938,8 @@ int get_ws(size_t bytes, cudaStream_t stream, void **out)
     if (!slot) return HEAL_ERR_WORKSPACE;                // capturing on a stream the library has never seen
     if (bytes > slot->ws_bytes) {
         if (capturing) return HEAL_ERR_WORKSPACE;        // run the call once eagerly, or supply a workspace
-        HEAL_CUDA(cudaStreamSynchronize(stream));        // earlier calls on this stream may still read the old planes
-        if (slot->ws) HEAL_CUDA(cudaFree(slot->ws));
-        slot->ws = nullptr;
-        slot->ws_bytes = 0;
-        HEAL_CUDA(cudaMalloc(&slot->ws, bytes));
-        slot->ws_bytes = bytes;
+        const int st = grow_buffer(slot, stream, &slot->ws, &slot->ws_bytes, bytes);
+        if (st) return st;
     }
     *out = slot->ws;
     return HEAL_OK;
@@ -1005,7 +1146,6 @@ int heal_gemm_ex(int64_t M, int64_t N, int64_t K, const void *A, int64_t lda, co
         if (st || handled) return st;
     }
 
-    std::lock_guard<std::mutex> lk(g_mu);
     const WsPlan p = plan_ws(M, N, K, nprod, b_nk);
     void *ws = nullptr;
     st = get_ws(p.total, stream, &ws);
@@ -1061,10 +1201,24 @@ int heal_gemm_host(int64_t M, int64_t N, int64_t K, const void *A_host, int64_t 
     const size_t a_bytes = static_cast<size_t>(round_up(M * dlda * 4, 256));
     const size_t b_bytes = static_cast<size_t>(round_up(brows * dldb * static_cast<int64_t>(b_es), 256));
     const size_t c_bytes = static_cast<size_t>(round_up(M * dldc * 4, 256));
+    // one host-variant call at a time: the staging buffers, copy streams and events below are shared
+    std::lock_guard<std::mutex> host_lk(g_host_mu);
+    // on an error return, nothing may still be reading or writing the caller's host buffers
+    struct Drain {
+        cudaStream_t s;
+        bool armed = true;
+        ~Drain()
+        {
+            if (!armed) return;
+            cudaStreamSynchronize(s);
+            if (g.copy_in) cudaStreamSynchronize(g.copy_in);
+            if (g.copy_out) cudaStreamSynchronize(g.copy_out);
+        }
+    } drain{stream};
     {
-        std::lock_guard<std::mutex> lk(g_mu);
         const size_t need = a_bytes + b_bytes + c_bytes;
         if (need > g.stage_bytes) {
+            HEAL_CUDA(cudaStreamSynchronize(stream));
             if (g.stage) HEAL_CUDA(cudaFree(g.stage));
             g.stage = nullptr;
             g.stage_bytes = 0;
@@ -1089,9 +1243,9 @@ int heal_gemm_host(int64_t M, int64_t N, int64_t K, const void *A_host, int64_t 
         if (st) return st;
         HEAL_CUDA(cudaMemcpy2DAsync(C_host, ldc * 4, dC, dldc * 4, N * 4, M, cudaMemcpyDeviceToHost, stream));
         HEAL_CUDA(cudaStreamSynchronize(stream));
+        drain.armed = false;
         return HEAL_OK;
     }
-    std::lock_guard<std::mutex> lk(g_host_mu);                  // the copy streams and events below are shared
     if (!g.copy_in) {
         HEAL_CUDA(cudaStreamCreateWithFlags(&g.copy_in, cudaStreamNonBlocking));
         HEAL_CUDA(cudaStreamCreateWithFlags(&g.copy_out, cudaStreamNonBlocking));
@@ -1127,6 +1281,7 @@ int heal_gemm_host(int64_t M, int64_t N, int64_t K, const void *A_host, int64_t 
     }
     HEAL_CUDA(cudaStreamSynchronize(g.copy_out));
     HEAL_CUDA(cudaStreamSynchronize(stream));
+    drain.armed = false;
     return HEAL_OK;
 }
 

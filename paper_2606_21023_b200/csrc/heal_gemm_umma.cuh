@@ -58,16 +58,105 @@ struct GemmArgs {
     int dp_tiles;           // tiles dealt whole, round-robin (multiple of the grid size)
     float *xfer;            // per-CTA hand-off slot: kBM * BN floats each
     uint32_t *flags;        // per-CTA flag: 1 once the slot is written, reset to 0 by its consumer
-    // ordered split-K (few tiles, many CTAs): every (tile, segment) partial goes to `part`, the CTAs that
-    // computed a tile's segments then each finish a share of its columns, adding the partials in ascending order
+    // ordered split-K (few tiles, many CTAs): every (tile, segment) partial goes to `part`; heal_splitk_reduce_kernel,
+    // launched right behind, adds them in ascending segment order and runs the epilogue
     int sk;
     float *part;            // [(tile * R + rank) * n_seg + seg] x (kBM * BN) floats, R = CTAs per tile
-    uint32_t *cnt;          // [(tile * R + rank) * 2]: partials written, shares finished (both back to 0 at the end)
 };
 
-// ---- ordered split-K helpers (256 epilogue threads, etid = 0..255; thread owns row quad*32+lane, CPW columns) ----
-// Partial layout: float4 index c4 * 256 + etid, c4 = 0..CPW/4-1 (the thread's columns 4*c4..4*c4+3): coalesced for
-// the writer and for the finisher, which use the same thread mapping.
+// ---- epilogue building blocks shared by the single-CTA and the CTA-pair kernel (256 epilogue threads, etid = 0..255;
+// a thread owns accumulator row quad*32+lane and CPW consecutive columns, kept as the FP32 running sum run[CPW]) -------
+
+// one finished K segment: TMEM -> registers, FP32 RN add into the running sum (the first segment initialises it)
+template <int CPW>
+__device__ __forceinline__ void epi_add_segment(uint32_t taddr, float (&run)[CPW], bool first)
+{
+#pragma unroll
+    for (int c = 0; c < CPW / 16; ++c) {
+        uint32_t v[16];
+        tmem_ld_32x32b_x16(taddr + c * 16, v);
+        tmem_ld_wait();
+        if (first) {
+#pragma unroll
+            for (int i = 0; i < 16; ++i) run[c * 16 + i] = __uint_as_float(v[i]);
+        } else {
+#pragma unroll
+            for (int i = 0; i < 16; ++i) run[c * 16 + i] = __fadd_rn(run[c * 16 + i], __uint_as_float(v[i]));
+        }
+    }
+}
+
+// Balanced schedule, tail of a shared tile: start from the running sum (segments 0..sb-1) that the neighbouring CTA
+// (or CTA pair) parked in `slot`, once its `flag` is up; the flag is re-armed for the next launch (launches on a stream
+// are serialised, and 0/1 flags -- unlike launch counters -- stay correct when a captured graph is replayed).
+// Progress: the producer is the CTA with the next lower index (same rank of the previous pair), which runs this tile's
+// head FIRST and never waits before it has parked the sum; it is resident whenever this CTA is, because the grid has at
+// most one CTA per SM and the launch is cooperative (all CTAs co-resident, see launch_gemm*_cfg) -- and even without
+// that guarantee blocks are dispatched in index order, so a lower-indexed block is never scheduled later.
+template <int CPW>
+__device__ __forceinline__ void epi_take_prefix(const float *slot, uint32_t *flag, float (&run)[CPW], int etid, int *diag)
+{
+    if (etid == 0) {
+        const uint64_t t0 = globaltimer_ns();
+        uint32_t f;
+        do {
+            asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(f) : "l"(flag) : "memory");
+            if (f == 0u && globaltimer_ns() - t0 > 4000000000ull) {
+                diag[0] = 800;
+                diag[1] = static_cast<int>(blockIdx.x);
+                __trap();
+            }
+        } while (f == 0u);
+    }
+    asm volatile("bar.sync 1, 256;" ::: "memory");
+    const float4 *src = reinterpret_cast<const float4 *>(slot);
+#pragma unroll
+    for (int c = 0; c < CPW / 4; ++c) {
+        float4 v;
+        asm volatile("ld.global.cg.v4.f32 {%0, %1, %2, %3}, [%4];"
+                     : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(src + c * 256 + etid) : "memory");
+        run[c * 4] = v.x; run[c * 4 + 1] = v.y; run[c * 4 + 2] = v.z; run[c * 4 + 3] = v.w;
+    }
+    asm volatile("bar.sync 1, 256;" ::: "memory");
+    if (etid == 0) asm volatile("st.relaxed.gpu.global.u32 [%0], %1;" ::"l"(flag), "r"(0u) : "memory");
+}
+// Balanced schedule, head of a shared tile: hand the running sum to the next CTA (pair)
+template <int CPW>
+__device__ __forceinline__ void epi_hand_on(float *slot, uint32_t *flag, const float (&run)[CPW], int etid)
+{
+    float4 *dst = reinterpret_cast<float4 *>(slot);
+#pragma unroll
+    for (int c = 0; c < CPW / 4; ++c)
+        dst[c * 256 + etid] = make_float4(run[c * 4], run[c * 4 + 1], run[c * 4 + 2], run[c * 4 + 3]);
+    __threadfence();
+    asm volatile("bar.sync 1, 256;" ::: "memory");
+    if (etid == 0) asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(flag), "r"(1u) : "memory");
+}
+// final store of a thread's row segment: plain FP32 (lean instantiation) or the extended epilogue
+template <int CPW, bool FULL>
+__device__ __forceinline__ void epi_store(const OutArgs &out, int row, int col0, const float (&run)[CPW], int M, int N)
+{
+    if (row >= M) return;
+    if constexpr (FULL) {
+        emit_dispatch(out, [&](const OutArgs &po, auto fast) {
+#pragma unroll
+            for (int c = 0; c < CPW; c += 4)
+                emit4<decltype(fast)::value>(po, row, col0 + c, make_float4(run[c], run[c + 1], run[c + 2], run[c + 3]), N);
+        });
+    } else {
+        float *crow = out.C + static_cast<int64_t>(row) * out.ldc;
+#pragma unroll
+        for (int c = 0; c < CPW; c += 4) emit4_plain(crow, col0 + c, make_float4(run[c], run[c + 1], run[c + 2], run[c + 3]), N);
+    }
+}
+
+// ---- ordered split-K (few tiles, many SMs) -------------------------------------------------------------------------
+// The (tile, K segment) units are dealt to more CTAs than there are tiles; every segment partial is parked in global
+// memory by the GEMM kernel and a second, dependent kernel (heal_splitk_reduce_kernel, programmatic dependent launch)
+// adds the n_seg partials of every element in ascending segment order in FP32 RN and runs the epilogue.  No CTA ever
+// waits for another one: nothing depends on which CTAs are resident, and no counters have to be re-armed.
+// Partial layout: float4 index c4 * 256 + etid, c4 = 0..CPW/4-1 (the thread's columns 4*c4..4*c4+3): coalesced for the
+// writer and for the reducer, which use the same thread mapping.
 template <int CPW>
 __device__ __forceinline__ void sk_store_partial(float *part, uint32_t taddr, int etid)
 {
@@ -83,41 +172,29 @@ __device__ __forceinline__ void sk_store_partial(float *part, uint32_t taddr, in
                                                         __uint_as_float(v[4 * q + 2]), __uint_as_float(v[4 * q + 3]));
     }
 }
-__device__ __forceinline__ void sk_signal(uint32_t *ctr, int etid)
+
+// grid = units * shares CTAs of 256 threads; unit = tile * R + rank (R = CTAs per tile: 1, or 2 for CTA pairs); CTA
+// `share` finishes float4 chunks [share*NC/shares, (share+1)*NC/shares) of every row of the unit's 128 x BN block.
+template <int BN>
+__global__ void __launch_bounds__(256)
+heal_splitk_reduce_kernel(const float *__restrict__ part, int n_seg, int R, int tiles_m, int shares, const OutArgs out, int M, int N)
 {
-    __threadfence();
-    asm volatile("bar.sync 1, 256;" ::: "memory");
-    if (etid == 0) asm volatile("red.release.gpu.global.add.u32 [%0], %1;" ::"l"(ctr), "r"(1u) : "memory");
-}
-__device__ __forceinline__ void sk_wait(const uint32_t *ctr, uint32_t want, int etid, int *diag)
-{
-    if (etid == 0) {
-        const uint64_t t0 = globaltimer_ns();
-        uint32_t f;
-        do {
-            asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(f) : "l"(ctr) : "memory");
-            if (f < want && globaltimer_ns() - t0 > 4000000000ull) {
-                diag[0] = 810;
-                diag[1] = static_cast<int>(blockIdx.x);
-                __trap();
-            }
-        } while (f < want);
-    }
-    asm volatile("bar.sync 1, 256;" ::: "memory");
-}
-// The CTA that computed segment `seg` finishes float4 chunks [seg*NC/n_seg, (seg+1)*NC/n_seg) of every row:
-// ascending-segment FP32 RN sum of the n_seg partials, then the predicated store to C.
-template <int CPW, bool EXT>
-__device__ __forceinline__ void sk_finish(const float *part0, int n_seg, int seg, int etid, const OutArgs &out, int64_t row, int col0, int N, bool row_ok)
-{
-    constexpr int NC = CPW / 4;
-    const int c_lo = seg * NC / n_seg, c_hi = (seg + 1) * NC / n_seg;
-    const float4 *src = reinterpret_cast<const float4 *>(part0);
-    const size_t seg_stride = static_cast<size_t>(kBM) * (2 * CPW) / 4;        // float4 per partial (kBM x BN floats)
+    pdl_wait();
+    pdl_launch_dependents();
+    constexpr int CPW = BN / 2, NC = CPW / 4;
+    const int unit = static_cast<int>(blockIdx.x) / shares, share = static_cast<int>(blockIdx.x) % shares;
+    const int tile = unit / R, rank = unit % R;
+    const int etid = threadIdx.x, warp = etid >> 5, lane = etid & 31, quad = warp & 3, chalf = warp >> 2;
+    const int64_t row = static_cast<int64_t>(tile % tiles_m) * (R * kBM) + rank * kBM + quad * 32 + lane;
+    const int col0 = (tile / tiles_m) * BN + chalf * CPW;
+    const float4 *src = reinterpret_cast<const float4 *>(part + static_cast<size_t>(unit) * n_seg * (kBM * BN));
+    const size_t seg_stride = static_cast<size_t>(kBM) * BN / 4;               // float4 per partial
+    const int c_lo = share * NC / shares, c_hi = (share + 1) * NC / shares;
     for (int c4 = c_lo; c4 < c_hi; ++c4) {
         float4 acc;
         asm volatile("ld.global.cg.v4.f32 {%0, %1, %2, %3}, [%4];"
                      : "=f"(acc.x), "=f"(acc.y), "=f"(acc.z), "=f"(acc.w) : "l"(src + c4 * 256 + etid) : "memory");
+#pragma unroll 4
         for (int s = 1; s < n_seg; ++s) {
             float4 v;
             asm volatile("ld.global.cg.v4.f32 {%0, %1, %2, %3}, [%4];"
@@ -125,27 +202,10 @@ __device__ __forceinline__ void sk_finish(const float *part0, int n_seg, int seg
             acc.x = __fadd_rn(acc.x, v.x); acc.y = __fadd_rn(acc.y, v.y);
             acc.z = __fadd_rn(acc.z, v.z); acc.w = __fadd_rn(acc.w, v.w);
         }
-        if (row_ok) {
-            if constexpr (EXT) {
-                emit_dispatch(out, [&](const OutArgs &po, auto fast) {
-                    emit4<decltype(fast)::value>(po, row, col0 + c4 * 4, acc, N);
-                });
-            } else {
-                emit4_plain(out.C + row * out.ldc, col0 + c4 * 4, acc, N);
-            }
-        }
-    }
-}
-// last finisher of a (tile, rank): re-arm both counters for the next launch on this stream
-__device__ __forceinline__ void sk_done(uint32_t *ctr, uint32_t n_seg, int etid)
-{
-    asm volatile("bar.sync 1, 256;" ::: "memory");
-    if (etid == 0) {
-        uint32_t old;
-        asm volatile("atom.acq_rel.gpu.global.add.u32 %0, [%1], %2;" : "=r"(old) : "l"(ctr + 1), "r"(1u) : "memory");
-        if (old == n_seg - 1) {
-            asm volatile("st.relaxed.gpu.global.u32 [%0], %1;" ::"l"(ctr), "r"(0u) : "memory");
-            asm volatile("st.relaxed.gpu.global.u32 [%0], %1;" ::"l"(ctr + 1), "r"(0u) : "memory");
+        if (row < M) {
+            emit_dispatch(out, [&](const OutArgs &po, auto fast) {
+                emit4<decltype(fast)::value>(po, row, col0 + c4 * 4, acc, N);
+            });
         }
     }
 }
@@ -305,129 +365,44 @@ heal_gemm_umma_kernel(const __grid_constant__ CUtensorMap tm_a_hi, const __grid_
             sched.get(ci, tile, sb_seg, se_seg);
             const int m0 = (tile % args.tiles_m) * kBM;
             const int n0 = (tile / args.tiles_m) * BN;
-            if (Cfg::FULL && args.sk) {
-                // ordered split-K: park every segment partial in global memory; the sums are formed below
-                for (int seg = sb_seg; seg < se_seg; ++seg) {
-                    mbar_wait_ool(tfull_bar(buf), (tphase >> buf) & 1u, args.diag, 400 + buf);
-                    tc_fence_after();
-                    const uint32_t taddr = tmem_base + (static_cast<uint32_t>(quad * 32) << 16) +
-                                           static_cast<uint32_t>(buf * BN + chalf * CPW);
-                    sk_store_partial<CPW>(args.part + (static_cast<size_t>(tile) * n_seg + seg) * (kBM * BN), taddr, etid);
-                    tc_fence_before();
-                    __syncwarp();
-                    if (lane == 0) mbar_arrive(tempty_bar(buf));
-                    tphase ^= 1u << buf;
-                    buf ^= 1;
-                    sk_signal(args.cnt + 2 * tile, etid);
+            if constexpr (Cfg::FULL) {
+                if (args.sk) {
+                    // ordered split-K: park every segment partial in global memory; heal_splitk_reduce_kernel forms the sums
+                    for (int seg = sb_seg; seg < se_seg; ++seg) {
+                        mbar_wait_ool(tfull_bar(buf), (tphase >> buf) & 1u, args.diag, 400 + buf);
+                        tc_fence_after();
+                        const uint32_t taddr = tmem_base + (static_cast<uint32_t>(quad * 32) << 16) +
+                                               static_cast<uint32_t>(buf * BN + chalf * CPW);
+                        sk_store_partial<CPW>(args.part + (static_cast<size_t>(tile) * n_seg + seg) * (kBM * BN), taddr, etid);
+                        tc_fence_before();
+                        __syncwarp();
+                        if (lane == 0) mbar_arrive(tempty_bar(buf));
+                        tphase ^= 1u << buf;
+                        buf ^= 1;
+                    }
+                    continue;
                 }
-                continue;
             }
-            if (sb_seg > 0) {
-                // tail of a shared tile: start from the neighbour's running sum (segments 0..sb_seg-1)
-                const uint32_t *flag = args.flags + (blockIdx.x - 1);
-                if (etid == 0) {
-                    const uint64_t t0 = globaltimer_ns();
-                    uint32_t f;
-                    do {
-                        asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(f) : "l"(flag) : "memory");
-                        if (f == 0u && globaltimer_ns() - t0 > 4000000000ull) {
-                            args.diag[0] = 800;
-                            args.diag[1] = static_cast<int>(blockIdx.x);
-                            __trap();
-                        }
-                    } while (f == 0u);
-                }
-                asm volatile("bar.sync 1, 256;" ::: "memory");
-                const float4 *src = reinterpret_cast<const float4 *>(args.xfer + static_cast<size_t>(blockIdx.x - 1) * (kBM * BN));
-#pragma unroll
-                for (int c = 0; c < CPW / 4; ++c) {
-                    float4 v;
-                    asm volatile("ld.global.cg.v4.f32 {%0, %1, %2, %3}, [%4];"
-                                 : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(src + c * 256 + etid) : "memory");
-                    run[c * 4] = v.x; run[c * 4 + 1] = v.y; run[c * 4 + 2] = v.z; run[c * 4 + 3] = v.w;
-                }
-                // consumed: re-arm the flag for the next launch (launches on a stream are serialised, and
-                // 0/1 flags -- unlike launch counters -- stay correct when a captured graph is replayed)
-                asm volatile("bar.sync 1, 256;" ::: "memory");
-                if (etid == 0) asm volatile("st.relaxed.gpu.global.u32 [%0], %1;" ::"l"(flag), "r"(0u) : "memory");
-            }
+            if (sb_seg > 0)        // tail of a shared tile: start from the neighbour's running sum (segments 0..sb_seg-1)
+                epi_take_prefix<CPW>(args.xfer + static_cast<size_t>(blockIdx.x - 1) * (kBM * BN), args.flags + (blockIdx.x - 1), run, etid, args.diag);
             for (int seg = sb_seg; seg < se_seg; ++seg) {
                 mbar_wait_ool(tfull_bar(buf), (tphase >> buf) & 1u, args.diag, 400 + buf);
                 tc_fence_after();
                 const uint32_t taddr = tmem_base + (static_cast<uint32_t>(quad * 32) << 16) +
                                        static_cast<uint32_t>(buf * BN + chalf * CPW);
-#pragma unroll
-                for (int c = 0; c < CPW / 16; ++c) {
-                    uint32_t v[16];
-                    tmem_ld_32x32b_x16(taddr + c * 16, v);
-                    tmem_ld_wait();
-                    if (seg == 0) {
-#pragma unroll
-                        for (int i = 0; i < 16; ++i) run[c * 16 + i] = __uint_as_float(v[i]);
-                    } else {
-#pragma unroll
-                        for (int i = 0; i < 16; ++i) run[c * 16 + i] = __fadd_rn(run[c * 16 + i], __uint_as_float(v[i]));
-                    }
-                }
+                epi_add_segment<CPW>(taddr, run, seg == 0);
                 tc_fence_before();
                 __syncwarp();
                 if (lane == 0) mbar_arrive(tempty_bar(buf));
                 tphase ^= 1u << buf;
                 buf ^= 1;
             }
-            if (se_seg < n_seg) {
-                // head of a shared tile: hand the running sum to the next CTA
-                float4 *dst = reinterpret_cast<float4 *>(args.xfer + static_cast<size_t>(blockIdx.x) * (kBM * BN));
-#pragma unroll
-                for (int c = 0; c < CPW / 4; ++c)
-                    dst[c * 256 + etid] = make_float4(run[c * 4], run[c * 4 + 1], run[c * 4 + 2], run[c * 4 + 3]);
-                __threadfence();
-                asm volatile("bar.sync 1, 256;" ::: "memory");
-                if (etid == 0)
-                    asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(args.flags + blockIdx.x), "r"(1u) : "memory");
+            if (se_seg < n_seg) {  // head of a shared tile: hand the running sum to the next CTA
+                epi_hand_on<CPW>(args.xfer + static_cast<size_t>(blockIdx.x) * (kBM * BN), args.flags + blockIdx.x, run, etid);
                 continue;
             }
             // ---- store: thread owns row m0 + quad*32 + lane, CPW consecutive columns
-            const int row = m0 + quad * 32 + lane;
-            const int col0 = n0 + chalf * CPW;
-            if (row < args.M) {
-                if constexpr (Cfg::FULL) {
-                    emit_dispatch(args.out, [&](const OutArgs &po, auto fast) {
-#pragma unroll
-                        for (int c = 0; c < CPW; c += 4)
-                            emit4<decltype(fast)::value>(po, row, col0 + c, make_float4(run[c], run[c + 1], run[c + 2], run[c + 3]), args.N);
-                    });
-                } else {
-                    float *crow = args.out.C + static_cast<int64_t>(row) * args.out.ldc;
-#pragma unroll
-                    for (int c = 0; c < CPW; c += 4) {
-                        const int col = col0 + c;
-                        if (col + 3 < args.N) {
-                            *reinterpret_cast<float4 *>(crow + col) = make_float4(run[c], run[c + 1], run[c + 2], run[c + 3]);
-                        } else {
-#pragma unroll
-                            for (int i = 0; i < 4; ++i)
-                                if (col + i < args.N) crow[col + i] = run[c + i];
-                        }
-                    }
-                }
-            }
-        }
-        if (Cfg::FULL && args.sk) {
-            // every partial of this CTA is parked: finish a share of the columns of each unit's tile
-            for (int ci = 0; ci < sched.n_chunks; ++ci) {
-                int tile, sb_seg, se_seg;
-                sched.get(ci, tile, sb_seg, se_seg);
-                const int m0 = (tile % args.tiles_m) * kBM;
-                const int n0 = (tile / args.tiles_m) * BN;
-                const int row = m0 + quad * 32 + lane;
-                sk_wait(args.cnt + 2 * tile, static_cast<uint32_t>(n_seg), etid, args.diag);
-                for (int seg = sb_seg; seg < se_seg; ++seg) {
-                    sk_finish<CPW, Cfg::FULL>(args.part + static_cast<size_t>(tile) * n_seg * (kBM * BN), n_seg, seg, etid,
-                                   args.out, row, n0 + chalf * CPW, args.N, row < args.M);
-                    sk_done(args.cnt + 2 * tile, static_cast<uint32_t>(n_seg), etid);
-                }
-            }
+            epi_store<CPW, Cfg::FULL>(args.out, m0 + quad * 32 + lane, n0 + chalf * CPW, run, args.M, args.N);
         }
     }
 

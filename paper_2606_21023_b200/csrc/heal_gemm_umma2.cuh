@@ -193,69 +193,32 @@ heal_gemm_umma2_kernel(const __grid_constant__ CUtensorMap tm_a_hi, const __grid
             sched.get(ci, tile, sb_seg, se_seg);
             const int m0 = (tile % args.tiles_m) * (2 * kBM) + rank * kBM;
             const int n0 = (tile / args.tiles_m) * BN;
-            if (Cfg::FULL && args.sk) {
-                // ordered split-K (see heal_gemm_umma.cuh): park every segment partial of this CTA's 128 rows
-                for (int seg = sb_seg; seg < se_seg; ++seg) {
-                    mbar_wait_ool(tfull_bar(buf), (tphase >> buf) & 1u, args.diag, 400 + buf);
-                    tc_fence_after();
-                    const uint32_t taddr = tmem_base + (static_cast<uint32_t>(quad * 32) << 16) +
-                                           static_cast<uint32_t>(buf * BN + chalf * CPW);
-                    sk_store_partial<CPW>(args.part + ((static_cast<size_t>(tile) * 2 + rank) * n_seg + seg) * (kBM * BN), taddr, etid);
-                    tc_fence_before();
-                    __syncwarp();
-                    if (lane == 0) mbar_arrive_cluster(leader_addr(tempty_bar(buf)));
-                    tphase ^= 1u << buf;
-                    buf ^= 1;
-                    sk_signal(args.cnt + 2 * (tile * 2 + rank), etid);
+            if constexpr (Cfg::FULL) {
+                if (args.sk) {
+                    // ordered split-K (see heal_gemm_umma.cuh): park every segment partial of this CTA's 128 rows
+                    for (int seg = sb_seg; seg < se_seg; ++seg) {
+                        mbar_wait_ool(tfull_bar(buf), (tphase >> buf) & 1u, args.diag, 400 + buf);
+                        tc_fence_after();
+                        const uint32_t taddr = tmem_base + (static_cast<uint32_t>(quad * 32) << 16) +
+                                               static_cast<uint32_t>(buf * BN + chalf * CPW);
+                        sk_store_partial<CPW>(args.part + ((static_cast<size_t>(tile) * 2 + rank) * n_seg + seg) * (kBM * BN), taddr, etid);
+                        tc_fence_before();
+                        __syncwarp();
+                        if (lane == 0) mbar_arrive_cluster(leader_addr(tempty_bar(buf)));
+                        tphase ^= 1u << buf;
+                        buf ^= 1;
+                    }
+                    continue;
                 }
-                continue;
             }
-            if (sb_seg > 0) {
-                const uint32_t *flag = args.flags + (blockIdx.x - 2);        // same rank, previous pair
-                if (etid == 0) {
-                    const uint64_t t0 = globaltimer_ns();
-                    uint32_t f;
-                    do {
-                        asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(f) : "l"(flag) : "memory");
-                        if (f == 0u && globaltimer_ns() - t0 > 4000000000ull) {
-                            args.diag[0] = 800;
-                            args.diag[1] = static_cast<int>(blockIdx.x);
-                            __trap();
-                        }
-                    } while (f == 0u);
-                }
-                asm volatile("bar.sync 1, 256;" ::: "memory");
-                const float4 *src = reinterpret_cast<const float4 *>(args.xfer + static_cast<size_t>(blockIdx.x - 2) * (kBM * 256));
-#pragma unroll
-                for (int c = 0; c < CPW / 4; ++c) {
-                    float4 v;
-                    asm volatile("ld.global.cg.v4.f32 {%0, %1, %2, %3}, [%4];"
-                                 : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(src + c * 256 + etid) : "memory");
-                    run[c * 4] = v.x; run[c * 4 + 1] = v.y; run[c * 4 + 2] = v.z; run[c * 4 + 3] = v.w;
-                }
-                // consumed: re-arm the flag for the next launch (launches on a stream are serialised, and
-                // 0/1 flags -- unlike launch counters -- stay correct when a captured graph is replayed)
-                asm volatile("bar.sync 1, 256;" ::: "memory");
-                if (etid == 0) asm volatile("st.relaxed.gpu.global.u32 [%0], %1;" ::"l"(flag), "r"(0u) : "memory");
-            }
+            if (sb_seg > 0)        // same rank of the previous pair
+                epi_take_prefix<CPW>(args.xfer + static_cast<size_t>(blockIdx.x - 2) * (kBM * 256), args.flags + (blockIdx.x - 2), run, etid, args.diag);
             for (int seg = sb_seg; seg < se_seg; ++seg) {
                 mbar_wait_ool(tfull_bar(buf), (tphase >> buf) & 1u, args.diag, 400 + buf);
                 tc_fence_after();
                 const uint32_t taddr = tmem_base + (static_cast<uint32_t>(quad * 32) << 16) +
                                        static_cast<uint32_t>(buf * BN + chalf * CPW);
-#pragma unroll
-                for (int c = 0; c < CPW / 16; ++c) {
-                    uint32_t v[16];
-                    tmem_ld_32x32b_x16(taddr + c * 16, v);
-                    tmem_ld_wait();
-                    if (seg == 0) {
-#pragma unroll
-                        for (int i = 0; i < 16; ++i) run[c * 16 + i] = __uint_as_float(v[i]);
-                    } else {
-#pragma unroll
-                        for (int i = 0; i < 16; ++i) run[c * 16 + i] = __fadd_rn(run[c * 16 + i], __uint_as_float(v[i]));
-                    }
-                }
+                epi_add_segment<CPW>(taddr, run, seg == 0);
                 tc_fence_before();
                 __syncwarp();
                 if (lane == 0) mbar_arrive_cluster(leader_addr(tempty_bar(buf)));
@@ -263,56 +226,10 @@ heal_gemm_umma2_kernel(const __grid_constant__ CUtensorMap tm_a_hi, const __grid
                 buf ^= 1;
             }
             if (se_seg < n_seg) {
-                float4 *dst = reinterpret_cast<float4 *>(args.xfer + static_cast<size_t>(blockIdx.x) * (kBM * 256));
-#pragma unroll
-                for (int c = 0; c < CPW / 4; ++c)
-                    dst[c * 256 + etid] = make_float4(run[c * 4], run[c * 4 + 1], run[c * 4 + 2], run[c * 4 + 3]);
-                __threadfence();
-                asm volatile("bar.sync 1, 256;" ::: "memory");
-                if (etid == 0)
-                    asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(args.flags + blockIdx.x), "r"(1u) : "memory");
+                epi_hand_on<CPW>(args.xfer + static_cast<size_t>(blockIdx.x) * (kBM * 256), args.flags + blockIdx.x, run, etid);
                 continue;
             }
-            const int row = m0 + quad * 32 + lane;
-            const int col0 = n0 + chalf * CPW;
-            if (row < args.M) {
-                if constexpr (Cfg::FULL) {
-                    emit_dispatch(args.out, [&](const OutArgs &po, auto fast) {
-#pragma unroll
-                        for (int c = 0; c < CPW; c += 4)
-                            emit4<decltype(fast)::value>(po, row, col0 + c, make_float4(run[c], run[c + 1], run[c + 2], run[c + 3]), args.N);
-                    });
-                } else {
-                    float *crow = args.out.C + static_cast<int64_t>(row) * args.out.ldc;
-#pragma unroll
-                    for (int c = 0; c < CPW; c += 4) {
-                        const int col = col0 + c;
-                        if (col + 3 < args.N) {
-                            *reinterpret_cast<float4 *>(crow + col) = make_float4(run[c], run[c + 1], run[c + 2], run[c + 3]);
-                        } else {
-#pragma unroll
-                            for (int i = 0; i < 4; ++i)
-                                if (col + i < args.N) crow[col + i] = run[c + i];
-                        }
-                    }
-                }
-            }
-        }
-        if (Cfg::FULL && args.sk) {
-            for (int ci = 0; ci < sched.n_chunks; ++ci) {
-                int tile, sb_seg, se_seg;
-                sched.get(ci, tile, sb_seg, se_seg);
-                const int m0 = (tile % args.tiles_m) * (2 * kBM) + rank * kBM;
-                const int n0 = (tile / args.tiles_m) * BN;
-                const int row = m0 + quad * 32 + lane;
-                uint32_t *ctr = args.cnt + 2 * (tile * 2 + rank);
-                sk_wait(ctr, static_cast<uint32_t>(n_seg), etid, args.diag);
-                for (int seg = sb_seg; seg < se_seg; ++seg) {
-                    sk_finish<CPW, Cfg::FULL>(args.part + (static_cast<size_t>(tile) * 2 + rank) * n_seg * (kBM * BN), n_seg, seg, etid,
-                                   args.out, row, n0 + chalf * CPW, args.N, row < args.M);
-                    sk_done(ctr, static_cast<uint32_t>(n_seg), etid);
-                }
-            }
+            epi_store<CPW, Cfg::FULL>(args.out, m0 + quad * 32 + lane, n0 + chalf * CPW, run, args.M, args.N);
         }
     }
 

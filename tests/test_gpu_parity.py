@@ -587,6 +587,54 @@ def test_ordered_split_k_two_streams(hb, inputs):
         assert torch.equal(a, r1) and torch.equal(d, r1) and torch.equal(b, r2) and torch.equal(c, r2)
 
 
+@pytest.mark.parametrize("M,N,K", [(1, 12800, 20480), (16, 6400, 20480), (8, 19200, 10240)])
+def test_small_m_cluster_grid_never_oversubscribes_tmem(hb, inputs, M, N, K):
+    """Cluster shapes whose CTAs each need 128..256 TMEM columns on a grid larger than two CTAs per SM: shared memory is
+    sized so that the CTAs resident on an SM can always allocate (a CTA blocked in tcgen05.alloc before its cluster
+    barrier, with peers holding TMEM elsewhere, could hang the GPU).  Result: bit-identical to the large-M kernel."""
+    A = dev(inputs.activations(M, K, seed=31, outliers=True))
+    W = dev(inputs.weights_f16(K, N, seed=31))
+    try:
+        hb.debug_force_kernel(0)
+        outs = [hb.heal_gemm(A, W, 2).clone() for _ in range(3)]
+        hb.debug_force_kernel(1)
+        ref = hb.heal_gemm(A, W, 2).clone()
+    finally:
+        hb.debug_force_kernel(0)
+    torch.cuda.synchronize()
+    assert all(torch.equal(o, ref) for o in outs)
+
+
+def test_graph_survives_workspace_growth(hb, inputs):
+    """Warm up and capture a small problem, then run a larger one eagerly on the same stream (the library-owned hi/lo
+    plane workspace and the split-K partial area have to grow), then replay the graph: the buffers baked into the graph
+    must still be alive and private (they are retired, not freed), so the replay reproduces the eager bits."""
+    A1 = dev(inputs.activations(32, 4096, seed=41, outliers=True)); W1 = dev(inputs.weights_f16(4096, 1032, seed=41))
+    A2 = dev(inputs.activations(128, 4096, seed=42)); W2 = dev(inputs.weights_f16(4096, 1032, seed=42))       # ordered split-K
+    A3 = dev(inputs.activations(1300, 8192, seed=43)); W3 = dev(inputs.weights_f16(8192, 4104, seed=43))
+    s = torch.cuda.Stream()
+    torch.cuda.synchronize()
+    with torch.cuda.stream(s):
+        r1 = hb.heal_gemm(A1, W1, 2).clone()
+        r2 = hb.heal_gemm(A2, W2, 2).clone()
+        C1, C2 = torch.zeros_like(r1), torch.zeros_like(r2)
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=s):
+            hb.heal_gemm(A1, W1, 2, C=C1)
+            hb.heal_gemm(A2, W2, 2, C=C2)
+        r3 = hb.heal_gemm(A3, W3, 2).clone()                  # grows the plane workspace of this stream
+        A4 = dev(inputs.activations(512, 8192, seed=44)); W4 = dev(inputs.weights_f16(8192, 2056, seed=44))
+        hb.heal_gemm(A4, W4, 2)                               # a larger split-K problem: grows the partial area
+        junk = [torch.full((1 << 22,), 3.0, device="cuda") for _ in range(8)]      # re-use whatever was freed
+        for _ in range(3):
+            C1.zero_(); C2.zero_()
+            g.replay()
+            c3 = hb.heal_gemm(A3, W3, 2)
+            s.synchronize()
+            assert torch.equal(C1, r1) and torch.equal(C2, r2) and torch.equal(c3, r3)
+        del junk
+
+
 def test_static_flag_with_on_the_fly_weight_split(hb, inputs):
     """HEAL_B_STATIC on a three-product heal_gemm: the B planes are written by the library's own split kernel right
     before the GEMM, so the flag must not let the GEMM prefetch them early (found by a soak run: stale planes of the
