@@ -67,6 +67,16 @@ typedef enum {
                                   still waits for the predecessor.  Same bits with or without the flag.  Ignored by
                                   heal_gemm in the FP32-B modes (3P/4P), whose B planes are produced on the fly. */
 
+#define HEAL_EPI_SILU_MUL 0x80u   /* step E fused with the MLP activation of Algorithm 1, "SiLU(g) (.) u" (SURVEY.md 8(f)
+                                     NEXT-3): the GEMM's N columns are (gate, up) pairs -- column 2j = g_j, column 2j+1 = u_j, i.e.
+                                     the gate and up projection weights interleaved column-wise -- N must be even, and every
+                                     output (C, C_hi/C_lo) is M x N/2 and receives  g_j / (1 + exp(-g_j)) * u_j  computed in FP32
+                                     from the (2^-scale_exp scaled) GEMM results; with C_hi/C_lo this is the activation of the down
+                                     projection, already split for heal_gemm_presplit.  ldc, ldc16 >= N/2. */
+#define HEAL_EPI_ACCUMULATE 0x100u /* step E fused with the residual add of Algorithm 1, "A_i + GEMM(...)" (FP32 residual
+                                     flow): C must hold the residual on entry and receives C + result (one FP32 RN add
+                                     per element); the planes, if requested, are the split of that sum.  Needs C. */
+
 #define HEAL_LO_SHIFT 10
 #define HEAL_LO_SCALED 0x40u   /* the paper's scaled residual, Eq. 10 as printed: h = h_hi +
                                   h_lo / 2^10 with h_lo = r16((h - h_hi) * 2^10), C = GEMM(h_hi, W) +
@@ -117,6 +127,16 @@ int heal_split(int64_t rows, int64_t cols, const void *X, int64_t ldx,
  * (PAPER.md:203 uses 10).  heal_split(...) == heal_split_scaled(..., 0, stream). */
 int heal_split_scaled(int64_t rows, int64_t cols, const void *X, int64_t ldx,
                       void *hi, void *lo, int64_t ld, int32_t lo_shift, void *stream);
+
+/*
+ * Norm -> step S in one pass ("GEMM(Norm(H_i), W)"; FP32 normalization): RMSNorm of
+ * every row of X in FP32,   y[r][c] = (X[r][c] * rstd_r) * gamma[c],   rstd_r = 1 / sqrt(mean_c X[r][c]^2 + eps),
+ * immediately split into hi = r16(y), lo = r16(y - hi) for heal_gemm_presplit -- the normalised FP32 activations are written
+ * only if Y != NULL (pitch ldy >= cols, % 4 == 0).  gamma: FP32 vector of `cols` elements, 16-byte aligned, or NULL (= ones).
+ * Other arguments as heal_split.  Deterministic: the result of a row does not depend on the other rows or on `rows`.
+ */
+int heal_rmsnorm_split(int64_t rows, int64_t cols, const void *X, int64_t ldx, const void *gamma, float eps,
+                       void *hi, void *lo, int64_t ld, void *Y, int64_t ldy, void *stream);
 
 /*
  * Steps G + E on pre-split planes: C = sum of the products `mode` keeps.

@@ -15,16 +15,17 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "heal_oracle.c")
+_SRC2 = os.path.join(_HERE, "heal_fusions.c")
 _LIB = os.path.join(_HERE, "liboracle.so")
 _lib = None
 
 
 def build(force: bool = False) -> str:
-    """Compile heal_oracle.c with gcc (-O2, OpenMP, no FP contraction) into liboracle.so."""
-    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+    """Compile heal_oracle.c + heal_fusions.c with gcc (-O2, OpenMP, no FP contraction) into liboracle.so."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < max(os.path.getmtime(_SRC), os.path.getmtime(_SRC2)):
         tmp = _LIB + ".tmp%d" % os.getpid()
         subprocess.check_call(["gcc", "-O2", "-fopenmp", "-ffp-contract=off", "-shared", "-fPIC",
-                               "-o", tmp, _SRC, "-lm"])
+                               "-o", tmp, _SRC, _SRC2, "-lm"])
         os.replace(tmp, _LIB)
     return _LIB
 
@@ -51,6 +52,15 @@ def lib():
         L.oracle_diff_sumsq.restype = ctypes.c_double
         L.oracle_diff_sumsq.argtypes = [i64, i64, vp, i64, vp, vp]
         L.oracle_num_threads.restype = ci
+        d = ctypes.c_double
+        L.oracle_rmsnorm_f64.restype = None
+        L.oracle_rmsnorm_f64.argtypes = [i64, i64, vp, i64, vp, d, vp]
+        L.oracle_silu_mul_f64.restype = None
+        L.oracle_silu_mul_f64.argtypes = [i64, i64, vp, vp]
+        L.oracle_gemm_dd.restype = ci
+        L.oracle_gemm_dd.argtypes = [i64, i64, i64, vp, vp, i64, ci, ci, vp, i64, vp]
+        L.oracle_add_f64.restype = None
+        L.oracle_add_f64.argtypes = [i64, i64, vp, i64, vp, vp]
         _lib = L
     return _lib
 
@@ -170,6 +180,49 @@ def normwise_error(C, Cref, A, B, rows=None) -> float:
     d = lib().oracle_diff_sumsq(R, C.shape[1], _ptr(C), C.strides[0] // 4, _ptr(r), _ptr(Cref))
     As = A if rows is None else np.ascontiguousarray(A[np.asarray(rows)])
     return float(np.sqrt(d)) / (fro_f32(As) * fro_b(B))
+
+
+def rmsnorm_f64(X, gamma=None, eps: float = 0.0) -> np.ndarray:
+    """F1: RMSNorm of every row of the float32 matrix X in double ("Norm"; A17)."""
+    ldx = _check_a(X)
+    g = None if gamma is None else np.ascontiguousarray(np.asarray(gamma, dtype=np.float32))
+    assert g is None or g.shape == (X.shape[1],)
+    Y = np.empty(X.shape, np.float64)
+    lib().oracle_rmsnorm_f64(X.shape[0], X.shape[1], _ptr(X), ldx, _ptr(g), float(eps), _ptr(Y))
+    return Y
+
+
+def silu_mul_f64(C) -> np.ndarray:
+    """F2: h[j] = silu(c[2j]) * c[2j+1] on every row of the double matrix C ("SiLU(g) (.) u"; A18)."""
+    C = np.ascontiguousarray(np.asarray(C, dtype=np.float64))
+    assert C.ndim == 2 and C.shape[1] % 2 == 0
+    H = np.empty((C.shape[0], C.shape[1] // 2), np.float64)
+    lib().oracle_silu_mul_f64(C.shape[0], C.shape[1] // 2, _ptr(C), _ptr(H))
+    return H
+
+
+def gemm_dd(A, B, b_nk: bool = False, rows=None) -> np.ndarray:
+    """F3: O1's definition for a double first operand (the next GEMM of a chain): A float64 (M, K), B as in gemm_f64."""
+    A = np.ascontiguousarray(np.asarray(A, dtype=np.float64))
+    b16, ldb = _check_b(B)
+    M, K = A.shape
+    N = B.shape[0] if b_nk else B.shape[1]
+    assert (B.shape[1] if b_nk else B.shape[0]) == K
+    r, nr = _rows(rows)
+    C = np.empty(((nr if rows is not None else M), N), np.float64)
+    rc = lib().oracle_gemm_dd(M, N, K, _ptr(A), _ptr(B), ldb, b16, int(b_nk), _ptr(r), nr, _ptr(C))
+    assert rc == 0
+    return C
+
+
+def add_f64(X, Y) -> np.ndarray:
+    """F4: the residual add X + Y, X float32, Y float64, in double."""
+    ldx = _check_a(X)
+    Y = np.ascontiguousarray(np.asarray(Y, dtype=np.float64))
+    assert Y.shape == X.shape
+    Z = np.empty(X.shape, np.float64)
+    lib().oracle_add_f64(X.shape[0], X.shape[1], _ptr(X), ldx, _ptr(Y), _ptr(Z))
+    return Z
 
 
 def num_threads() -> int:

@@ -17,6 +17,8 @@ MODE_1P, MODE_2P, MODE_3P, MODE_4P = 1, 2, 3, 4
 B_NK = 0x10
 B_STATIC = 0x20
 LO_SCALED = 0x40
+EPI_SILU_MUL = 0x80
+EPI_ACCUMULATE = 0x100
 LO_SHIFT = 10
 K_SEGMENT = 512
 
@@ -44,6 +46,8 @@ def lib():
         L.heal_split.argtypes = [i64, i64, vp, i64, vp, vp, i64, vp]
         L.heal_split_scaled.restype = ci
         L.heal_split_scaled.argtypes = [i64, i64, vp, i64, vp, vp, i64, ctypes.c_int32, vp]
+        L.heal_rmsnorm_split.restype = ci
+        L.heal_rmsnorm_split.argtypes = [i64, i64, vp, i64, vp, ctypes.c_float, vp, vp, i64, vp, i64, vp]
         L.heal_gemm_presplit.restype = ci
         L.heal_gemm_presplit.argtypes = [i64, i64, i64, vp, vp, i64, vp, vp, i64, vp, i64, u32, vp]
         i32 = ctypes.c_int32
@@ -120,10 +124,15 @@ def heal_gemm(A: torch.Tensor, B: torch.Tensor, mode: int = MODE_2P, C: torch.Te
     N = B.shape[0] if mode & B_NK else B.shape[1]
     assert (B.shape[1] if mode & B_NK else B.shape[0]) == K
     if C is None:
-        C = torch.empty((M, N), dtype=torch.float32, device=A.device)
+        C = torch.empty((M, _n_out(N, mode)), dtype=torch.float32, device=A.device)
     _check(lib().heal_gemm(M, N, K, A.data_ptr(), _ld(A), B.data_ptr(), _ld(B), C.data_ptr(), _ld(C), mode,
                            _stream(stream)))
     return C
+
+
+def _n_out(N: int, mode: int) -> int:
+    """Output columns: N, or N/2 with the SiLU-mul epilogue ((gate, up) column pairs -> one activation)."""
+    return N // 2 if mode & EPI_SILU_MUL else N
 
 
 def _planes(M, N, device):
@@ -140,9 +149,9 @@ def heal_gemm_ex(A: torch.Tensor, B: torch.Tensor, mode: int = MODE_2P, C: torch
     M, K = A.shape
     N = B.shape[0] if mode & B_NK else B.shape[1]
     if C is None and want_c:
-        C = torch.empty((M, N), dtype=torch.float32, device=A.device)
+        C = torch.empty((M, _n_out(N, mode)), dtype=torch.float32, device=A.device)
     if want_planes and C_hi is None:
-        C_hi, C_lo = _planes(M, N, A.device)
+        C_hi, C_lo = _planes(M, _n_out(N, mode), A.device)
     p = lambda t: None if t is None else t.data_ptr()
     _check(lib().heal_gemm_ex(M, N, K, A.data_ptr(), _ld(A), B.data_ptr(), _ld(B), p(C), 0 if C is None else _ld(C),
                               p(C_hi), p(C_lo), 0 if C_hi is None else _ld(C_hi), scale_exp, mode, _stream(stream)))
@@ -155,9 +164,9 @@ def heal_gemm_presplit_ex(A_hi, A_lo, B_hi, B_lo, mode: int, C: torch.Tensor | N
     M, K = A_hi.shape
     N = B_hi.shape[0] if mode & B_NK else B_hi.shape[1]
     if C is None and want_c:
-        C = torch.empty((M, N), dtype=torch.float32, device=A_hi.device)
+        C = torch.empty((M, _n_out(N, mode)), dtype=torch.float32, device=A_hi.device)
     if want_planes and C_hi is None:
-        C_hi, C_lo = _planes(M, N, A_hi.device)
+        C_hi, C_lo = _planes(M, _n_out(N, mode), A_hi.device)
     p = lambda t: None if t is None else t.data_ptr()
     _check(lib().heal_gemm_presplit_ex(M, N, K, p(A_hi), p(A_lo), _ld(A_hi), p(B_hi), p(B_lo), _ld(B_hi), p(C),
                                        0 if C is None else _ld(C), p(C_hi), p(C_lo), 0 if C_hi is None else _ld(C_hi),
@@ -184,12 +193,25 @@ def heal_split(X: torch.Tensor, hi: torch.Tensor | None = None, lo: torch.Tensor
     return hi, lo
 
 
+def heal_rmsnorm_split(X: torch.Tensor, gamma: torch.Tensor | None = None, eps: float = 1e-6, want_y: bool = False, stream=None):
+    """RMSNorm of every row of the fp32 matrix X, split into (hi, lo) fp16 planes in the same pass (PAPER.md:76 Norm -> GEMM);
+    returns (hi, lo, Y or None) where Y is the fp32 normalised matrix (only written when asked for)."""
+    assert X.is_cuda and X.dtype == torch.float32 and X.dim() == 2
+    rows, cols = X.shape
+    hi, lo = _planes(rows, cols, X.device)
+    Y = torch.empty((rows, (cols + 3) // 4 * 4), dtype=torch.float32, device=X.device)[:, :cols] if want_y else None
+    _check(lib().heal_rmsnorm_split(rows, cols, X.data_ptr(), _ld(X), None if gamma is None else gamma.data_ptr(), float(eps),
+                                    hi.data_ptr(), lo.data_ptr(), _ld(hi), None if Y is None else Y.data_ptr(),
+                                    0 if Y is None else _ld(Y), _stream(stream)))
+    return hi, lo, Y
+
+
 def heal_gemm_presplit(A_hi, A_lo, B_hi, B_lo, mode: int, C: torch.Tensor | None = None, stream=None):
     """C from pre-split fp16 planes (steps G + E)."""
     M, K = A_hi.shape
     N = B_hi.shape[0] if mode & B_NK else B_hi.shape[1]
     if C is None:
-        C = torch.empty((M, N), dtype=torch.float32, device=A_hi.device)
+        C = torch.empty((M, _n_out(N, mode)), dtype=torch.float32, device=A_hi.device)
     p = lambda t: None if t is None else t.data_ptr()
     _check(lib().heal_gemm_presplit(M, N, K, p(A_hi), p(A_lo), _ld(A_hi), p(B_hi), p(B_lo), _ld(B_hi),
                                     C.data_ptr(), _ld(C), mode, _stream(stream)))

@@ -404,12 +404,13 @@ int64_t set_balance(GemmArgs &args, int64_t tiles, int64_t n_seg, int64_t G_max,
 }
 
 // Balanced-schedule launches spin on a flag written by a lower-indexed CTA (epi_take_prefix).  0 = plain launch (relies on
-// in-order block dispatch), 1 = cooperative launch instead of PDL, 2 = cooperative + PDL.  HEAL_COOP overrides (debug).
+// in-order block dispatch), 1 = cooperative launch instead of PDL, 2 = cooperative + PDL (the default: measured at no cost on
+// the headline GEMM).  HEAL_COOP overrides (debug).
 int coop_mode()
 {
     static const int mode = [] {
         const char *e = std::getenv("HEAL_COOP");
-        return e ? std::atoi(e) : 0;
+        return e ? std::atoi(e) : 2;
     }();
     return mode;
 }
@@ -545,7 +546,7 @@ int launch_gemm2_cfg(int64_t M, int64_t N, int64_t K, const void *A_hi, const vo
     return HEAL_OK;
 }
 
-inline bool needs_ext(const OutArgs &out) { return out.hi != nullptr || out.accumulate != 0 || out.scale != 1.0f || out.C == nullptr; }
+inline bool needs_ext(const OutArgs &out) { return out.hi != nullptr || out.accumulate != 0 || out.silu != 0 || out.scale != 1.0f || out.C == nullptr; }
 
 template <bool B_MN>
 int launch_gemm2_np(int nprod, int64_t M, int64_t N, int64_t K, const void *A_hi, const void *A_lo, int64_t lda,
@@ -850,7 +851,8 @@ int forced_kernel()
 
 int validate_mode(uint32_t mode, int *nprod, bool *b_nk)
 {
-    if (mode & ~(HEAL_MODE_PRODUCTS_MASK | HEAL_B_NK | HEAL_B_STATIC | HEAL_LO_SCALED)) return HEAL_ERR_UNSUPPORTED_MODE;
+    if (mode & ~(HEAL_MODE_PRODUCTS_MASK | HEAL_B_NK | HEAL_B_STATIC | HEAL_LO_SCALED | HEAL_EPI_SILU_MUL | HEAL_EPI_ACCUMULATE))
+        return HEAL_ERR_UNSUPPORTED_MODE;
     const uint32_t p = mode & HEAL_MODE_PRODUCTS_MASK;
     if (p < 1 || p > 4) return HEAL_ERR_UNSUPPORTED_MODE;
     if ((mode & HEAL_LO_SCALED) && p != 2) return HEAL_ERR_UNSUPPORTED_MODE;      // Eq. 10 as printed: two products only
@@ -865,20 +867,24 @@ int presplit_impl(int64_t M, int64_t N, int64_t K, const void *A_hi, const void 
                   cudaStream_t stream, const float *A32 = nullptr, int64_t lda32 = 0, bool *handled_out = nullptr)
 {
     if (handled_out) *handled_out = true;
-    if (K == 0) {                                       // empty sum: zeros in every requested output
-        if (out.C)
-            HEAL_CUDA(cudaMemset2DAsync(out.C, static_cast<size_t>(out.ldc) * 4, 0, static_cast<size_t>(N) * 4,
+    if (K == 0) {                                       // empty sum: zeros in every requested output (SiLU(0) * 0 = 0 as well)
+        const int64_t n_out = out.silu ? N / 2 : N;
+        if (out.C && !out.accumulate)                    // accumulate: C + 0 = C
+            HEAL_CUDA(cudaMemset2DAsync(out.C, static_cast<size_t>(out.ldc) * 4, 0, static_cast<size_t>(n_out) * 4,
                                         static_cast<size_t>(M), stream));
+        if (out.hi && out.accumulate)                    // planes of the unchanged residual
+            return launch_split(M, n_out, out.C, out.ldc, out.hi, out.lo, out.ld16, stream);
         if (out.hi) {
-            HEAL_CUDA(cudaMemset2DAsync(out.hi, static_cast<size_t>(out.ld16) * 2, 0, static_cast<size_t>(N) * 2,
+            HEAL_CUDA(cudaMemset2DAsync(out.hi, static_cast<size_t>(out.ld16) * 2, 0, static_cast<size_t>(n_out) * 2,
                                         static_cast<size_t>(M), stream));
-            HEAL_CUDA(cudaMemset2DAsync(out.lo, static_cast<size_t>(out.ld16) * 2, 0, static_cast<size_t>(N) * 2,
+            HEAL_CUDA(cudaMemset2DAsync(out.lo, static_cast<size_t>(out.ld16) * 2, 0, static_cast<size_t>(n_out) * 2,
                                         static_cast<size_t>(M), stream));
         }
         return HEAL_OK;
     }
     const int force = forced_kernel();
-    if ((M <= 64 && force != 1) || (force == 2 && M <= 64)) {
+    // (the SiLU-mul epilogue pairs adjacent columns inside one thread: large-M kernels only)
+    if (((M <= 64 && force != 1) || (force == 2 && M <= 64)) && !out.silu) {
         bool handled = false;
         const SmallIn in{A_hi, A_lo, lda, A32, lda32, b_static};
         int st = b_nk ? launch_small<false>(nprod, M, N, K, in, B_hi, B_lo, ldb, out, stream, &handled)
@@ -958,7 +964,7 @@ int scaled_two_gemms(int64_t M, int64_t N, int64_t K, const void *A_hi, const vo
     first.hi = first.lo = nullptr;
     const uint32_t bits = static_cast<uint32_t>(127 - scale_exp - HEAL_LO_SHIFT) << 23;
     memcpy(&first.scale, &bits, 4);
-    first.accumulate = 0;
+    // (with HEAL_EPI_ACCUMULATE the first GEMM already adds onto the residual held in C)
     int st = presplit_impl(M, N, K, A_lo, nullptr, lda, B, nullptr, ldb, first, 1, b_nk, b_static, stream);
     if (st) return st;
     OutArgs second = out;
@@ -1046,15 +1052,45 @@ int heal_split_scaled(int64_t rows, int64_t cols, const void *X, int64_t ldx, vo
                         static_cast<__half *>(lo), ld, static_cast<cudaStream_t>(stream), lo_shift);
 }
 
+int heal_rmsnorm_split(int64_t rows, int64_t cols, const void *X, int64_t ldx, const void *gamma, float eps, void *hi, void *lo,
+                       int64_t ld, void *Y, int64_t ldy, void *stream)
+{
+    if (rows < 0 || cols < 0 || ldx < cols || ld < cols || (Y && ldy < cols) || !(eps >= 0.0f)) return HEAL_ERR_INVALID_VALUE;
+    if (rows == 0 || cols == 0) return HEAL_OK;
+    if (!X || !hi || !lo) return HEAL_ERR_NULL_POINTER;
+    if (!aligned16(X) || !aligned16(hi) || !aligned16(lo) || !aligned16(gamma) || !aligned16(Y) || (ldx & 3) || (ld & 7) || (Y && (ldy & 3)))
+        return HEAL_ERR_MISALIGNED;
+    int st = ensure_init();
+    if (st) return st;
+    cudaLaunchConfig_t cfg = {};
+    const int64_t cap = static_cast<int64_t>(g.num_sms) * 8;
+    cfg.gridDim = dim3(static_cast<unsigned>(rows < cap ? rows : cap));
+    cfg.blockDim = dim3(256);
+    cfg.stream = static_cast<cudaStream_t>(stream);
+    cudaLaunchAttribute attr[3];
+    cfg.numAttrs = fill_attrs(attr, 1);
+    cfg.attrs = attr;
+    HEAL_CUDA(cudaLaunchKernelEx(&cfg, heal_rmsnorm_split_kernel, static_cast<const float *>(X), ldx, rows, cols,
+                                 static_cast<const float *>(gamma), eps, static_cast<__half *>(hi), static_cast<__half *>(lo), ld,
+                                 static_cast<float *>(Y), ldy));
+    g_launches.fetch_add(1);
+    return HEAL_OK;
+}
+
 // Output validation shared by the _ex entry points: builds the OutArgs of step E.
 static int make_out(int64_t M, int64_t N, void *C, int64_t ldc, void *C_hi, void *C_lo, int64_t ldc16, int scale_exp,
-                    heal::OutArgs *out)
+                    uint32_t mode, heal::OutArgs *out)
 {
+    const bool silu = (mode & HEAL_EPI_SILU_MUL) != 0, acc = (mode & HEAL_EPI_ACCUMULATE) != 0;
     if (scale_exp < -126 || scale_exp > 126) return HEAL_ERR_INVALID_VALUE;
-    if ((C || !C_hi) && ldc < N) return HEAL_ERR_INVALID_VALUE;
-    if ((C_hi || C_lo) && ldc16 < N) return HEAL_ERR_INVALID_VALUE;
+    if (silu && (N & 1)) return HEAL_ERR_INVALID_VALUE;                    // (gate, up) column pairs
+    if (silu && (mode & HEAL_LO_SCALED)) return HEAL_ERR_UNSUPPORTED_MODE; // the two-GEMM form sums raw GEMM outputs
+    const int64_t n_out = silu ? N / 2 : N;
+    if ((C || !C_hi) && ldc < n_out) return HEAL_ERR_INVALID_VALUE;
+    if ((C_hi || C_lo) && ldc16 < n_out) return HEAL_ERR_INVALID_VALUE;
     if (M == 0 || N == 0) return HEAL_OK;
     if (!C && !C_hi) return HEAL_ERR_NULL_POINTER;
+    if (acc && !C) return HEAL_ERR_NULL_POINTER;                           // the residual lives in C
     if ((C_hi == nullptr) != (C_lo == nullptr)) return HEAL_ERR_NULL_POINTER;
     if (C && (!aligned16(C) || (ldc & 3))) return HEAL_ERR_MISALIGNED;
     if (C_hi && (!aligned16(C_hi) || !aligned16(C_lo) || (ldc16 & 7))) return HEAL_ERR_MISALIGNED;
@@ -1068,7 +1104,8 @@ static int make_out(int64_t M, int64_t N, void *C, int64_t ldc, void *C_hi, void
     float sc;
     memcpy(&sc, &bits, 4);
     out->scale = sc;
-    out->accumulate = 0;
+    out->accumulate = acc ? 1 : 0;
+    out->silu = silu ? 1 : 0;
     return HEAL_OK;
 }
 
@@ -1084,7 +1121,7 @@ int heal_gemm_presplit_ex(int64_t M, int64_t N, int64_t K, const void *A_hi, con
     if (M > 0x7fffff00 || N > 0x7fffff00 || K > 0x7fffff00) return HEAL_ERR_INVALID_VALUE;
     if (lda < K || ldb < (b_nk ? K : N)) return HEAL_ERR_INVALID_VALUE;
     heal::OutArgs out = {};
-    st = make_out(M, N, C, ldc, C_hi, C_lo, ldc16, scale_exp, &out);
+    st = make_out(M, N, C, ldc, C_hi, C_lo, ldc16, scale_exp, mode, &out);
     if (st) return st;
     if (M == 0 || N == 0) return HEAL_OK;
     if (K > 0) {
@@ -1121,7 +1158,7 @@ int heal_gemm_ex(int64_t M, int64_t N, int64_t K, const void *A, int64_t lda, co
     if (M > 0x7fffff00 || N > 0x7fffff00 || K > 0x7fffff00) return HEAL_ERR_INVALID_VALUE;
     if (lda < K || ldb < (b_nk ? K : N)) return HEAL_ERR_INVALID_VALUE;
     heal::OutArgs out = {};
-    st = make_out(M, N, C, ldc, C_hi, C_lo, ldc16, scale_exp, &out);
+    st = make_out(M, N, C, ldc, C_hi, C_lo, ldc16, scale_exp, mode, &out);
     if (st) return st;
     if (M == 0 || N == 0) return HEAL_OK;
     const bool b_f32 = nprod >= 3;
@@ -1136,7 +1173,7 @@ int heal_gemm_ex(int64_t M, int64_t N, int64_t K, const void *A, int64_t lda, co
     if (K == 0) return presplit_impl(M, N, K, nullptr, nullptr, lda, nullptr, nullptr, ldb, out, nprod, b_nk, b_static, stream);
     static const bool no_fused = std::getenv("HEAL_NO_FUSED") != nullptr;          // debug only
     const bool lo_scaled = (mode & HEAL_LO_SCALED) != 0;
-    if (M <= 16 && K <= 8192 && !b_f32 && !no_fused && !lo_scaled && forced_kernel() != 1) {
+    if (M <= 16 && K <= 8192 && !b_f32 && !no_fused && !lo_scaled && !out.silu && forced_kernel() != 1) {
         // decode shapes (M <= 16) with FP16 weights: step S runs inside the GEMM kernel (no planes, one launch);
         // above that -- and for long K, where a CTA converts many k-tiles -- the in-kernel conversion costs more
         // than the split launch it saves (measured: M = 1, K = 14336 31 vs 28 us)
@@ -1188,6 +1225,7 @@ int heal_gemm_host(int64_t M, int64_t N, int64_t K, const void *A_host, int64_t 
     int st = validate_mode(mode, &nprod, &b_nk);
     if (st) return st;
     if (M < 0 || N < 0 || K < 0) return HEAL_ERR_INVALID_VALUE;
+    if (mode & (HEAL_EPI_SILU_MUL | HEAL_EPI_ACCUMULATE)) return HEAL_ERR_UNSUPPORTED_MODE;     // device entry points only
     if (lda < K || ldc < N || ldb < (b_nk ? K : N)) return HEAL_ERR_INVALID_VALUE;
     if (M == 0 || N == 0) return HEAL_OK;
     if (!C_host || (K > 0 && (!A_host || !B_host))) return HEAL_ERR_NULL_POINTER;

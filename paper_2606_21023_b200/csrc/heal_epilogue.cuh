@@ -19,8 +19,10 @@ struct OutArgs {
     __half *hi, *lo;      // FP16 M x N planes, pitch ld16 (elements, % 8 == 0); null = not requested
     int64_t ld16;
     float scale;          // 2^-p, exactly representable; 1.0f = none
-    int accumulate;       // C += scaled result (needs C): second launch of the scaled-lo variant, which forms
-                          // C = 2^-10 (lo'.W) + hi.W as the paper's two GEMMs summed into one FP32 output
+    int accumulate;       // C += scaled result (needs C): the residual add "A_i + GEMM(...)" of Algorithm 1 with
+                          // C holding A_i (HEAL_EPI_ACCUMULATE), and the second launch of the two-GEMM scaled-lo form
+    int silu;             // HEAL_EPI_SILU_MUL: the GEMM's columns are (gate, up) pairs -- column 2j = g_j, 2j+1 = u_j -- and the
+                          // outputs (C and/or planes, N/2 columns wide) receive SiLU(g_j) * u_j; large-M kernels only
 };
 
 // The output mode is uniform for the launch.  The store loops of the kernels are fully unrolled, run once per CTA (cold
@@ -38,7 +40,7 @@ struct EmitTag {
 __device__ __forceinline__ OutArgs pin_out(const OutArgs &o)
 {
     OutArgs r = o;
-    asm volatile("" : "+l"(r.C), "+l"(r.ldc), "+l"(r.hi), "+l"(r.lo), "+l"(r.ld16), "+f"(r.scale), "+r"(r.accumulate));
+    asm volatile("" : "+l"(r.C), "+l"(r.ldc), "+l"(r.hi), "+l"(r.lo), "+l"(r.ld16), "+f"(r.scale), "+r"(r.accumulate), "+r"(r.silu));
     return r;
 }
 // f(out, fast): `fast` is EmitTag<true> when only the FP32 matrix is written and nothing is accumulated
@@ -46,14 +48,55 @@ template <class F>
 __device__ __forceinline__ void emit_dispatch(const OutArgs &o_, F &&f)
 {
     const OutArgs o = pin_out(o_);
-    if (o.hi == nullptr && o.accumulate == 0) f(o, EmitTag<true>{});
+    if (o.hi == nullptr && o.accumulate == 0 && o.silu == 0) f(o, EmitTag<true>{});
     else f(o, EmitTag<false>{});
 }
 
 // general forms, out of line, arguments by value (the caller's OutArgs stays in registers); v is already scaled
-__device__ __noinline__ void emit4_any(float *C, int64_t ldc, __half *hi, __half *lo, int64_t ld16, int accumulate,
+// SiLU(g) * u in FP32: g / (1 + exp(-g)) * u with IEEE division (expf: <= 2 ulp; the parity tests bound the result
+// against the FP64 definition oracle/heal_fusions.c F2)
+__device__ __forceinline__ float silu_mul(float g, float u)
+{
+    return __fmul_rn(__fdiv_rn(g, __fadd_rn(1.0f, expf(-g))), u);
+}
+
+// two output columns col2, col2+1 (col2 even) of one row, N2 output columns in all: FP32 and/or hi/lo planes
+__device__ __forceinline__ void emit2_out(float *C, int64_t ldc, __half *hi, __half *lo, int64_t ld16, int accumulate,
+                                          int64_t row, int col2, float a, float b, int N2)
+{
+    const bool full = col2 + 1 < N2;
+    if (col2 >= N2) return;
+    if (C) {
+        float *c = C + row * ldc + col2;
+        if (accumulate) {
+            a = __fadd_rn(c[0], a);
+            if (full) b = __fadd_rn(c[1], b);
+        }
+        if (full) *reinterpret_cast<float2 *>(c) = make_float2(a, b);
+        else c[0] = a;
+    }
+    if (hi) {
+        uint32_t h, l;
+        split2(a, b, h, l);
+        __half *ph = hi + row * ld16 + col2, *pl = lo + row * ld16 + col2;
+        if (full) {
+            *reinterpret_cast<uint32_t *>(ph) = h;
+            *reinterpret_cast<uint32_t *>(pl) = l;
+        } else {
+            *reinterpret_cast<uint16_t *>(ph) = static_cast<uint16_t>(h);
+            *reinterpret_cast<uint16_t *>(pl) = static_cast<uint16_t>(l);
+        }
+    }
+}
+
+// general forms, out of line, arguments by value (the caller's OutArgs stays in registers); v is already scaled
+__device__ __noinline__ void emit4_any(float *C, int64_t ldc, __half *hi, __half *lo, int64_t ld16, int accumulate, int silu,
                                        int64_t row, int col, float4 v, int N)
 {
+    if (silu) {                                  // columns col..col+3 = (g, u, g, u) -> output columns col/2, col/2 + 1
+        emit2_out(C, ldc, hi, lo, ld16, accumulate, row, col >> 1, silu_mul(v.x, v.y), silu_mul(v.z, v.w), N >> 1);
+        return;
+    }
     const bool full = col + 3 < N;
     if (C) {
         float *c = C + row * ldc + col;
@@ -139,7 +182,7 @@ __device__ __forceinline__ void emit4(const OutArgs &o, int64_t row, int col, fl
             if (col + 2 < N) c[2] = v.z;
         }
     } else {
-        emit4_any(o.C, o.ldc, o.hi, o.lo, o.ld16, o.accumulate, row, col, v, N);
+        emit4_any(o.C, o.ldc, o.hi, o.lo, o.ld16, o.accumulate, o.silu, row, col, v, N);
     }
 }
 

@@ -498,6 +498,129 @@ def test_small_m_single_cta_panels_tmem_ring(hb, inputs, M, N, K, nprod, b_nk):
         hb.debug_force_kernel(0)
 
 
+# --------------------------------------------------------------------------------- NEXT-3 fusions
+@pytest.mark.parametrize("rows,cols,pad,use_gamma", [(1, 4096, 0, True), (5, 100, 4, True), (64, 1000, 0, False), (300, 14336, 8, True), (3, 7, 1, True)])
+def test_rmsnorm_split_vs_oracle(hb, oracle, inputs, rows, cols, pad, use_gamma):
+    """heal_rmsnorm_split: the FP32 normalised row within a few FP32 roundings of the FP64 definition F1 (sum of squares in
+    FP32: <= cols * 2^-24 relative on the mean, halved by the root; three more roundings for 1/sqrt and the two products),
+    the planes bit-exactly the oracle's split O2 of that FP32 row, and each row independent of the others."""
+    X = inputs.activations(rows, cols, seed=51, outliers=True)
+    gam = inputs.activations(1, cols, seed=52)[0] * 0.1 + 1.0 if use_gamma else None
+    Xd = dev_padded(X, pad)
+    gd = None if gam is None else dev(gam)
+    hi, lo, Y = hb.heal_rmsnorm_split(Xd, gd, eps=1e-6, want_y=True)
+    torch.cuda.synchronize()
+    Yc = Y.cpu().numpy()
+    ref = oracle.rmsnorm_f64(X, gamma=gam, eps=1e-6)
+    tol = (cols * 2.0 ** -25 + 4 * 2.0 ** -24) * np.abs(ref) + 1e-30
+    assert np.all(np.abs(Yc - ref) <= tol), float(np.max(np.abs(Yc - ref) / (np.abs(ref) + 1e-30)))
+    oh, ol = oracle.split(np.ascontiguousarray(Yc))
+    assert np.array_equal(hi.cpu().numpy().view(np.uint16), oh) and np.array_equal(lo.cpu().numpy().view(np.uint16), ol)
+    # without the FP32 output: same planes; a single row submitted alone: same bits
+    h2, l2, none = hb.heal_rmsnorm_split(Xd, gd, eps=1e-6)
+    assert none is None and torch.equal(h2, hi) and torch.equal(l2, lo)
+    r = rows // 2
+    h3, l3, _ = hb.heal_rmsnorm_split(Xd[r:r + 1], gd, eps=1e-6)
+    assert torch.equal(h3, hi[r:r + 1]) and torch.equal(l3, lo[r:r + 1])
+
+
+@pytest.mark.parametrize("M,N,K,nprod", [(300, 520, 1024, 2), (2048, 1024, 512, 2), (128, 1032, 4096, 2), (8, 264, 1024, 2),
+                                         (64, 2050, 520, 3), (1300, 4104, 2056, 2)])
+def test_silu_mul_and_accumulate_epilogue(hb, oracle, inputs, M, N, K, nprod):
+    """HEAL_EPI_SILU_MUL: every output is SiLU(g) * u of the (gate, up) column pairs of the GEMM result -- checked against
+    the FP64 definition F2 applied to the plain FP32 GEMM output of the same call (FP32 evaluation: expf <= 2 ulp, one
+    add, one IEEE division, one product: 8 * 2^-24 relative, plus the absolute term of exp(-g) for large negative g);
+    the planes are bit-exactly the split of the FP32 activations.  HEAL_EPI_ACCUMULATE: C_in + result, one FP32 RN add.
+    Shapes cover both large-M kernel families, the balanced schedule, ordered split-K, M <= 64 and a ragged last pair."""
+    A = dev(inputs.activations(M, K, seed=61, outliers=True))
+    B = dev(inputs.weights_f32(K, N, seed=61, dist="normal", sigma=0.05) if nprod >= 3 else inputs.weights_f16(K, N, seed=61, sigma=0.05))
+    plain = hb.heal_gemm(A, B, nprod)
+    act, ahi, alo = hb.heal_gemm_ex(A, B, nprod | hb.EPI_SILU_MUL)
+    torch.cuda.synchronize()
+    assert act.shape == (M, N // 2)
+    ref = oracle.silu_mul_f64(plain.cpu().numpy().astype(np.float64))
+    got = act.cpu().numpy()
+    g = plain.cpu().numpy().astype(np.float64)[:, 0::2]
+    u = np.abs(plain.cpu().numpy().astype(np.float64)[:, 1::2])
+    tol = 8 * 2.0 ** -24 * np.abs(ref) + 4 * 2.0 ** -24 * np.abs(g) * np.exp(-np.abs(g)) * u + 1e-37
+    assert np.all(np.abs(got - ref) <= tol), float(np.max(np.abs(got - ref) / (np.abs(ref) + 1e-30)))
+    oh, ol = oracle.split(got)
+    assert np.array_equal(ahi.cpu().numpy().view(np.uint16), oh) and np.array_equal(alo.cpu().numpy().view(np.uint16), ol)
+    # planes only (no FP32 matrix), and the 2^-p scale applies to the GEMM result before the activation
+    _, h2, l2 = hb.heal_gemm_ex(A, B, nprod | hb.EPI_SILU_MUL, want_c=False)
+    assert torch.equal(h2, ahi) and torch.equal(l2, alo)
+    sc, _, _ = hb.heal_gemm_ex(A, B, nprod | hb.EPI_SILU_MUL, scale_exp=3, want_planes=False)
+    ref_s = oracle.silu_mul_f64((plain.cpu().numpy() * np.float32(0.125)).astype(np.float64))
+    assert np.all(np.abs(sc.cpu().numpy() - ref_s) <= 8 * 2.0 ** -24 * np.abs(ref_s) + 4 * 2.0 ** -24 * np.abs(g / 8) * np.exp(-np.abs(g / 8)) * u / 8 + 1e-37)
+    # residual add: bit-exact FP32 sum, through heal_gemm and with chained planes
+    R = dev(inputs.activations(M, N, seed=62))
+    C = R.clone()
+    hb.heal_gemm(A, B, nprod | hb.EPI_ACCUMULATE, C=C)
+    assert torch.equal(C, R + plain)
+    C2 = R.clone()
+    _, rh, rl = hb.heal_gemm_ex(A, B, nprod | hb.EPI_ACCUMULATE, C=C2)
+    torch.cuda.synchronize()
+    assert torch.equal(C2, C)
+    oh, ol = oracle.split(C.cpu().numpy())
+    assert np.array_equal(rh.cpu().numpy().view(np.uint16), oh) and np.array_equal(rl.cpu().numpy().view(np.uint16), ol)
+
+
+def test_fused_epilogue_errors(hb):
+    L = hb.lib()
+    A = torch.zeros(8, 64, device="cuda"); W = torch.zeros(64, 66, device="cuda", dtype=torch.float16)
+    C = torch.zeros(8, 72, device="cuda")
+    st = lambda mode, N=66, ldc=72, Cp=C.data_ptr(): L.heal_gemm(8, N, 64, A.data_ptr(), 64, W.data_ptr(), 72 if N > 66 else 66 + 6, Cp, ldc, mode, None)
+    assert L.heal_gemm(8, 65, 64, A.data_ptr(), 64, W.data_ptr(), 72, C.data_ptr(), 72, 2 | hb.EPI_SILU_MUL, None) == 1      # odd N
+    assert L.heal_gemm(8, 64, 64, A.data_ptr(), 64, W.data_ptr(), 72, C.data_ptr(), 28, 2 | hb.EPI_SILU_MUL, None) == 1      # ldc < N/2
+    assert L.heal_gemm(8, 64, 64, A.data_ptr(), 64, W.data_ptr(), 72, C.data_ptr(), 32, 2 | hb.EPI_SILU_MUL | hb.LO_SCALED, None) == 4
+    assert L.heal_gemm_ex(8, 64, 64, A.data_ptr(), 64, W.data_ptr(), 72, None, 0, C.data_ptr(), C.data_ptr(), 72, 0,
+                          2 | hb.EPI_ACCUMULATE, None) == 2                                                               # accumulate needs C
+    assert L.heal_gemm_host(8, 64, 64, A.data_ptr(), 64, W.data_ptr(), 72, C.data_ptr(), 72, 2 | hb.EPI_ACCUMULATE, None) == 4
+    assert L.heal_rmsnorm_split(4, 64, A.data_ptr(), 32, None, 1e-6, C.data_ptr(), C.data_ptr(), 64, None, 0, None) == 1   # ldx < cols
+    assert L.heal_rmsnorm_split(4, 64, None, 64, None, 1e-6, C.data_ptr(), C.data_ptr(), 64, None, 0, None) == 2
+    assert L.heal_rmsnorm_split(4, 64, A.data_ptr(), 64, None, -1.0, C.data_ptr(), C.data_ptr(), 64, None, 0, None) == 1
+    assert L.heal_rmsnorm_split(0, 64, None, 64, None, 1e-6, None, None, 64, None, 0, None) == 0
+    torch.cuda.synchronize()
+
+
+def test_mlp_chain_three_launches_vs_fp64_chain(hb, oracle, inputs):
+    """The MLP block of Algorithm 1 at Llama-3-8B size through the C ABI in three launches -- Norm -> split,
+    gate_up GEMM with the SiLU-mul epilogue emitting the activation planes, down GEMM adding onto the residual:
+        H_out = H + GEMM(SiLU(g) (.) u, W_down),   g, u = GEMM(RMSNorm(H), W_gate_up)
+    against the FP64 chain F1 -> F3 -> F2 -> F3 -> F4 on sampled rows: normwise error of the GEMM contribution
+    ||(H_out - H) - ref||_F / (||act||_F ||W_down||_F) <= 2e-6 (the north_star gate, applied to the last GEMM of the chain)."""
+    M, D, FF = 2048, 4096, 14336
+    H = inputs.activations(M, D, seed=71, outliers=True)
+    gam = (inputs.activations(1, D, seed=72)[0] * 0.1 + 1.0).astype(np.float32)
+    Wg = inputs.weights_f16(D, FF, seed=73)                   # gate projection
+    Wu = inputs.weights_f16(D, FF, seed=74)                   # up projection
+    Wgu = np.empty((D, 2 * FF), np.float16)
+    Wgu[:, 0::2] = Wg
+    Wgu[:, 1::2] = Wu
+    Wd = inputs.weights_f16(FF, D, seed=75)
+    Hd, gd, Wgud, Wdd = dev(H), dev(gam), dev(Wgu), dev(Wd)
+    out = Hd.clone()
+    n0 = hb.launch_count()
+    xh, xl, _ = hb.heal_rmsnorm_split(Hd, gd, eps=1e-6)
+    _, ah, al = hb.heal_gemm_presplit_ex(xh, xl, Wgud, None, 2 | hb.EPI_SILU_MUL, want_c=False)
+    hb.heal_gemm_presplit_ex(ah, al, Wdd, None, 2 | hb.EPI_ACCUMULATE, C=out, want_planes=False)
+    torch.cuda.synchronize()
+    assert hb.launch_count() - n0 == 3
+    rows = [0, 127, 128, 1000, 2047]
+    y = oracle.rmsnorm_f64(H[rows], gamma=gam, eps=1e-6)
+    gu = oracle.gemm_dd(y, Wgu)
+    act = oracle.silu_mul_f64(gu)
+    ref = oracle.gemm_dd(act, Wd)
+    full = oracle.add_f64(np.ascontiguousarray(H[rows]), ref)
+    got = out.cpu().numpy()[rows].astype(np.float64)
+    e = np.linalg.norm((got - H[rows].astype(np.float64)) - ref) / (np.linalg.norm(act) * oracle.fro_b(Wd))
+    assert e <= GATE, e
+    assert np.all(np.abs(got - full) <= 2.0 ** -23 * np.abs(full) + 4e-6 * np.sqrt((act ** 2).sum(1, keepdims=True)) * np.sqrt((Wd.astype(np.float64) ** 2).sum(0, keepdims=True)))
+    # the intermediate activation planes reconstruct SiLU(g) * u to FP32-level accuracy
+    a32 = ah.float().cpu().numpy()[rows].astype(np.float64) + al.float().cpu().numpy()[rows].astype(np.float64)
+    assert np.linalg.norm(a32 - act) <= 1e-5 * np.linalg.norm(act)
+
+
 def test_scaled_split_bit_exact(hb, oracle, inputs):
     """heal_split_scaled(lo_shift = 10): lo = r16((x - hi) * 2^10), the paper's h = h_hi + h_lo / 2^10,
     bit for bit against the oracle's integer split, including magnitudes where the unscaled residual underflows."""

@@ -359,3 +359,83 @@ def test_metric_rows_list_and_padded_operands_vs_numpy(oracle):
     L = oracle.lib()
     assert abs(L.oracle_sumsq_f16(K, N, Bbuf.ctypes.data, N + 8) - float((B.astype(np.float64) ** 2).sum())) <= 1e-14 * float((B.astype(np.float64) ** 2).sum())
     assert abs(L.oracle_sumsq_f32(M, K, Abuf.ctypes.data, K + 4) - float((A.astype(np.float64) ** 2).sum())) <= 1e-13 * float((A.astype(np.float64) ** 2).sum())
+
+
+# ---------------------------------------------------------------- F1-F4: steps around the GEMMs (oracle/heal_fusions.c)
+def test_f1_rmsnorm_hand_values_and_invariants(oracle):
+    """F1 ("Norm"; A17).  Hand-worked: x = (3, 4): mean square 12.5, so y = x / sqrt(12.5) =
+    (0.6 sqrt 2, 0.8 sqrt 2); with gamma = (2, -1): (1.2 sqrt 2, -0.8 sqrt 2).  Invariants a wrong formula breaks: unit mean
+    square for gamma = 1, eps = 0 (fails for LayerNorm-style mean subtraction or a sum instead of a mean), invariance under
+    scaling the row (fails if eps or the 1/K is misplaced), a constant row maps to sign(c) gamma, the zero row with eps > 0 maps
+    to 0, eps enters under the root (x = (1, 1), eps = 3: y = 1/2), per-row statistics and per-column gamma (fails if
+    transposed), padding ignored."""
+    r2 = np.sqrt(2.0)
+    X = np.array([[3.0, 4.0]], np.float32)
+    assert np.allclose(oracle.rmsnorm_f64(X), [[0.6 * r2, 0.8 * r2]], rtol=1e-15, atol=0)
+    assert np.allclose(oracle.rmsnorm_f64(X, gamma=[2.0, -1.0]), [[1.2 * r2, -0.8 * r2]], rtol=1e-15, atol=0)
+    assert np.allclose(oracle.rmsnorm_f64(np.ones((1, 2), np.float32), eps=3.0), [[0.5, 0.5]], rtol=1e-15, atol=0)
+    rng = np.random.default_rng(11)
+    buf = rng.standard_normal((5, 40)).astype(np.float32)
+    buf[:, 37:] = 1e6                                            # padding
+    Xp = buf[:, :37]
+    Y = oracle.rmsnorm_f64(Xp)
+    assert np.allclose((Y ** 2).mean(axis=1), 1.0, rtol=1e-14)
+    assert np.allclose(oracle.rmsnorm_f64(np.ascontiguousarray(Xp) * np.float32(8.0)), Y, rtol=1e-15)      # exact power-of-two scaling
+    gam = rng.standard_normal(37).astype(np.float32)
+    Yg = oracle.rmsnorm_f64(Xp, gamma=gam)
+    assert np.allclose(Yg, Y * gam.astype(np.float64)[None, :], rtol=1e-15)
+    Xc = np.full((2, 7), -2.5, np.float32)
+    assert np.allclose(oracle.rmsnorm_f64(Xc, gamma=np.arange(1, 8)), -np.arange(1, 8, dtype=np.float64)[None, :].repeat(2, 0), rtol=1e-15)
+    assert np.array_equal(oracle.rmsnorm_f64(np.zeros((1, 4), np.float32), eps=1e-6), np.zeros((1, 4)))
+    # rows are independent: a row with 100x the magnitude does not change its neighbour
+    X2 = np.ascontiguousarray(Xp[:2]).copy()
+    X2[1] *= 100
+    assert np.array_equal(oracle.rmsnorm_f64(X2)[0], Y[0])
+
+
+def test_f2_silu_mul_closed_forms_and_interleaving(oracle):
+    """F2 (PAPER.md:76 "SiLU(g) (.) u"; DESIGN.md A18).  Closed forms: silu(0) = 0; silu(ln 3) = 3/4 ln 3 (sigmoid(ln 3) = 3/4);
+    silu(-ln 3) = -1/4 ln 3; silu(x) - silu(-x) = x; large x: silu(x) -> x, silu(-x) -> 0.  Interleaving: gate is the EVEN
+    column, up the ODD one (swapping them, or reading g and u from two halves of the row, fails the asymmetric cases)."""
+    l3 = np.log(3.0)
+    C = np.array([[0.0, 5.0, l3, 2.0, -l3, 4.0, 40.0, 0.5, -40.0, 7.0]])
+    H = oracle.silu_mul_f64(C)
+    assert H.shape == (1, 5)
+    assert np.allclose(H[0, :3], [0.0, 0.75 * l3 * 2.0, -0.25 * l3 * 4.0], rtol=1e-15, atol=0)
+    assert abs(H[0, 3] - 20.0) < 1e-14 and abs(H[0, 4]) < 1e-14
+    rng = np.random.default_rng(12)
+    g = rng.standard_normal((6, 9)) * 3
+    Cp = np.empty((6, 18)); Cp[:, 0::2] = g; Cp[:, 1::2] = 1.0
+    Cm = np.empty((6, 18)); Cm[:, 0::2] = -g; Cm[:, 1::2] = 1.0
+    assert np.allclose(oracle.silu_mul_f64(Cp) - oracle.silu_mul_f64(Cm), g, rtol=1e-14, atol=1e-15)
+    # u scales linearly, g does not; rows keep their place
+    u = rng.standard_normal((6, 9))
+    Cu = Cp.copy(); Cu[:, 1::2] = u
+    assert np.allclose(oracle.silu_mul_f64(Cu), oracle.silu_mul_f64(Cp) * u, rtol=1e-15)
+    assert np.array_equal(oracle.silu_mul_f64(Cu[2:3]), oracle.silu_mul_f64(Cu)[2:3])
+
+
+def test_f3_gemm_dd_matches_o1_and_integers(oracle, inputs):
+    """F3 = O1's definition with a double first operand: bit-identical to O1 when the doubles are FP32 values (same sums in
+    the same order), exact on integer matrices, honours b_nk, row lists and padded B; asymmetric shapes catch a transposed
+    operand.  F4: the residual add."""
+    A = inputs.activations(9, 50, seed=3)
+    W = inputs.weights_f16(50, 24, seed=3, ld=32)
+    B32 = inputs.weights_f32(50, 24, seed=3, ld=28)
+    Ad = A.astype(np.float64)
+    assert np.array_equal(oracle.gemm_dd(Ad, W), oracle.gemm_f64(A, W))
+    assert np.array_equal(oracle.gemm_dd(Ad, B32), oracle.gemm_f64(A, B32))
+    rows = [7, 0, 3]
+    assert np.array_equal(oracle.gemm_dd(Ad, W, rows=rows), oracle.gemm_f64(A, W)[rows])
+    Wnk = inputs.weights_f16(50, 24, seed=3, nk=True)
+    assert np.array_equal(oracle.gemm_dd(Ad, Wnk, b_nk=True), oracle.gemm_f64(A, W))
+    Ai = inputs.integers(5, 33, -8, 8, seed=1)
+    Bi = inputs.integers(33, 7, -8, 8, seed=2)
+    assert np.array_equal(oracle.gemm_dd(Ai.astype(np.float64), Bi), (Ai.astype(np.int64) @ Bi.astype(np.int64)).astype(np.float64))
+    # a genuinely double operand: against numpy float64 matmul
+    Ah = Ad + 1e-9 * np.arange(Ad.size).reshape(Ad.shape)
+    ref = Ah @ W.astype(np.float64)
+    assert np.allclose(oracle.gemm_dd(Ah, W), ref, rtol=1e-13, atol=1e-14)
+    Y = np.arange(18, dtype=np.float64).reshape(3, 6) * 0.25
+    Xb = np.arange(24, dtype=np.float32).reshape(3, 8)
+    assert np.array_equal(oracle.add_f64(Xb[:, :6], Y), Xb[:, :6].astype(np.float64) + Y)
