@@ -525,7 +525,7 @@ def test_rmsnorm_split_vs_oracle(hb, oracle, inputs, rows, cols, pad, use_gamma)
 
 
 @pytest.mark.parametrize("M,N,K,nprod", [(300, 520, 1024, 2), (2048, 1024, 512, 2), (128, 1032, 4096, 2), (8, 264, 1024, 2),
-                                         (64, 2050, 520, 3), (1300, 4104, 2056, 2)])
+                                         (64, 2056, 520, 3), (1300, 4104, 2056, 2)])
 def test_silu_mul_and_accumulate_epilogue(hb, oracle, inputs, M, N, K, nprod):
     """HEAL_EPI_SILU_MUL: every output is SiLU(g) * u of the (gate, up) column pairs of the GEMM result -- checked against
     the FP64 definition F2 applied to the plain FP32 GEMM output of the same call (FP32 evaluation: expf <= 2 ulp, one
@@ -563,6 +563,26 @@ def test_silu_mul_and_accumulate_epilogue(hb, oracle, inputs, M, N, K, nprod):
     assert torch.equal(C2, C)
     oh, ol = oracle.split(C.cpu().numpy())
     assert np.array_equal(rh.cpu().numpy().view(np.uint16), oh) and np.array_equal(rl.cpu().numpy().view(np.uint16), ol)
+
+
+def test_silu_mul_ragged_last_pair(hb, oracle, inputs):
+    """N = 522: the last group of four GEMM columns holds a single (gate, up) pair; N/2 = 261 outputs in padded buffers."""
+    M, N, K = 200, 522, 1024
+    A = dev(inputs.activations(M, K, seed=63))
+    W = dev_padded(inputs.weights_f16(K, N, seed=63, sigma=0.05), 6)
+    plain = hb.heal_gemm(A, W, 2, C=torch.zeros(M, 524, device="cuda")[:, :N])
+    C = torch.full((M, 264), 7.0, device="cuda")
+    Ch = torch.full((M, 264), 7.0, device="cuda", dtype=torch.float16)
+    Cl = torch.full((M, 264), 7.0, device="cuda", dtype=torch.float16)
+    hb.heal_gemm_ex(A, W, 2 | hb.EPI_SILU_MUL, C=C[:, :261], C_hi=Ch[:, :261], C_lo=Cl[:, :261])
+    torch.cuda.synchronize()
+    ref = oracle.silu_mul_f64(plain.cpu().numpy().astype(np.float64))
+    got = C.cpu().numpy()
+    assert np.all(got[:, 261:] == 7.0) and np.all(Ch.cpu().numpy()[:, 261:] == 7.0) and np.all(Cl.cpu().numpy()[:, 261:] == 7.0)
+    assert np.all(np.abs(got[:, :261] - ref) <= 8 * 2.0 ** -24 * np.abs(ref) + 1e-9)
+    oh, ol = oracle.split(np.ascontiguousarray(got[:, :261]))
+    assert np.array_equal(np.ascontiguousarray(Ch.cpu().numpy()[:, :261]).view(np.uint16), oh)
+    assert np.array_equal(np.ascontiguousarray(Cl.cpu().numpy()[:, :261]).view(np.uint16), ol)
 
 
 def test_fused_epilogue_errors(hb):
