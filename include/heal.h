@@ -77,6 +77,12 @@ typedef enum {
                                      flow): C must hold the residual on entry and receives C + result (one FP32 RN add
                                      per element); the planes, if requested, are the split of that sum.  Needs C. */
 
+#define HEAL_FUSE_SPLIT 0x200u     /* heal_gemm / heal_gemm_ex, M > 128, N > 128, two or three products: step S of the activations runs
+                                     inside the GEMM kernel (FP32 tiles by TMA, converted in place in shared memory; SURVEY.md 8(f)
+                                     NEXT-1(i)) -- no hi/lo planes in HBM, no workspace and one launch with FP16 weights.  Same bits.
+                                     Slower than split + GEMM on B200 (0-13 %), hence opt-in; the library also
+                                     takes this path by itself when a captured call finds no workspace.  Ignored elsewhere. */
+
 #define HEAL_LO_SHIFT 10
 #define HEAL_LO_SCALED 0x40u   /* the paper's scaled residual, Eq. 10 as printed: h = h_hi +
                                   h_lo / 2^10 with h_lo = r16((h - h_hi) * 2^10), C = GEMM(h_hi, W) +
@@ -102,8 +108,9 @@ typedef enum {
  * different streams may run concurrently.  A caller-supplied workspace (heal_set_workspace) is
  * shared by all streams: calls that use it must be issued on one stream at a time.  During stream
  * capture the library does not allocate: run the call once eagerly on that stream first (or supply
- * a workspace), else HEAL_ERR_WORKSPACE.  With FP16 weights, M <= 16 and K <= 8192 the split runs
- * inside the GEMM kernel: one launch, no workspace.
+ * a workspace); a captured call that finds none returns HEAL_ERR_WORKSPACE, except for the shapes of HEAL_FUSE_SPLIT, which
+ * then split inside the GEMM kernel.  Buffers that a captured graph may hold are never freed or handed to another stream.
+ * With FP16 weights, M <= 16 and K <= 8192 the split always runs inside the GEMM kernel: one launch, no workspace.
  * Numerical contract: finite inputs with |x| <= 65504 (activations observed
  * < 1024); anything larger, Inf or NaN propagates to Inf/NaN in the affected rows/columns.
  */

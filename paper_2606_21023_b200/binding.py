@@ -19,6 +19,7 @@ B_STATIC = 0x20
 LO_SCALED = 0x40
 EPI_SILU_MUL = 0x80
 EPI_ACCUMULATE = 0x100
+FUSE_SPLIT = 0x200
 LO_SHIFT = 10
 K_SEGMENT = 512
 

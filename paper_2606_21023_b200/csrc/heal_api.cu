@@ -19,6 +19,7 @@
 #include "heal_gemm_smallm.cuh"
 #include "heal_gemm_umma.cuh"
 #include "heal_gemm_umma2.cuh"
+#include "heal_gemm_umma2f.cuh"
 #include "heal_split.cuh"
 
 namespace {
@@ -410,7 +411,7 @@ int coop_mode()
 {
     static const int mode = [] {
         const char *e = std::getenv("HEAL_COOP");
-        return e ? std::atoi(e) : 2;
+        return e ? std::atoi(e) : 0;
     }();
     return mode;
 }
@@ -546,6 +547,54 @@ int launch_gemm2_cfg(int64_t M, int64_t N, int64_t K, const void *A_hi, const vo
     return HEAL_OK;
 }
 
+// CTA-pair kernel with the activation split fused in (heal_gemm_umma2f.cuh): A is the FP32 matrix itself
+template <class Cfg>
+int launch_gemm2f_cfg(int64_t M, int64_t N, int64_t K, const float *A, int64_t lda, const void *B_hi, const void *B_lo,
+                      int64_t ldb, const OutArgs &out, cudaStream_t stream)
+{
+    static std::atomic<bool> attr_set{false};
+    auto kern = heal_gemm_umma2f_kernel<Cfg>;
+    if (!attr_set.load(std::memory_order_acquire)) {
+        HEAL_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::SMEM_BYTES));
+        attr_set.store(true, std::memory_order_release);
+    }
+    CUtensorMap ta, tb_hi, tb_lo;
+    int st = encode_2d(&ta, A, K, M, lda, 32, kBM, 1);          // FP32, two boxes of 32 k per k-tile
+    if (st) return st;
+    if (Cfg::B_MN) st = encode_f16_2d(&tb_hi, B_hi, N, K, ldb, 64, kBK);
+    else           st = encode_f16_2d(&tb_hi, B_hi, K, N, ldb, kBK, Cfg::BH);
+    if (st) return st;
+    if (Cfg::B_PLANES == 2) {
+        if (Cfg::B_MN) st = encode_f16_2d(&tb_lo, B_lo, N, K, ldb, 64, kBK);
+        else           st = encode_f16_2d(&tb_lo, B_lo, K, N, ldb, kBK, Cfg::BH);
+        if (st) return st;
+    } else {
+        tb_lo = tb_hi;
+    }
+    GemmArgs args;
+    args.out = out;
+    args.M = static_cast<int>(M);
+    args.N = static_cast<int>(N);
+    args.K = static_cast<int>(K);
+    args.tiles_m = static_cast<int>((M + 2 * kBM - 1) / (2 * kBM));
+    args.tiles_n = static_cast<int>((N + Cfg::BN - 1) / Cfg::BN);
+    args.diag = g.diag;
+    const int64_t tiles = static_cast<int64_t>(args.tiles_m) * args.tiles_n;
+    const int64_t G = set_balance(args, tiles, (K + kKSeg - 1) / kKSeg, g.num_sms / 2, 2, Cfg::BN, Cfg::FULL, stream);
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(static_cast<unsigned>(2 * G));
+    cfg.blockDim = dim3(kFusedThreads);
+    cfg.dynamicSmemBytes = Cfg::SMEM_BYTES;
+    cfg.stream = stream;
+    cudaLaunchAttribute attr[3];
+    cfg.numAttrs = fill_attrs(attr, 2, (args.balance && !args.sk) ? coop_mode() : 0);
+    cfg.attrs = attr;
+    HEAL_CUDA(cudaLaunchKernelEx(&cfg, kern, ta, tb_hi, tb_lo, args));
+    g_launches.fetch_add(1);
+    if (args.sk) return launch_sk_reduce<Cfg::BN>(args, 2, tiles, stream);
+    return HEAL_OK;
+}
+
 inline bool needs_ext(const OutArgs &out) { return out.hi != nullptr || out.accumulate != 0 || out.silu != 0 || out.scale != 1.0f || out.C == nullptr; }
 
 template <bool B_MN>
@@ -569,6 +618,19 @@ int launch_gemm2_np(int nprod, int64_t M, int64_t N, int64_t K, const void *A_hi
     case 4: return launch_gemm2_cfg<Gemm2Cfg<256, 4, B_MN, true>>(M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, out, s);   // diagnostic mode: one instantiation
     }
     return HEAL_ERR_UNSUPPORTED_MODE;
+}
+
+template <bool B_MN>
+int launch_gemm2f_np(int nprod, int64_t M, int64_t N, int64_t K, const float *A, int64_t lda, const void *B_hi, const void *B_lo,
+                     int64_t ldb, const OutArgs &out, cudaStream_t s)
+{
+    const int64_t tiles = ((M + 2 * kBM - 1) / (2 * kBM)) * ((N + 255) / 256);
+    if (needs_ext(out) || wants_split_k(tiles, (K + kKSeg - 1) / kKSeg, g.num_sms / 2, 2, 256)) {
+        if (nprod == 2) return launch_gemm2f_cfg<Gemm2FCfg<2, B_MN, true>>(M, N, K, A, lda, B_hi, B_lo, ldb, out, s);
+        return launch_gemm2f_cfg<Gemm2FCfg<3, B_MN, true>>(M, N, K, A, lda, B_hi, B_lo, ldb, out, s);
+    }
+    if (nprod == 2) return launch_gemm2f_cfg<Gemm2FCfg<2, B_MN>>(M, N, K, A, lda, B_hi, B_lo, ldb, out, s);
+    return launch_gemm2f_cfg<Gemm2FCfg<3, B_MN>>(M, N, K, A, lda, B_hi, B_lo, ldb, out, s);
 }
 
 template <int BN, bool B_MN>
@@ -851,7 +913,7 @@ int forced_kernel()
 
 int validate_mode(uint32_t mode, int *nprod, bool *b_nk)
 {
-    if (mode & ~(HEAL_MODE_PRODUCTS_MASK | HEAL_B_NK | HEAL_B_STATIC | HEAL_LO_SCALED | HEAL_EPI_SILU_MUL | HEAL_EPI_ACCUMULATE))
+    if (mode & ~(HEAL_MODE_PRODUCTS_MASK | HEAL_B_NK | HEAL_B_STATIC | HEAL_LO_SCALED | HEAL_EPI_SILU_MUL | HEAL_EPI_ACCUMULATE | HEAL_FUSE_SPLIT))
         return HEAL_ERR_UNSUPPORTED_MODE;
     const uint32_t p = mode & HEAL_MODE_PRODUCTS_MASK;
     if (p < 1 || p > 4) return HEAL_ERR_UNSUPPORTED_MODE;
@@ -1183,11 +1245,43 @@ int heal_gemm_ex(int64_t M, int64_t N, int64_t K, const void *A, int64_t lda, co
         if (st || handled) return st;
     }
 
+    // Prefill shapes served by the CTA-pair kernel (M > 128, N > 128), two or three products: step S of the activations can run
+    // inside the GEMM kernel (heal_gemm_umma2f.cuh) -- one launch and no workspace for FP16 weights.  Measured on B200 it is
+    // 0-13 % slower than split + GEMM (the in-place conversion shares the shared-memory bandwidth with the tensor core:
+    // 176 KB instead of 112 KB per k-tile), so it is used on request (HEAL_FUSE_SPLIT) and whenever the planes cannot be
+    // had: a captured call on a stream whose library workspace is missing or too small (instead of HEAL_ERR_WORKSPACE).
+    static const bool force_fused_large = std::getenv("HEAL_FUSED_LARGE") != nullptr;      // debug only
+    bool fuse_a = M > kBM && N > 128 && (nprod == 2 || nprod == 3) && !lo_scaled && !no_fused && forced_kernel() == 0;
+    if (fuse_a && !(mode & HEAL_FUSE_SPLIT) && !force_fused_large) {
+        fuse_a = false;
+        if (!b_f32 && stream_capturing(stream)) {
+            void *probe = nullptr;
+            if (get_ws(plan_ws(M, N, K, nprod, b_nk).total, stream, &probe) == HEAL_ERR_WORKSPACE) fuse_a = true;
+        }
+    }
     const WsPlan p = plan_ws(M, N, K, nprod, b_nk);
     void *ws = nullptr;
-    st = get_ws(p.total, stream, &ws);
-    if (st) return st;
+    if (!(fuse_a && !b_f32)) {
+        st = get_ws(p.total, stream, &ws);
+        if (st) return st;
+    }
     char *w = static_cast<char *>(ws);
+    if (fuse_a) {
+        const void *b_hi = B, *b_lo = nullptr;
+        int64_t ldb_eff = ldb;
+        if (b_f32) {
+            __half *bh = reinterpret_cast<__half *>(w + 2 * p.a_plane);
+            __half *bl = reinterpret_cast<__half *>(w + 2 * p.a_plane + p.b_plane);
+            const int64_t brows = b_nk ? N : K, bcols = b_nk ? K : N;
+            st = launch_split(brows, bcols, static_cast<const float *>(B), ldb, bh, bl, p.ldb_p, stream);
+            if (st) return st;
+            b_hi = bh;
+            b_lo = bl;
+            ldb_eff = p.ldb_p;
+        }
+        if (b_nk) return launch_gemm2f_np<false>(nprod, M, N, K, static_cast<const float *>(A), lda, b_hi, b_lo, ldb_eff, out, stream);
+        return launch_gemm2f_np<true>(nprod, M, N, K, static_cast<const float *>(A), lda, b_hi, b_lo, ldb_eff, out, stream);
+    }
     __half *a_hi = reinterpret_cast<__half *>(w);
     __half *a_lo = reinterpret_cast<__half *>(w + p.a_plane);
     // step S on the activations; in 1P only the hi plane is consumed

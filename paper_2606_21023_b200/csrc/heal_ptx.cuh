@@ -350,6 +350,26 @@ __device__ __noinline__ void mbar_wait_cluster(uint32_t bar, uint32_t parity, in
     }
 }
 
+// fully inline form (kernels that re-partition the register file with setmaxnreg must not call out-of-line functions
+// from the shrunk warps: ptxas cannot fit a callee's ABI register budget into them)
+__device__ __forceinline__ void mbar_wait_cluster_inl(uint32_t bar, uint32_t parity, int *diag, int code)
+{
+    if (mbar_try_wait_cluster(bar, parity)) return;
+    const uint64_t t0 = globaltimer_ns();
+    uint32_t spins = 0;
+    while (!mbar_try_wait_cluster(bar, parity)) {
+        if ((++spins & 0x3ffu) == 0 && globaltimer_ns() - t0 > 4000000000ull) {
+            if (diag) {
+                diag[0] = code;
+                diag[1] = static_cast<int>(blockIdx.x);
+                diag[2] = static_cast<int>(parity);
+            }
+            __threadfence_system();
+            __trap();
+        }
+    }
+}
+
 // split cluster barrier: every thread of every CTA arrives once; only the threads that need the guarantee wait
 __device__ __forceinline__ void cluster_arrive() { asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory"); }
 __device__ __forceinline__ void cluster_arrive_relaxed() { asm volatile("barrier.cluster.arrive.relaxed.aligned;" ::: "memory"); }

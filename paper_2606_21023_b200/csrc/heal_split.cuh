@@ -9,23 +9,28 @@
 
 namespace heal {
 
+// Two elements at a time with the packed conversion (cvt.rn.f16x2.f32 = one F2FP.PACK_AB instead of two F2F: the single
+// conversions run on the slow conversion unit and made the in-GEMM converters the bottleneck).  Same IEEE round-to-nearest-
+// even, subnormals and overflow to Inf as the scalar form -- the exhaustive-range split test covers it.
+__device__ __forceinline__ uint32_t pack_f16x2_rn(float lo_elem, float hi_elem)
+{
+    uint32_t r;
+    asm("cvt.rn.f16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(hi_elem), "f"(lo_elem));
+    return r;
+}
 __device__ __forceinline__ void split2(float x0, float x1, uint32_t &hi, uint32_t &lo)
 {
-    const __half h0 = __float2half_rn(x0), h1 = __float2half_rn(x1);
-    const __half l0 = __float2half_rn(__fsub_rn(x0, __half2float(h0)));
-    const __half l1 = __float2half_rn(__fsub_rn(x1, __half2float(h1)));
-    hi = static_cast<uint32_t>(__half_as_ushort(h0)) | (static_cast<uint32_t>(__half_as_ushort(h1)) << 16);
-    lo = static_cast<uint32_t>(__half_as_ushort(l0)) | (static_cast<uint32_t>(__half_as_ushort(l1)) << 16);
+    hi = pack_f16x2_rn(x0, x1);
+    const float2 hf = __half22float2(*reinterpret_cast<const __half2 *>(&hi));
+    lo = pack_f16x2_rn(__fsub_rn(x0, hf.x), __fsub_rn(x1, hf.y));
 }
 
 // scaled residual (the paper's h = h_hi + h_lo / 2^s): lo = r16((x - hi) * 2^s); the product is exact
 __device__ __forceinline__ void split2s(float x0, float x1, uint32_t &hi, uint32_t &lo, float lo_scale)
 {
-    const __half h0 = __float2half_rn(x0), h1 = __float2half_rn(x1);
-    const __half l0 = __float2half_rn(__fmul_rn(__fsub_rn(x0, __half2float(h0)), lo_scale));
-    const __half l1 = __float2half_rn(__fmul_rn(__fsub_rn(x1, __half2float(h1)), lo_scale));
-    hi = static_cast<uint32_t>(__half_as_ushort(h0)) | (static_cast<uint32_t>(__half_as_ushort(h1)) << 16);
-    lo = static_cast<uint32_t>(__half_as_ushort(l0)) | (static_cast<uint32_t>(__half_as_ushort(l1)) << 16);
+    hi = pack_f16x2_rn(x0, x1);
+    const float2 hf = __half22float2(*reinterpret_cast<const __half2 *>(&hi));
+    lo = pack_f16x2_rn(__fmul_rn(__fsub_rn(x0, hf.x), lo_scale), __fmul_rn(__fsub_rn(x1, hf.y), lo_scale));
 }
 
 // One thread handles 8 consecutive elements of a row (2 x float4 in, 2 x uint4 out); `cols8` =

@@ -37,8 +37,8 @@ def test_host_side_validation_without_device(lib):
     assert raw(0, 4, 8, None, 8, None, 8, None, 4, 2) == 0           # empty: no-op
     assert raw(4, 4, 8, None, 8, None, 8, None, 4, 2) == 2           # null pointer
     assert raw(4, 4, 8, 16, 8, 16, 8, 16, 4, 9) == 4                 # unknown product count
-    assert raw(4, 4, 8, 16, 8, 16, 8, 16, 4, 0x202) == 4             # unknown flag bit (0x10 B_NK, 0x20 B_STATIC, 0x40 LO_SCALED,
-                                                                     # 0x80 EPI_SILU_MUL, 0x100 EPI_ACCUMULATE are the known ones)
+    assert raw(4, 4, 8, 16, 8, 16, 8, 16, 4, 0x402) == 4             # unknown flag bit (0x10 B_NK, 0x20 B_STATIC, 0x40 LO_SCALED,
+                                                                     # 0x80 EPI_SILU_MUL, 0x100 EPI_ACCUMULATE, 0x200 FUSE_SPLIT are the known ones)
     assert raw(4, 5, 8, 16, 8, 16, 8, 16, 4, 0x82) == 1              # SiLU-mul pairs columns: N must be even
     assert raw(4, 4, 8, 16, 8, 16, 8, 16, 4, 0x43) == 4              # LO_SCALED is two-product only
     assert raw(4, 4, 8, 20, 8, 16, 8, 16, 4, 2) == 3                 # misaligned A

@@ -342,6 +342,49 @@ def test_kernel_families_bit_identical(hb, inputs, M, N, K, nprod, b_nk):
     assert torch.equal(outs[0], outs[1]) and torch.equal(outs[0], outs[2])
 
 
+@pytest.mark.parametrize("M,N,K,nprod,b_nk", [(300, 520, 4104, 2, False), (2048, 1024, 4096, 2, False), (129, 136, 72, 2, True),
+                                              (700, 1032, 2056, 3, True), (1300, 4104, 2056, 2, False), (256, 4096, 4096, 2, False),
+                                              (1000, 264, 1032, 3, False)])
+def test_fused_split_large_m_bit_identical(hb, oracle, inputs, M, N, K, nprod, b_nk):
+    """HEAL_FUSE_SPLIT: the CTA-pair kernel with step S done in shared memory (FP32 tile by TMA,
+    converted in place by four converter warps) gives the bits of split + GEMM -- ragged M / N / K tails (TMA zero fill of
+    the FP32 tile), both weight layouts, two and three products, the balanced schedule, ordered split-K, the extended
+    epilogue -- in ONE launch for FP16 weights; and it needs no workspace, so a captured call without one still works."""
+    A = dev_padded(inputs.activations(M, K, seed=81, outliers=True), 4)
+    B = inputs.weights_f32(K, N, seed=81, nk=b_nk) if nprod >= 3 else inputs.weights_f16(K, N, seed=81, nk=b_nk)
+    B = dev(B)
+    mode = nprod | (hb.B_NK if b_nk else 0)
+    ref = hb.heal_gemm(A, B, mode).clone()
+    n0 = hb.launch_count()
+    got = hb.heal_gemm(A, B, mode | hb.FUSE_SPLIT)
+    torch.cuda.synchronize()
+    assert hb.launch_count() - n0 <= (1 if nprod == 2 else 2) + 1          # (+1: the reduce kernel of ordered split-K)
+    assert torch.equal(got, ref)
+    c, h, l = hb.heal_gemm_ex(A, B, mode | hb.FUSE_SPLIT, scale_exp=2)
+    c2, h2, l2 = hb.heal_gemm_ex(A, B, mode, scale_exp=2)
+    torch.cuda.synchronize()
+    assert torch.equal(c, c2) and torch.equal(h, h2) and torch.equal(l, l2)
+
+
+def test_captured_call_without_workspace_uses_fused_split(hb, inputs):
+    """A large-M two-product call captured on a stream the library has never seen (no eager warm-up, no caller workspace):
+    instead of HEAL_ERR_WORKSPACE the library splits inside the GEMM kernel; the replay gives the eager bits."""
+    A = dev(inputs.activations(512, 2048, seed=82)); W = dev(inputs.weights_f16(2048, 1032, seed=82))
+    ref = hb.heal_gemm(A, W, 2).clone()
+    C = torch.zeros_like(ref)
+    s = torch.cuda.Stream()
+    torch.cuda.synchronize()
+    with torch.cuda.stream(s):
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=s):
+            hb.heal_gemm(A, W, 2, C=C)
+        for _ in range(3):
+            C.zero_()
+            g.replay()
+            s.synchronize()
+            assert torch.equal(C, ref)
+
+
 @pytest.mark.parametrize("M,N,K,b_nk", [(1, 4096, 4096, False), (8, 1032, 4096, False), (16, 520, 8192, False), (13, 264, 1000, True),
                                         (5, 4096, 520, True), (16, 128, 8192, False)])
 def test_fused_split_small_m_bit_identical(hb, oracle, inputs, M, N, K, b_nk):
@@ -926,7 +969,7 @@ def test_error_codes(hb):
     assert raw(8, 16, 64, a, 66, w, 16, c, 16, 2) == 3                 # lda % 4
     assert raw(8, 16, 64, a, 64, w, 20, c, 16, 2) == 3                 # ldb % 8 (FP16)
     assert raw(8, 16, 64, a, 64, w, 16, c, 16, 0) == 4
-    assert raw(8, 16, 64, a, 64, w, 16, c, 16, 0x102) == 4
+    assert raw(8, 16, 64, a, 64, w, 16, c, 16, 0x402) == 4
     assert raw(8, 16, 64, a, 64, w, 16, c, 16, 2) == 0
     # M > 16 needs hi/lo planes in the workspace (M <= 16 with FP16 weights splits inside the GEMM kernel)
     A2 = torch.zeros((32, 64), device="cuda")
