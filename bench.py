@@ -9,18 +9,20 @@ over one batch of synthetic input, for both MLP GEMMs:
     down    : [2048 x 14336] . [14336 x 4096]
 value = sum(2 M N K) / time  (effective TFLOP/s; the tensor cores do n_prod = 2 times that).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--full]
 
-N > 1 is launched by torchrun (one rank per GPU); the path shards over independent token batches
-(M) with no data-path collective -> "scaling": "weak".  `--impl reference` times the CPU oracle (as it
-stands) on a bounded row sample of the same workload.
+N > 1: one rank per GPU (launched by torchrun; `python bench.py --gpus N` alone re-executes itself under
+torch.distributed.run); the path shards over independent token batches (M) with no data-path collective ->
+"scaling": "weak".  `--impl reference` times the CPU oracle (as it stands) on a bounded row sample of the same
+workload.  Besides the contract keys the line carries the other BASELINE.json configs as context (`small_m`: decode and
+LM-head bandwidth, `square`: the three-product sweep, `lm_head_M512`, `cublas_context`, `error_contrast_vs_fp64`,
+`elementwise_err_vs_fp64`, `mlp_block`); `--full` adds the qkv / o-proj / Qwen3-14B / mid-size-M table (`shapes`).
 """
 from __future__ import annotations
 
 import argparse
 import json
 import os
-import subprocess
 import sys
 import threading
 import time
@@ -65,7 +67,7 @@ class ClockSampler(threading.Thread):
                 self.rows.append((float(nv.nvmlDeviceGetClockInfo(h, nv.NVML_CLOCK_SM)),
                                   nv.nvmlDeviceGetPowerUsage(h) / 1000.0,
                                   int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(h))))
-                time.sleep(0.005)
+                time.sleep(0.001)
         except Exception as e:  # noqa: BLE001
             self.err = repr(e)
 
@@ -82,11 +84,12 @@ class ClockSampler(threading.Thread):
                 "power_w_max": max(r[1] for r in self.rows), "samples": len(self.rows)}
 
 
-def make_inputs(seed):
+def make_inputs(seed, row0=0):
+    """The two GEMMs' inputs; `row0` = first row of the global activation matrix this rank owns (rows are regenerable)."""
     from paper_2606_21023_b200 import inputs
     out = []
     for name, M, N, K in SHAPES:
-        A = inputs.activations(M, K, seed=seed, outliers=True)
+        A = inputs.activations(M, K, seed=seed, outliers=True, row0=row0)
         W = inputs.weights_f16(K, N, seed=seed)
         out.append((name, A, W))
     return out
@@ -128,48 +131,157 @@ def run_reference(args):
         "gpu_launches": 0}))
 
 
+L2_BYTES = 126e6
+
+
+def time_calls(fns, graph, reps=5, cool=0.3):
+    """Median microseconds per call of `fns` run back to back (one callable per weight copy) on a side stream: as a
+    CUDA graph (launch-latency-scale kernels, rotating over the copies) or as a plain loop; CUDA events on that stream."""
+    import torch
+    time.sleep(cool)                                    # start from an idle GPU: burst figures
+    s = torch.cuda.Stream()
+    n_calls = len(fns) if graph else max(len(fns), 10 // len(fns) * len(fns))
+    with torch.cuda.stream(s):
+        for f in fns:
+            f()
+        s.synchronize()
+        if graph:
+            g = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(g, stream=s):
+                for f in fns:
+                    f()
+            run = g.replay
+        else:
+            def run():
+                for i in range(n_calls):
+                    fns[i % len(fns)]()
+        run()
+        s.synchronize()
+        ts = []
+        for _ in range(reps):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(s)
+            run()
+            e1.record(s)
+            s.synchronize()
+            ts.append(e0.elapsed_time(e1) * 1e3 / n_calls)
+    ts.sort()
+    return ts[len(ts) // 2]
+
+
+def shape_report(hb, peaks, M, N, K, nprod, dist="normal", cublas=True, flags=0):
+    """One shape through the C ABI: `full` = heal_gemm (FP32 in, everything included), `gemm` = heal_gemm_presplit (steps G + E on
+    planes; in 3P the weights are pre-split, the static-weight case), plus cuBLAS SGEMM (TF32 off) / FP16 / BF16 via
+    torch.matmul on the same inputs as context.  Inputs are made on the device (timing only; parity lives in tests/)."""
+    import torch
+    gen = torch.Generator(device="cuda")
+    gen.manual_seed(1234)
+    w_bytes = K * N * (4 if nprod >= 3 else 2)
+    small = 2.0 * nprod * M * N * K < 5e10
+    ncopies = max(2, min(12, int(3 * L2_BYTES // w_bytes) + 1)) if small else 1
+    if dist == "uniform":
+        A = torch.rand(M, K, device="cuda", generator=gen) * 2 - 1
+        Bs = [torch.rand(K, N, device="cuda", generator=gen) * 2 - 1 for _ in range(ncopies)]
+    else:
+        A = torch.randn(M, K, device="cuda", generator=gen)
+        Bs = [torch.randn(K, N, device="cuda", generator=gen) * (1.0 if nprod >= 3 else 0.02) for _ in range(ncopies)]
+    if nprod < 3:
+        Bs = [b.half() for b in Bs]
+    C = torch.empty(M, N, device="cuda")
+    ws = torch.empty(max(256, hb.workspace_size(M, N, K, nprod)), dtype=torch.uint8, device="cuda")
+    hb.set_workspace(ws)
+    reps = max(1, 24 // ncopies) if small else 1
+    out = {"MxNxK": f"{M}x{N}x{K}", "mode": f"{nprod}P", "timing": f"graph, {ncopies} weight copies" if small else "loop"}
+    t_full = time_calls([(lambda b=b: hb.heal_gemm(A, b, nprod | flags, C=C)) for b in Bs] * reps, small)
+    ah, al = hb.heal_split(A, lo_shift=hb.LO_SHIFT if flags & hb.LO_SCALED else 0)
+    planes = [(hb.heal_split(b) if nprod >= 3 else (b, None)) for b in Bs]
+    t_gemm = time_calls([(lambda q=q: hb.heal_gemm_presplit(ah, al, q[0], q[1], nprod | flags, C=C)) for q in planes] * reps, small)
+    del planes
+    hb.set_workspace(None)
+    flop = 2.0 * M * N * K
+    byt = K * N * 2 + M * K * 4 + M * N * 4
+    out.update({"full_us": t_full, "gemm_us": t_gemm, "eff_tflops_full": flop / t_full / 1e6, "eff_tflops_gemm": flop / t_gemm / 1e6,
+                "tensor_tflops_gemm": nprod * flop / t_gemm / 1e6,
+                "tensor_frac_of_measured_burst": nprod * flop / t_gemm / 1e6 / peaks["burst"],
+                "tensor_frac_of_nominal_2250": nprod * flop / t_gemm / 1e6 / 2250.0})
+    if M <= 64:
+        out["GBps_full"] = byt / t_full / 1e3
+        out["frac_of_measured_hbm_peak"] = byt / t_full / 1e3 / peaks["hbm"]
+    if cublas:
+        torch.backends.cuda.matmul.allow_tf32 = False
+        A16, Ab = A.half(), A.bfloat16()
+        C16 = torch.empty(M, N, device="cuda", dtype=torch.float16)
+        Cb = torch.empty(M, N, device="cuda", dtype=torch.bfloat16)
+        B32 = [b.float() for b in Bs]
+        out["cublas_sgemm_us"] = time_calls([(lambda b=b: torch.matmul(A, b, out=C)) for b in B32] * reps, small, reps=3)
+        del B32
+        B16 = [b.half() for b in Bs]
+        out["cublas_fp16_us"] = time_calls([(lambda b=b: torch.matmul(A16, b, out=C16)) for b in B16] * reps, small, reps=3)
+        del B16
+        Bb = [b.bfloat16() for b in Bs]
+        out["cublas_bf16_us"] = time_calls([(lambda b=b: torch.matmul(Ab, b, out=Cb)) for b in Bb] * reps, small, reps=3)
+        del Bb
+    del Bs
+    torch.cuda.empty_cache()
+    return out
+
+
+def mlp_block_report(hb):
+    """The MLP block of Algorithm 1 at Llama-3-8B size, M = 2048, through the fused entry points: Norm -> split,
+    gate_up GEMM with the SiLU-mul epilogue (activation planes out), down GEMM adding onto the residual: three launches."""
+    import torch
+    M, D, FF = 2048, 4096, 14336
+    gen = torch.Generator(device="cuda")
+    gen.manual_seed(5)
+    H = torch.randn(M, D, device="cuda", generator=gen)
+    gam = torch.ones(D, device="cuda")
+    Wgu = (torch.randn(D, 2 * FF, device="cuda", generator=gen) * 0.02).half()
+    Wd = (torch.randn(FF, D, device="cuda", generator=gen) * 0.02).half()
+    out = H.clone()
+    xh, xl, _ = hb.heal_rmsnorm_split(H, gam)
+    _, ah, al = hb.heal_gemm_presplit_ex(xh, xl, Wgu, None, 2 | hb.EPI_SILU_MUL, want_c=False)
+
+    def block():
+        hb.heal_rmsnorm_split(H, gam)                                   # (writes fresh planes each call)
+        hb.heal_gemm_presplit_ex(xh, xl, Wgu, None, 2 | hb.EPI_SILU_MUL, want_c=False, C_hi=ah, C_lo=al)
+        hb.heal_gemm_presplit_ex(ah, al, Wd, None, 2 | hb.EPI_ACCUMULATE, C=out, want_planes=False)
+
+    n0 = hb.launch_count()
+    block()
+    launches = hb.launch_count() - n0
+    t = time_calls([block], False)
+    flop = 2.0 * M * D * (2 * FF) + 2.0 * M * FF * D
+    return {"shape": "M=2048, d=4096, ff=14336 (gate_up interleaved 4096x28672, down 14336x4096)", "launches": int(launches), "us": t,
+            "eff_tflops": flop / t / 1e6, "tensor_tflops": 2 * flop / t / 1e6}
+
+
 def small_m_report(hb, peaks):
     """HBM-bound shapes of BASELINE.json configs[1] (decode 4096x4096, M = 1/8/32) and configs[4] (LM head, M = 1/64):
-    achieved GB/s = (2KN + 4MK + 4MN) / t through heal_gemm (device buffers; one fused kernel for M <= 16), timed as a
-    CUDA graph of back-to-back calls rotating over enough distinct weight copies to exceed the 126 MB L2."""
+    achieved GB/s = (2KN + 4MK + 4MN) / t through heal_gemm (device buffers; one fused kernel for decode-sized M), timed as a
+    CUDA graph of back-to-back calls rotating over enough distinct weight copies to exceed the 126 MB L2; `eager_us` = the
+    same calls issued one by one from the host (no graph): host-side launch cost included."""
     import torch
     out = {}
     for tag, M, N, K in [("decode_M1", 1, 4096, 4096), ("decode_M8", 8, 4096, 4096), ("decode_M32", 32, 4096, 4096),
                          ("lm_head_M1", 1, 128256, 4096), ("lm_head_M64", 64, 128256, 4096)]:
         gen = torch.Generator(device="cuda")
         gen.manual_seed(7)
-        ncopies = max(2, min(12, int(3 * 126e6 // (K * N * 2)) + 1))
+        ncopies = max(2, min(12, int(3 * L2_BYTES // (K * N * 2)) + 1))
         A = torch.randn(M, K, device="cuda", generator=gen)
         Ws = [(torch.randn(K, N, device="cuda", generator=gen) * 0.02).half() for _ in range(ncopies)]
         C = torch.empty(M, N, device="cuda")
         ws = torch.empty(max(256, hb.workspace_size(M, N, K, hb.MODE_2P)), dtype=torch.uint8, device="cuda")
         hb.set_workspace(ws)
         byt = K * N * 2 + M * K * 4 + M * N * 4
+        reps = max(1, 24 // ncopies)
         res = {}
         for name, mode in (("heal_gemm", hb.MODE_2P), ("heal_gemm+B_STATIC", hb.MODE_2P | hb.B_STATIC)):
-            s = torch.cuda.Stream()
-            with torch.cuda.stream(s):
-                for W in Ws:
-                    hb.heal_gemm(A, W, mode, C=C)
-                s.synchronize()
-                g = torch.cuda.CUDAGraph()
-                reps = 2 if ncopies < 8 else 1
-                with torch.cuda.graph(g, stream=s):
-                    for _ in range(reps):
-                        for W in Ws:
-                            hb.heal_gemm(A, W, mode, C=C)
-                g.replay()
-                s.synchronize()
-                ts = []
-                for _ in range(5):
-                    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-                    e0.record(s)
-                    g.replay()
-                    e1.record(s)
-                    s.synchronize()
-                    ts.append(e0.elapsed_time(e1) * 1e3 / (reps * ncopies))
-            t = sorted(ts)[2]
+            fns = [(lambda W=W: hb.heal_gemm(A, W, mode, C=C)) for W in Ws] * reps
+            t = time_calls(fns, True, cool=0.0)
             res[name] = {"us": t, "GB/s": byt / t / 1e3, "frac_of_measured_hbm_peak": byt / t / 1e3 / peaks["hbm"]}
+            if name == "heal_gemm":
+                res[name]["eager_us"] = time_calls(fns, False, cool=0.0)
+                res[name]["kernel"] = hb.last_kernel()
         out[tag] = res
         hb.set_workspace(None)
         del Ws
@@ -177,22 +289,41 @@ def small_m_report(hb, peaks):
     return out
 
 
+def elementwise_stats(X, ref, rows):
+    """max / median of |x - ref| / |ref| over the sampled rows (elements with |ref| below 1e-3 of the row's RMS are left
+    out of the relative statistics: they are cancellations, where any FP32 algorithm has a large relative error)."""
+    d = np.abs(X[rows].astype(np.float64) - ref)
+    rms = np.sqrt((ref ** 2).mean(axis=1, keepdims=True))
+    keep = np.abs(ref) >= 1e-3 * rms
+    rel = d[keep] / np.abs(ref[keep])
+    return {"max_rel": float(rel.max()), "median_rel": float(np.median(rel)), "max_abs_over_row_rms": float((d / rms).max())}
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
     from paper_2606_21023_b200 import binding as hb
+    from paper_2606_21023_b200 import shard
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device (no CPU fallback)")
+    if world != args.gpus:
+        raise SystemExit(f"bench.py: --gpus {args.gpus} but WORLD_SIZE={world}")
+    if torch.cuda.device_count() <= local:
+        raise SystemExit(f"bench.py: rank {rank} needs cuda:{local}, only {torch.cuda.device_count()} device(s) visible")
     torch.cuda.set_device(local)
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     hb.lib()
 
-    data = make_inputs(seed=rank)                      # each rank: its own token batch (weak scaling)
+    # M-sharding (DESIGN.md 9): the global batch of world x 2048 tokens is cut into contiguous row ranges, one per rank; weights
+    # are replicated; no data-path collective.  Rows are regenerable, so rank r generates exactly its rows of the global matrix.
+    r0, r1 = shard.shard_rows(world * M_TOK, world, rank)
+    assert r1 - r0 == M_TOK
+    data = make_inputs(seed=0, row0=r0)
     host = [(n, torch.from_numpy(A).pin_memory(), torch.from_numpy(W).pin_memory()) for n, A, W in data]
     devs = [(n, A.cuda(), W.cuda(), torch.empty((A.shape[0], W.shape[1]), device="cuda")) for n, A, W in host]
     ws = torch.empty(max(hb.workspace_size(m, n, k, hb.MODE_2P) for _, m, n, k in SHAPES), dtype=torch.uint8, device="cuda")
@@ -228,13 +359,13 @@ def run_ours(args):
     sampler = ClockSampler(int(os.environ.get("CUDA_VISIBLE_DEVICES", str(local)).split(",")[local]) if world == 1 else local)
     l0 = hb.launch_count()
     sampler.start()
+    time.sleep(0.01)
     ms_total = timed(step, args.steps)
-    sampler.stop_flag = True
     launches = hb.launch_count() - l0
     ms_step = ms_total / args.steps
-    value = world * FLOP_STEP / (ms_step * 1e-3) / 1e12
+    value = shard.aggregate_throughput([FLOP_STEP] * world, [ms_step] * world) / 1e12      # all ranks' flops / the slowest rank's time
 
-    # ---- roofline of the dominant kernel (heal_gemm_umma_kernel), timed alone on pre-split planes
+    # ---- roofline of the dominant kernel, timed alone on pre-split planes (same launch configuration as in the step)
     planes = []
     for _, A, W, C in devs:
         ah, al = hb.heal_split(A)
@@ -246,17 +377,24 @@ def run_ours(args):
 
     for _ in range(3):
         gemm_only()
+    kernel_name = hb.last_kernel()
     ms_gemm = timed(gemm_only, args.steps) / args.steps / len(SHAPES)        # average launch duration
+    sampler.stop_flag = True
     sampler.join()
     peaks = load_peaks()
     long_run = ms_total > 1000.0
     peak = peaks["sustained"] if long_run else peaks["burst"]
     flop_launch = N_PROD * FLOP_STEP / len(SHAPES)
     achieved = flop_launch / (ms_gemm * 1e-3) / 1e12
-    traffic = None
+    traffic, traffic_src = None, None
     tpath = os.path.join(ROOT, "profiles", "gemm_dram_traffic.json")
     if os.path.exists(tpath):
-        traffic = json.load(open(tpath)).get("dram_bytes_per_launch")
+        tj = json.load(open(tpath))
+        traffic, traffic_src = tj.get("dram_bytes_per_launch"), tj.get("source")
+    # operand delivery (L2 -> SM) of the same launches: the measured limiter of this kernel; per k-tile a CTA
+    # receives its 128 rows of A_hi and A_lo and half of the 256-column W tile = 48 KB
+    ktile_steps = sum((m // 256) * (n // 256) * (k // 64) for _, m, n, k in SHAPES) * 2 / len(SHAPES)       # CTA k-tile steps per launch
+    delivery = 48 * 1024 * ktile_steps / (ms_gemm * 1e-3) / 1e9 / 148
 
     # ---- end to end through the C ABI with HOST buffers (H2D + path + D2H inside the timed region)
     e2e_steps = max(1, min(args.steps, 5))
@@ -276,15 +414,18 @@ def run_ours(args):
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
             "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f16xf16->f32",
             "data": "synthetic",
-            "config": {"workload": WORKLOAD, "global_tokens": world * M_TOK, "parallelism": f"dp{world} over token batches",
+            "config": {"workload": WORKLOAD, "global_tokens": world * M_TOK, "parallelism": f"dp{world} over token batches (M-sharding, no collective)",
                        "l2": "inputs larger than L2 (A+W+C = 268 MB per GEMM vs 126 MB L2)",
                        "tensor_tflops": N_PROD * value},
-            "roofline": {"bound": "tensor", "kernel": "heal_gemm_umma2_kernel<BN=256,2P> (CTA pairs)", "achieved": achieved, "peak": peak,
-                         "unit": "TFLOP/s", "frac": achieved / peak, "traffic": traffic,
+            "roofline": {"bound": "tensor", "kernel": kernel_name, "achieved": achieved, "peak": peak,
+                         "unit": "TFLOP/s", "frac": achieved / peak, "traffic": traffic, "traffic_source": traffic_src,
                          "peak_kind": f"{peaks['src']} cuBLAS bf16 {'sustained' if long_run else 'burst'} (fp16 = bf16 rate)",
                          "frac_of_nominal_2250": achieved / 2250.0, "frac_of_measured_burst": achieved / peaks["burst"],
                          "frac_of_measured_sustained": achieved / peaks["sustained"], "avg_launch_ms": ms_gemm,
-                         "flops_per_launch": flop_launch},
+                         "flops_per_launch": flop_launch,
+                         "limiter": {"what": "L2 -> SM operand delivery (48 KB per CTA and k-tile; tensor pipe ~80 % active in ncu)",
+                                     "achieved_GBps_per_sm": delivery, "probe_peak_GBps_per_sm": 69.4,
+                                     "source": "profiles/probes_r01.md, DESIGN.md section 7"}},
             "e2e": {"value": world * FLOP_STEP / (ms_e2e * 1e-3) / 1e12, "unit": UNIT, "h2d_bytes_per_step": h2d,
                     "d2h_bytes_per_step": d2h, "ms_per_step": ms_e2e},
             "gpu_launches": int(launches),
@@ -296,24 +437,62 @@ def run_ours(args):
             line["cpu_baseline"] = {"value": tf, "unit": UNIT, "cores": cores, "kind": "oracle", "seconds": dt,
                                     "sample": f"{rows_n} evenly spaced rows of each of the two GEMMs (full N and K)"}
             import oracle
-            errs = {}
-            contrast = {}
+            errs, contrast, elem = {}, {}, {}
             torch.backends.cuda.matmul.allow_tf32 = False
             for (name, A, W), (_, Ad, Wd, C), ref in zip(data, devs, refs):
-                errs[name] = oracle.normwise_error(C.cpu().numpy(), ref, A, W, rows=rows)
+                hb.heal_gemm(Ad, Wd, hb.MODE_2P, C=C)
+                heal = C.cpu().numpy()
+                fp16 = hb.heal_gemm(Ad, Wd, hb.MODE_1P).cpu().numpy()
+                bf16 = torch.matmul(Ad.bfloat16(), Wd.bfloat16()).float().cpu().numpy()
+                sgemm = torch.matmul(Ad, Wd.float()).cpu().numpy()
+                errs[name] = oracle.normwise_error(heal, ref, A, W, rows=rows)
                 # context (north_star): the same inputs through plain 16-bit GEMMs and cuBLAS SGEMM, scored the same way
-                e = lambda X: oracle.normwise_error(X.float().cpu().numpy(), ref, A, W, rows=rows)
-                contrast[name] = {"heal_2P": errs[name],
-                                  "plain_fp16_1P (heal_gemm mode 1)": e(hb.heal_gemm(Ad, Wd, hb.MODE_1P)),
-                                  "plain_bf16 (cuBLAS, bf16 out)": e(torch.matmul(Ad.bfloat16(), Wd.bfloat16())),
-                                  "sgemm_fp32 (cuBLAS, TF32 off)": e(torch.matmul(Ad, Wd.float()))}
+                e = lambda X: oracle.normwise_error(X, ref, A, W, rows=rows)
+                contrast[name] = {"heal_2P": errs[name], "plain_fp16_1P (heal_gemm mode 1)": e(fp16),
+                                  "plain_bf16 (cuBLAS, bf16 out)": e(bf16), "sgemm_fp32 (cuBLAS, TF32 off)": e(sgemm)}
+                # element-wise view of "near-FP32": relative error per element on the sampled rows
+                elem[name] = {"heal_2P": elementwise_stats(heal, ref, rows), "sgemm_fp32 (cuBLAS, TF32 off)": elementwise_stats(sgemm, ref, rows),
+                              "plain_fp16_1P": elementwise_stats(fp16, ref, rows)}
             line["normwise_err_vs_fp64"] = errs
             line["error_contrast_vs_fp64"] = contrast
+            line["elementwise_err_vs_fp64"] = elem
+            del devs, planes
+            torch.cuda.empty_cache()
+            # ---- the other BASELINE.json configs and context rows (CUDA-event timings of the same process, burst regime)
+            line["cublas_context"] = {name: {k: v for k, v in shape_report(hb, peaks, m, n, k_, 2).items() if k.startswith("cublas") or k in ("full_us", "gemm_us")}
+                                      for name, m, n, k_ in SHAPES}
             line["small_m"] = small_m_report(hb, peaks)
+            line["square"] = {str(n): shape_report(hb, peaks, n, n, n, 3, dist="uniform") for n in (1024, 2048, 4096, 8192)}
+            line["lm_head_M512"] = shape_report(hb, peaks, 512, 128256, 4096, 2)
+            line["mlp_block"] = mlp_block_report(hb)
+            if args.full:
+                extra = [("L3-8B qkv", 2048, 6144, 4096), ("L3-8B o-proj", 2048, 4096, 4096), ("Q3-14B gate_up", 2048, 17408, 5120),
+                         ("Q3-14B down", 2048, 5120, 17408), ("Q3-14B qkv", 2048, 7168, 5120), ("decode down M=1", 1, 4096, 14336),
+                         ("decode down M=32", 32, 4096, 14336), ("decode gate+up M=1", 1, 28672, 4096), ("decode qkv M=1", 1, 6144, 4096),
+                         ("decode M=64", 64, 4096, 4096), ("mid M=128", 128, 4096, 4096), ("mid M=256", 256, 4096, 4096),
+                         ("mid M=512", 512, 4096, 4096), ("mid M=1024", 1024, 4096, 4096), ("cfg0 single (3P)", 64, 256, 256)]
+                line["shapes"] = {name: shape_report(hb, peaks, m, n, k_, 3 if "3P" in name else 2) for name, m, n, k_ in extra}
+                line["shapes"]["cfg2 up/gate, s=10 (HEAL_LO_SCALED)"] = shape_report(hb, peaks, 2048, 14336, 4096, 2, cublas=False, flags=hb.LO_SCALED)
+                line["shapes"]["decode M=8, s=10 (HEAL_LO_SCALED)"] = shape_report(hb, peaks, 8, 4096, 4096, 2, cublas=False, flags=hb.LO_SCALED)
+                line["shapes"]["cfg2 up/gate, HEAL_FUSE_SPLIT"] = shape_report(hb, peaks, 2048, 14336, 4096, 2, cublas=False, flags=hb.FUSE_SPLIT)
         print(json.dumps(line))
     hb.set_workspace(None)
     if world > 1:
         dist.destroy_process_group()
+
+
+def relaunch_under_torchrun(args):
+    """`python bench.py --gpus N` (N > 1) outside torchrun: start N ranks of this script, one per GPU, rendezvous on 127.0.0.1."""
+    import subprocess
+    import torch
+    if not torch.cuda.is_available() or torch.cuda.device_count() < args.gpus:
+        n = torch.cuda.device_count() if torch.cuda.is_available() else 0
+        raise SystemExit(f"bench.py: --gpus {args.gpus} needs {args.gpus} CUDA devices, {n} visible")
+    port = 29500 + os.getpid() % 1000
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}", "--master-addr", "127.0.0.1",
+           "--master-port", str(port), os.path.abspath(__file__), "--gpus", str(args.gpus), "--steps", str(args.steps),
+           "--warmup", str(args.warmup), "--impl", args.impl] + (["--full"] if args.full else [])
+    raise SystemExit(subprocess.call(cmd))
 
 
 if __name__ == "__main__":
@@ -322,5 +501,8 @@ if __name__ == "__main__":
     ap.add_argument("--steps", type=int, default=1500)      # > 1 s of back-to-back GEMMs: the sustained (power-capped) regime
     ap.add_argument("--warmup", type=int, default=10)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--full", action="store_true", help="also time the qkv / o-proj / Qwen3-14B / mid-size-M shapes (key `shapes`)")
     a = ap.parse_args()
+    if a.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        relaunch_under_torchrun(a)
     run_reference(a) if a.impl == "reference" else run_ours(a)

@@ -110,7 +110,8 @@ typedef enum {
  * capture the library does not allocate: run the call once eagerly on that stream first (or supply
  * a workspace); a captured call that finds none returns HEAL_ERR_WORKSPACE, except for the shapes of HEAL_FUSE_SPLIT, which
  * then split inside the GEMM kernel.  Buffers that a captured graph may hold are never freed or handed to another stream.
- * With FP16 weights, M <= 16 and K <= 8192 the split always runs inside the GEMM kernel: one launch, no workspace.
+ * With FP16 weights and decode-sized M (M <= 16 with K <= 16384; M <= 32 for problems of up to 32 Mi weights) the split
+ * always runs inside the GEMM kernel: one launch, no workspace.
  * Numerical contract: finite inputs with |x| <= 65504 (activations observed
  * < 1024); anything larger, Inf or NaN propagates to Inf/NaN in the affected rows/columns.
  */
@@ -219,6 +220,10 @@ uint64_t heal_launch_count(void);
  * instead of CTA pairs.  Results are bit-identical whichever kernel runs; only speed changes.
  */
 int heal_debug_force_kernel(int which);
+
+/* Name (static string) of the GEMM kernel instantiation the calling thread's most recent heal_gemm* call launched, e.g.
+ * "heal_gemm_umma2_kernel<256,2P,KxN,cta_group::2>"; "none" before the first launch.  For reports (bench.py). */
+const char *heal_last_kernel(void);
 
 /* Library version: major * 10000 + minor * 100 + patch. */
 int heal_version(void);

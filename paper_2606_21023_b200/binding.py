@@ -65,6 +65,7 @@ def lib():
         L.heal_launch_count.restype = ctypes.c_uint64
         L.heal_version.restype = ci
         L.heal_last_cuda_error.restype = ci
+        L.heal_last_kernel.restype = ctypes.c_char_p
         L.heal_status_string.restype = ctypes.c_char_p
         L.heal_status_string.argtypes = [ci]
         _lib = L
@@ -98,6 +99,10 @@ def version() -> int:
 def debug_force_kernel(which: int):
     """0 auto, 1 large-M kernels only, 2 small-M for M <= 64, 3 single-CTA large-M kernel (debug)."""
     _check(lib().heal_debug_force_kernel(which))
+
+
+def last_kernel() -> str:
+    return lib().heal_last_kernel().decode()
 
 
 def launch_count() -> int:

@@ -14,6 +14,7 @@
 #include <cstring>
 #include <deque>
 #include <mutex>
+#include <string>
 #include <vector>
 
 #include "heal_gemm_smallm.cuh"
@@ -26,6 +27,11 @@ namespace {
 
 using namespace heal;
 
+thread_local const char *t_last_kernel = "none";      // heal_last_kernel(): the GEMM kernel of this thread's latest call
+std::string kernel_name(const char *family, int a, int nprod, bool b_mn, const char *extra)
+{
+    return std::string(family) + "<" + std::to_string(a) + "," + std::to_string(nprod) + "P," + (b_mn ? "KxN" : "NxK") + extra + ">";
+}
 std::atomic<int> g_last_cuda_error{0};
 std::atomic<uint64_t> g_launches{0};
 std::mutex g_mu;
@@ -489,6 +495,8 @@ int launch_gemm_cfg(int64_t M, int64_t N, int64_t K, const void *A_hi, const voi
     cfg.attrs = attr;
     HEAL_CUDA(cudaLaunchKernelEx(&cfg, kern, ta_hi, ta_lo, tb_hi, tb_lo, args));
     g_launches.fetch_add(1);
+    static const std::string name = kernel_name("heal_gemm_umma_kernel", Cfg::BN, Cfg::NPROD, Cfg::B_MN, Cfg::FULL ? ",full" : "");
+    t_last_kernel = name.c_str();
     if (args.sk) return launch_sk_reduce<Cfg::BN>(args, 1, tiles, stream);
     return HEAL_OK;
 }
@@ -543,6 +551,8 @@ int launch_gemm2_cfg(int64_t M, int64_t N, int64_t K, const void *A_hi, const vo
     cfg.attrs = attr;
     HEAL_CUDA(cudaLaunchKernelEx(&cfg, kern, ta_hi, ta_lo, tb_hi, tb_lo, args));
     g_launches.fetch_add(1);
+    static const std::string name = kernel_name("heal_gemm_umma2_kernel", Cfg::BN, Cfg::NPROD, Cfg::B_MN, Cfg::FULL ? ",full,cta_group::2" : ",cta_group::2");
+    t_last_kernel = name.c_str();
     if (args.sk) return launch_sk_reduce<Cfg::BN>(args, 2, tiles, stream);
     return HEAL_OK;
 }
@@ -591,6 +601,8 @@ int launch_gemm2f_cfg(int64_t M, int64_t N, int64_t K, const float *A, int64_t l
     cfg.attrs = attr;
     HEAL_CUDA(cudaLaunchKernelEx(&cfg, kern, ta, tb_hi, tb_lo, args));
     g_launches.fetch_add(1);
+    static const std::string name = kernel_name("heal_gemm_umma2f_kernel", Cfg::BN, Cfg::NPROD, Cfg::B_MN, Cfg::FULL ? ",full,cta_group::2,fused split" : ",cta_group::2,fused split");
+    t_last_kernel = name.c_str();
     if (args.sk) return launch_sk_reduce<Cfg::BN>(args, 2, tiles, stream);
     return HEAL_OK;
 }
@@ -849,6 +861,9 @@ int launch_small_cfg(int64_t M, int64_t N, int64_t K, const SmallIn &in, const v
     cfg.attrs = attr;
     HEAL_CUDA(cudaLaunchKernelEx(&cfg, kern, tx_hi, tx_lo, tw_hi, tw_lo, args));
     g_launches.fetch_add(1);
+    static const std::string name = kernel_name("heal_gemm_smallm_kernel", Cfg::MPAD, Cfg::NPROD, Cfg::B_MN,
+                                                Cfg::FUSED ? ",fused split" : (Cfg::PAIR ? ",cta_group::2" : ""));
+    t_last_kernel = name.c_str();
     *handled = true;
     return HEAL_OK;
 }
@@ -1060,6 +1075,8 @@ int heal_debug_set_trace(void *ptr)
 
 int heal_last_cuda_error(void) { return g_last_cuda_error.load(); }
 
+const char *heal_last_kernel(void) { return t_last_kernel; }
+
 uint64_t heal_launch_count(void) { return g_launches.load(); }
 
 const char *heal_status_string(int status)
@@ -1235,10 +1252,15 @@ int heal_gemm_ex(int64_t M, int64_t N, int64_t K, const void *A, int64_t lda, co
     if (K == 0) return presplit_impl(M, N, K, nullptr, nullptr, lda, nullptr, nullptr, ldb, out, nprod, b_nk, b_static, stream);
     static const bool no_fused = std::getenv("HEAL_NO_FUSED") != nullptr;          // debug only
     const bool lo_scaled = (mode & HEAL_LO_SCALED) != 0;
-    if (M <= 16 && K <= 8192 && !b_f32 && !no_fused && !lo_scaled && !out.silu && forced_kernel() != 1) {
-        // decode shapes (M <= 16) with FP16 weights: step S runs inside the GEMM kernel (no planes, one launch);
-        // above that -- and for long K, where a CTA converts many k-tiles -- the in-kernel conversion costs more
-        // than the split launch it saves (measured: M = 1, K = 14336 31 vs 28 us)
+    // Decode shapes with FP16 weights: step S runs inside the small-M GEMM kernel (no planes, one launch) while the conversion
+    // work of a CTA stays small next to its weight stream: up to 16 tokens always (K <= 16384), up to 32 tokens for small
+    // problems, where the second launch costs more than the conversion (measured with the packed conversion of split2:
+    // 32 x 4096 x 4096 12.1 -> 10.9 us, 24 x 6144 x 4096 22.0 -> 19.9 us, 1 x 4096 x 14336 25.6 -> 23.8 us; but
+    // 32 x 28672 x 4096 44.8 vs 51.0 us, 32 x 4096 x 14336 36.0 vs 39.7 us, LM head M = 32 177 vs 199 us fused).
+    static const long fused_max_m = std::getenv("HEAL_FUSED_MAX_M") ? std::atol(std::getenv("HEAL_FUSED_MAX_M")) : 0;        // tuning
+    const bool fuse_small = fused_max_m > 0 ? (M <= fused_max_m && K <= 16384)
+                                            : ((M <= 16 && K <= 16384) || (M <= 32 && K <= 8192 && N * K <= (static_cast<int64_t>(32) << 20)));
+    if (fuse_small && !b_f32 && !no_fused && !lo_scaled && !out.silu && forced_kernel() != 1) {
         bool handled = false;
         st = presplit_impl(M, N, K, nullptr, nullptr, 0, B, nullptr, ldb, out, nprod, b_nk, b_static, stream,
                            static_cast<const float *>(A), lda, &handled);
