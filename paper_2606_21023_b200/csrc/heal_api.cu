@@ -347,7 +347,7 @@ bool bind_xfer(GemmArgs &args, cudaStream_t stream, size_t part_bytes = 0)
 // Ordered split-K pays while a CTA gets few units: a parked unit costs about `a/b` plain segments more than a unit of a
 // whole tile (its partial travels to L2 and back through the reduce kernel), whole tiles cost n_seg segments per CTA.
 // HEAL_SK_RULE="a,b" overrides the measured default (debug / tuning).
-bool sk_rule(int64_t units_per_cta, int64_t n_seg)
+bool sk_rule(int64_t units_per_cta, int64_t n_seg, int64_t tiles, int64_t G_max)
 {
     static int a = 12, b = 5;
     static const bool init = [] {
@@ -358,6 +358,9 @@ bool sk_rule(int64_t units_per_cta, int64_t n_seg)
         return true;
     }();
     (void)init;
+    // two segments only (K <= 1024): worth it when the tiles fill at most a quarter of the machine (measured: 1024^3 three
+    // products 22.9 -> 18.8 us; with more tiles the parked partials cost more than the idle SMs)
+    if (n_seg == 2) return units_per_cta == 1 && 4 * tiles <= G_max;
     return a * units_per_cta < b * n_seg;
 }
 
@@ -367,7 +370,7 @@ bool wants_split_k(int64_t tiles, int64_t n_seg, int64_t G_max, int ctas_per_til
     const int64_t units = tiles * n_seg;
     const int64_t G = units < G_max ? units : G_max;
     const size_t part_bytes = static_cast<size_t>(units) * ctas_per_tile * kBM * bn * sizeof(float);
-    return G > tiles && sk_rule((units + G - 1) / G, n_seg) && part_bytes <= (static_cast<size_t>(128) << 20);
+    return G > tiles && sk_rule((units + G - 1) / G, n_seg, tiles, G_max) && part_bytes <= (static_cast<size_t>(128) << 20);
 }
 
 int64_t set_balance(GemmArgs &args, int64_t tiles, int64_t n_seg, int64_t G_max, int ctas_per_tile, int bn, bool full_kernel,
@@ -389,7 +392,7 @@ int64_t set_balance(GemmArgs &args, int64_t tiles, int64_t n_seg, int64_t G_max,
         // Worth it only while a CTA gets few units: parking and re-reading a partial costs about 1.4 segments of
         // L2 traffic (measured: a parked unit takes 2.4x a plain segment), whole tiles cost n_seg segments.
         const int64_t units_per_cta = (units + G - 1) / G;
-        if (full_kernel && !no_balance && n_seg > 1 && G > tiles && sk_rule(units_per_cta, n_seg) &&
+        if (full_kernel && !no_balance && n_seg > 1 && G > tiles && sk_rule(units_per_cta, n_seg, tiles, G_max) &&
             part_bytes <= (static_cast<size_t>(128) << 20) && bind_xfer(args, stream, part_bytes)) {
             args.balance = 1;
             args.sk = 1;

@@ -194,13 +194,21 @@ heal_splitk_reduce_kernel(const float *__restrict__ part, int n_seg, int R, int 
         float4 acc;
         asm volatile("ld.global.cg.v4.f32 {%0, %1, %2, %3}, [%4];"
                      : "=f"(acc.x), "=f"(acc.y), "=f"(acc.z), "=f"(acc.w) : "l"(src + c4 * 256 + etid) : "memory");
-#pragma unroll 4
-        for (int s = 1; s < n_seg; ++s) {
-            float4 v;
-            asm volatile("ld.global.cg.v4.f32 {%0, %1, %2, %3}, [%4];"
-                         : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(src + s * seg_stride + c4 * 256 + etid) : "memory");
-            acc.x = __fadd_rn(acc.x, v.x); acc.y = __fadd_rn(acc.y, v.y);
-            acc.z = __fadd_rn(acc.z, v.z); acc.w = __fadd_rn(acc.w, v.w);
+        // (non-volatile loads, eight segments per batch: the loads of a batch are all in flight before the first add)
+#pragma unroll 1
+        for (int s0 = 1; s0 < n_seg; s0 += 8) {
+            float4 v[8];
+#pragma unroll
+            for (int u = 0; u < 8; ++u)
+                if (s0 + u < n_seg)
+                    asm("ld.global.cg.v4.f32 {%0, %1, %2, %3}, [%4];"
+                        : "=f"(v[u].x), "=f"(v[u].y), "=f"(v[u].z), "=f"(v[u].w) : "l"(src + (s0 + u) * seg_stride + c4 * 256 + etid));
+#pragma unroll
+            for (int u = 0; u < 8; ++u)
+                if (s0 + u < n_seg) {
+                    acc.x = __fadd_rn(acc.x, v[u].x); acc.y = __fadd_rn(acc.y, v[u].y);
+                    acc.z = __fadd_rn(acc.z, v[u].z); acc.w = __fadd_rn(acc.w, v[u].w);
+                }
         }
         if (row < M) {
             emit_dispatch(out, [&](const OutArgs &po, auto fast) {
