@@ -971,16 +971,16 @@ def test_error_codes(hb):
     assert raw(8, 16, 64, a, 64, w, 16, c, 16, 0) == 4
     assert raw(8, 16, 64, a, 64, w, 16, c, 16, 0x402) == 4
     assert raw(8, 16, 64, a, 64, w, 16, c, 16, 2) == 0
-    # M > 16 needs hi/lo planes in the workspace (M <= 16 with FP16 weights splits inside the GEMM kernel)
-    A2 = torch.zeros((32, 64), device="cuda")
-    C2 = torch.zeros((32, 16), device="cuda")
+    # M > 32 needs hi/lo planes in the workspace (decode-sized M with FP16 weights splits inside the GEMM kernel)
+    A2 = torch.zeros((48, 64), device="cuda")
+    C2 = torch.zeros((48, 16), device="cuda")
     ws = torch.zeros(256, dtype=torch.uint8, device="cuda")
     hb.set_workspace(ws)
-    assert raw(32, 16, 64, A2.data_ptr(), 64, w, 16, C2.data_ptr(), 16, 2) == 6       # supplied workspace too small
+    assert raw(48, 16, 64, A2.data_ptr(), 64, w, 16, C2.data_ptr(), 16, 2) == 6       # supplied workspace too small
     assert raw(8, 16, 64, a, 64, w, 16, c, 16, 2) == 0                               # fused path: no workspace needed
-    big = torch.zeros(hb.workspace_size(32, 16, 64, 2), dtype=torch.uint8, device="cuda")
+    big = torch.zeros(hb.workspace_size(48, 16, 64, 2), dtype=torch.uint8, device="cuda")
     hb.set_workspace(big)
-    assert raw(32, 16, 64, A2.data_ptr(), 64, w, 16, C2.data_ptr(), 16, 2) == 0
+    assert raw(48, 16, 64, A2.data_ptr(), 64, w, 16, C2.data_ptr(), 16, 2) == 0
     hb.set_workspace(None)
     torch.cuda.synchronize()
 
