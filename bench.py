@@ -481,6 +481,81 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+def run_trace():
+    """`bench.py --trace`: builds libheal_trace.so (the same sources with -DHEAL_TRACE) and prints, as markdown, (1) the %globaltimer
+    phase stamps of the decode GEMM 4096 x 4096 (M = 1, 32) inside a CUDA graph of twelve launches rotating over twelve weight copies,
+    (2) the same graph with ONE weight copy (weights resident in L2: the latency floor of the kernel structure), (3) the wait counters of
+    the CTA-pair kernel on the two MLP GEMMs.  Diagnostics only: nothing here is a bench value."""
+    import ctypes
+    import torch
+    from paper_2606_21023_b200 import build as hbuild
+    from paper_2606_21023_b200 import binding as hb
+    hb.LIB_PATH = hbuild.build(trace=True)
+    L = hb.lib()
+    L.heal_debug_set_trace.argtypes = [ctypes.c_void_p]
+    names = {0: "kernel entry", 13: "TMEM allocated", 1: "prologue done", 2: "griddepcontrol.wait returned", 3: "first TMA issued",
+             4: "first operand tile complete", 5: "last MMA issued", 6: "commit seen by epilogue", 7: "partials pushed",
+             8: "all partials landed (owners)", 9: "C stored", 11: "TMEM released"}
+    print("# Phase trace of the small-M kernel and wait counters of the CTA-pair kernel (`python bench.py --trace`, trace build)\n")
+    for M in (1, 32):
+        for ncopies in (12, 1):
+            gen = torch.Generator(device="cuda")
+            gen.manual_seed(7)
+            A = torch.randn(M, 4096, device="cuda", generator=gen)
+            Ws = [(torch.randn(4096, 4096, device="cuda", generator=gen) * 0.02).half() for _ in range(ncopies)]
+            C = torch.empty(M, 4096, device="cuda")
+            tr = torch.zeros(16 * 1024 * 64, dtype=torch.int64, device="cuda")
+            s = torch.cuda.Stream()
+            with torch.cuda.stream(s):
+                for W in Ws:
+                    hb.heal_gemm(A, W, hb.MODE_2P, C=C)
+                s.synchronize()
+                L.heal_debug_set_trace(ctypes.c_void_p(tr.data_ptr()))
+                g = torch.cuda.CUDAGraph()
+                with torch.cuda.graph(g, stream=s):
+                    for i in range(12):
+                        hb.heal_gemm(A, Ws[i % ncopies], hb.MODE_2P, C=C)
+                for _ in range(3):
+                    g.replay()
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record(s)
+                g.replay()
+                e1.record(s)
+                s.synchronize()
+            L.heal_debug_set_trace(None)
+            t = tr.cpu().numpy().reshape(16, 1024, 64)
+            a, nxt = t[6], t[7]
+            act = a[:, 0] > 0
+            base = a[act, 2].min()
+            print(f"## decode {M} x 4096 x 4096, {hb.last_kernel()}, {int(act.sum())} CTAs, {ncopies} weight cop{'y (L2-resident)' if ncopies == 1 else 'ies (HBM)'}: "
+                  f"{e0.elapsed_time(e1) * 1e3 / 12:.2f} us per GEMM in the graph\n")
+            print("| phase (us after the launch's earliest griddepcontrol.wait return) | min | median | max |\n|---|---|---|---|")
+            for k in (0, 13, 1, 2, 3, 4, 5, 6, 7, 8, 9, 11):
+                v = a[act, k]
+                v = v[v > 0]
+                if v.size:
+                    print(f"| {names[k]} | {(v.min() - base) / 1e3:.2f} | {(np.median(v) - base) / 1e3:.2f} | {(v.max() - base) / 1e3:.2f} |")
+            print(f"| next launch: griddepcontrol.wait returned | {(nxt[nxt[:, 0] > 0, 2].min() - base) / 1e3:.2f} | | |\n")
+    L.heal_debug_read_pair_trace.argtypes = [ctypes.c_void_p, ctypes.c_int]
+    print("## CTA-pair kernel: where the MMA thread and an epilogue warp wait (clock64 counters, median over the 74 pairs)\n")
+    print("| GEMM | MMA thread: waits for operands | waits for a free accumulator | issues | epilogue warp: waits for a segment | drains TMEM (cycles per segment) | stores C (cycles per tile) |\n|---|---|---|---|---|---|---|")
+    for name, M, N, K in SHAPES:
+        A = torch.randn(M, K, device="cuda")
+        W = (torch.randn(K, N, device="cuda") * 0.02).half()
+        ah, al = hb.heal_split(A)
+        C = torch.empty(M, N, device="cuda")
+        for _ in range(5):
+            hb.heal_gemm_presplit(ah, al, W, None, hb.MODE_2P, C=C)
+        torch.cuda.synchronize()
+        buf = (ctypes.c_ulonglong * (74 * 8))()
+        L.heal_debug_read_pair_trace(buf, 74 * 8)
+        t = np.array(buf[:], dtype=np.float64).reshape(74, 8)
+        tiles = (M // 256) * (N // 256) / 74.0
+        print(f"| {name} {M}x{N}x{K} | {np.median(t[:, 0] / t[:, 2]) * 100:.1f} % | {np.median(t[:, 1] / t[:, 2]) * 100:.1f} % | "
+              f"{100 - np.median((t[:, 0] + t[:, 1]) / t[:, 2]) * 100:.1f} % | {np.median(t[:, 3] / t[:, 6]) * 100:.1f} % | "
+              f"{np.median(t[:, 4] / t[:, 6]) * 100:.1f} % ({np.median(t[:, 4] / t[:, 7]):.0f}) | {np.median(t[:, 5] / t[:, 6]) * 100:.1f} % ({np.median(t[:, 5]) / tiles:.0f}) |")
+
+
 def relaunch_under_torchrun(args):
     """`python bench.py --gpus N` (N > 1) outside torchrun: start N ranks of this script, one per GPU, rendezvous on 127.0.0.1."""
     import subprocess
@@ -502,7 +577,11 @@ if __name__ == "__main__":
     ap.add_argument("--warmup", type=int, default=10)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--full", action="store_true", help="also time the qkv / o-proj / Qwen3-14B / mid-size-M shapes (key `shapes`)")
+    ap.add_argument("--trace", action="store_true", help="diagnostics: phase stamps / wait counters from a -DHEAL_TRACE build (markdown)")
     a = ap.parse_args()
+    if a.trace:
+        run_trace()
+        raise SystemExit(0)
     if a.gpus > 1 and "WORLD_SIZE" not in os.environ:
         relaunch_under_torchrun(a)
     run_reference(a) if a.impl == "reference" else run_ours(a)

@@ -1,6 +1,9 @@
 """Build libheal.so in-tree with nvcc for sm_100a (cross-compiles without a GPU).
 
-    python -m paper_2606_21023_b200.build [--force]
+    python -m paper_2606_21023_b200.build [--force] [-v] [--trace]
+
+--trace builds libheal_trace.so instead: the same sources with -DHEAL_TRACE (%globaltimer phase stamps in the small-M kernel, wait
+counters in the CTA-pair kernel), used only by `bench.py --trace`; the product library has none of it.
 """
 from __future__ import annotations
 
@@ -12,6 +15,7 @@ import sys
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _CSRC = os.path.join(_HERE, "csrc")
 LIB_PATH = os.path.join(_HERE, "libheal.so")
+TRACE_LIB_PATH = os.path.join(_HERE, "libheal_trace.so")
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-shared", "-Xcompiler", "-fPIC", "--split-compile", "0"]     # parallel back end: 2m20 -> 1m
@@ -26,17 +30,18 @@ def _deps():
         [os.path.join(_HERE, "..", "include", "heal.h")]
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
-    if not force and os.path.exists(LIB_PATH) and \
-            os.path.getmtime(LIB_PATH) >= max(os.path.getmtime(p) for p in _deps()):
-        return LIB_PATH
+def build(force: bool = False, verbose: bool = False, trace: bool = False) -> str:
+    out = TRACE_LIB_PATH if trace else LIB_PATH
+    if not force and os.path.exists(out) and \
+            os.path.getmtime(out) >= max(os.path.getmtime(p) for p in _deps()):
+        return out
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-    tmp = LIB_PATH + ".tmp%d" % os.getpid()
-    cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", tmp] + _sources()
+    tmp = out + ".tmp%d" % os.getpid()
+    cmd = [nvcc] + NVCC_FLAGS + (["-DHEAL_TRACE"] if trace else []) + (["-Xptxas", "-v"] if verbose else []) + ["-o", tmp] + _sources()
     subprocess.check_call(cmd)
-    os.replace(tmp, LIB_PATH)
-    return LIB_PATH
+    os.replace(tmp, out)
+    return out
 
 
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
+    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv, trace="--trace" in sys.argv))

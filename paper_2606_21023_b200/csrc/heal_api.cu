@@ -1067,6 +1067,11 @@ int heal_debug_force_kernel(int which)
 }
 
 #ifdef HEAL_TRACE
+// trace builds only (not part of include/heal.h): the pair kernel's wait counters of the most recent launch, 8 values per CTA pair
+int heal_debug_read_pair_trace(unsigned long long *host, int n)
+{
+    return static_cast<int>(cudaMemcpyFromSymbol(host, heal::g_pair_trace, static_cast<size_t>(n) * sizeof(unsigned long long)));
+}
 // trace builds only (not part of include/heal.h): device buffer of 16 x 1024 x 16 uint64 phase stamps
 int heal_debug_set_trace(void *ptr)
 {

@@ -16,6 +16,16 @@
 
 namespace heal {
 
+#ifdef HEAL_TRACE
+// trace builds only (python -m paper_2606_21023_b200.build --trace; the product library compiles all of this out): per CTA pair,
+// cycles the MMA thread waited for operands / for a free accumulator / in total, and cycles one epilogue warp of the leader
+// waited for a finished segment / drained TMEM / stored C / in total.  Read back with heal_debug_read_pair_trace().
+__device__ unsigned long long g_pair_trace[512 * 8];
+#define HEAL_TCLK() clock64()
+#else
+#define HEAL_TCLK() 0ll
+#endif
+
 template <int BN_, int NPROD_, bool B_MN_, bool FULL_ = false>
 struct Gemm2Cfg {
     static constexpr bool FULL = FULL_;                 // with the extended epilogue (2^-p scale, chained planes, accumulate) and the
@@ -141,17 +151,23 @@ heal_gemm_umma2_kernel(const __grid_constant__ CUtensorMap tm_a_hi, const __grid
             uint32_t phase = 0;
             int buf = 0;
             uint32_t tphase = 0;
+            long long w_full = 0, w_tempty = 0;
+            const long long t_begin = HEAL_TCLK();
             for (int ci = 0; ci < sched.n_chunks; ++ci) {
                 int tile, sb_seg, se_seg;
                 sched.get(ci, tile, sb_seg, se_seg);
                 for (int seg = sb_seg; seg < se_seg; ++seg) {
+                    const long long t0 = HEAL_TCLK();
                     mbar_wait_ool(tempty_bar(buf), ((tphase >> buf) & 1u) ^ 1u, args.diag, 300 + buf);
+                    w_tempty += HEAL_TCLK() - t0;
                     tc_fence_after();
                     const uint32_t d_tmem = tmem_base + static_cast<uint32_t>(buf * BN);
                     const int kt_end = min(k_tiles, (seg + 1) * kTilesPerSeg);
                     uint32_t accumulate = 0;
                     for (int kt = seg * kTilesPerSeg; kt < kt_end; ++kt) {
+                        const long long t1 = HEAL_TCLK();
                         mbar_wait_ool(full_bar(stage), phase, args.diag, 200 + stage);
+                        w_full += HEAL_TCLK() - t1;
                         tc_fence_after();
                         const uint32_t sb = smem_base + stage * Cfg::STAGE_BYTES;
                         const uint64_t a_hi = adesc0 | desc_addr(sb);
@@ -178,6 +194,15 @@ heal_gemm_umma2_kernel(const __grid_constant__ CUtensorMap tm_a_hi, const __grid
                     buf ^= 1;
                 }
             }
+#ifdef HEAL_TRACE
+            if ((blockIdx.x >> 1) < 512) {
+                unsigned long long *tr = g_pair_trace + (blockIdx.x >> 1) * 8;
+                tr[0] = static_cast<unsigned long long>(w_full);
+                tr[1] = static_cast<unsigned long long>(w_tempty);
+                tr[2] = static_cast<unsigned long long>(HEAL_TCLK() - t_begin);
+            }
+#endif
+            (void)w_full; (void)w_tempty; (void)t_begin;
         }
     } else if (warp >= 4) {
         // ================================ epilogue (both CTAs) =========================
@@ -188,6 +213,8 @@ heal_gemm_umma2_kernel(const __grid_constant__ CUtensorMap tm_a_hi, const __grid
         float run[CPW];
         int buf = 0;
         uint32_t tphase = 0;
+        long long e_wait = 0, e_drain = 0, e_store = 0, e_segs = 0;
+        const long long e_begin = HEAL_TCLK();
         for (int ci = 0; ci < sched.n_chunks; ++ci) {
             int tile, sb_seg, se_seg;
             sched.get(ci, tile, sb_seg, se_seg);
@@ -214,7 +241,9 @@ heal_gemm_umma2_kernel(const __grid_constant__ CUtensorMap tm_a_hi, const __grid
             if (sb_seg > 0)        // same rank of the previous pair
                 epi_take_prefix<CPW>(args.xfer + static_cast<size_t>(blockIdx.x - 2) * (kBM * 256), args.flags + (blockIdx.x - 2), run, etid, args.diag);
             for (int seg = sb_seg; seg < se_seg; ++seg) {
+                const long long t0 = HEAL_TCLK();
                 mbar_wait_ool(tfull_bar(buf), (tphase >> buf) & 1u, args.diag, 400 + buf);
+                const long long t1 = HEAL_TCLK();
                 tc_fence_after();
                 const uint32_t taddr = tmem_base + (static_cast<uint32_t>(quad * 32) << 16) +
                                        static_cast<uint32_t>(buf * BN + chalf * CPW);
@@ -222,6 +251,9 @@ heal_gemm_umma2_kernel(const __grid_constant__ CUtensorMap tm_a_hi, const __grid
                 tc_fence_before();
                 __syncwarp();
                 if (lane == 0) mbar_arrive_cluster(leader_addr(tempty_bar(buf)));
+                e_wait += t1 - t0;
+                e_drain += HEAL_TCLK() - t1;
+                ++e_segs;
                 tphase ^= 1u << buf;
                 buf ^= 1;
             }
@@ -229,8 +261,21 @@ heal_gemm_umma2_kernel(const __grid_constant__ CUtensorMap tm_a_hi, const __grid
                 epi_hand_on<CPW>(args.xfer + static_cast<size_t>(blockIdx.x) * (kBM * 256), args.flags + blockIdx.x, run, etid);
                 continue;
             }
+            const long long t2 = HEAL_TCLK();
             epi_store<CPW, Cfg::FULL>(args.out, m0 + quad * 32 + lane, n0 + chalf * CPW, run, args.M, args.N);
+            e_store += HEAL_TCLK() - t2;
         }
+#ifdef HEAL_TRACE
+        if (etid == 0 && rank == 0 && (blockIdx.x >> 1) < 512) {
+            unsigned long long *tr = g_pair_trace + (blockIdx.x >> 1) * 8;
+            tr[3] = static_cast<unsigned long long>(e_wait);
+            tr[4] = static_cast<unsigned long long>(e_drain);
+            tr[5] = static_cast<unsigned long long>(e_store);
+            tr[6] = static_cast<unsigned long long>(HEAL_TCLK() - e_begin);
+            tr[7] = static_cast<unsigned long long>(e_segs);
+        }
+#endif
+        (void)e_wait; (void)e_drain; (void)e_store; (void)e_begin; (void)e_segs;
     }
 
     tc_fence_before();
