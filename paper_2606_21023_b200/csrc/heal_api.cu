@@ -1422,6 +1422,23 @@ int heal_gemm_host(int64_t M, int64_t N, int64_t K, const void *A_host, int64_t 
     HEAL_CUDA(cudaStreamWaitEvent(g.copy_out, g.ev_start, 0));
     HEAL_CUDA(cudaMemcpy2DAsync(dA, dlda * 4, A_host, lda * 4, K * 4, M, cudaMemcpyHostToDevice, g.copy_in));
     const char *Bh = static_cast<const char *>(B_host);
+    // The activations are the same for every block: with FP16 weights and more tokens than the fused decode path takes, split
+    // them once (step S) instead of once per block; the blocks then run steps G + E on the planes.  Same bits either way.
+    __half *a_hi = nullptr, *a_lo = nullptr;
+    int64_t lda_p = 0;
+    if (nprod <= 2 && M > 32 && !(mode & (HEAL_LO_SCALED | HEAL_FUSE_SPLIT))) {
+        const WsPlan p = plan_ws(M, kBlockCols, K, nprod, b_nk);
+        void *ws = nullptr;
+        st = get_ws(p.total, stream, &ws);
+        if (st) return st;
+        a_hi = static_cast<__half *>(ws);
+        a_lo = reinterpret_cast<__half *>(static_cast<char *>(ws) + p.a_plane);
+        lda_p = p.lda_p;
+        HEAL_CUDA(cudaEventRecord(g.ev_start, g.copy_in));                   // A has arrived
+        HEAL_CUDA(cudaStreamWaitEvent(stream, g.ev_start, 0));
+        st = launch_split(M, K, reinterpret_cast<const float *>(dA), dlda, a_hi, a_lo, lda_p, stream);
+        if (st) return st;
+    }
     for (int64_t b = 0; b < nb; ++b) {
         const int64_t c0 = b * kBlockCols, cw = (N - c0 < kBlockCols) ? N - c0 : kBlockCols;
         if (b >= kEv) HEAL_CUDA(cudaEventSynchronize(g.ev_done[b % kEv]));       // block b - kEv fully consumed: its events are free
@@ -1434,7 +1451,17 @@ int heal_gemm_host(int64_t M, int64_t N, int64_t K, const void *A_host, int64_t 
                                         cudaMemcpyHostToDevice, g.copy_in));
         HEAL_CUDA(cudaEventRecord(g.ev_in[b % kEv], g.copy_in));
         HEAL_CUDA(cudaStreamWaitEvent(stream, g.ev_in[b % kEv], 0));
-        st = heal_gemm(M, cw, K, dA, dlda, b_nk ? dB + c0 * dldb * b_es : dB + c0 * b_es, dldb, dC + c0 * 4, dldc, mode, stream_);
+        const void *Bblk = b_nk ? dB + c0 * dldb * b_es : dB + c0 * b_es;
+        if (a_hi) {
+            // FP16 weights, activations split once before the loop: steps G + E on the planes
+            heal::OutArgs out = {};
+            out.C = reinterpret_cast<float *>(dC + c0 * 4);
+            out.ldc = dldc;
+            out.scale = 1.0f;
+            st = presplit_impl(M, cw, K, a_hi, a_lo, lda_p, Bblk, nullptr, dldb, out, nprod, b_nk, false, stream);
+        } else {
+            st = heal_gemm(M, cw, K, dA, dlda, Bblk, dldb, dC + c0 * 4, dldc, mode, stream_);
+        }
         if (st) return st;
         HEAL_CUDA(cudaEventRecord(g.ev_done[b % kEv], stream));
         HEAL_CUDA(cudaStreamWaitEvent(g.copy_out, g.ev_done[b % kEv], 0));
