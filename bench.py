@@ -226,11 +226,11 @@ def shape_report(hb, peaks, M, N, K, nprod, dist="normal", cublas=True, flags=0)
     return out
 
 
-def mlp_block_report(hb):
-    """The MLP block of Algorithm 1 at Llama-3-8B size, M = 2048, through the fused entry points: Norm -> split,
+def mlp_block_report(hb, M=2048):
+    """The MLP block of Algorithm 1 at Llama-3-8B size, M tokens, through the fused entry points: Norm -> split,
     gate_up GEMM with the SiLU-mul epilogue (activation planes out), down GEMM adding onto the residual: three launches."""
     import torch
-    M, D, FF = 2048, 4096, 14336
+    D, FF = 4096, 14336
     gen = torch.Generator(device="cuda")
     gen.manual_seed(5)
     H = torch.randn(M, D, device="cuda", generator=gen)
@@ -249,10 +249,14 @@ def mlp_block_report(hb):
     n0 = hb.launch_count()
     block()
     launches = hb.launch_count() - n0
-    t = time_calls([block], False)
+    t = time_calls([block] * (1 if M > 64 else 8), M <= 64)
     flop = 2.0 * M * D * (2 * FF) + 2.0 * M * FF * D
-    return {"shape": "M=2048, d=4096, ff=14336 (gate_up interleaved 4096x28672, down 14336x4096)", "launches": int(launches), "us": t,
-            "eff_tflops": flop / t / 1e6, "tensor_tflops": 2 * flop / t / 1e6}
+    byt = 2.0 * (D * 2 * FF + FF * D)                                   # FP16 weights: what a decode-sized block has to stream
+    out = {"shape": f"M={M}, d=4096, ff=14336 (gate_up interleaved 4096x28672, down 14336x4096)", "launches": int(launches), "us": t,
+           "eff_tflops": flop / t / 1e6, "tensor_tflops": 2 * flop / t / 1e6}
+    if M <= 64:
+        out["weights_GBps"] = byt / t / 1e3                               # (weights stay the same copy: 352 MB per block > L2)
+    return out
 
 
 def small_m_report(hb, peaks):
@@ -465,6 +469,7 @@ def run_ours(args):
             line["square"] = {str(n): shape_report(hb, peaks, n, n, n, 3, dist="uniform") for n in (1024, 2048, 4096, 8192)}
             line["lm_head_M512"] = shape_report(hb, peaks, 512, 128256, 4096, 2)
             line["mlp_block"] = mlp_block_report(hb)
+            line["mlp_block_decode_M8"] = mlp_block_report(hb, M=8)
             if args.full:
                 extra = [("L3-8B qkv", 2048, 6144, 4096), ("L3-8B o-proj", 2048, 4096, 4096), ("Q3-14B gate_up", 2048, 17408, 5120),
                          ("Q3-14B down", 2048, 5120, 17408), ("Q3-14B qkv", 2048, 7168, 5120), ("decode down M=1", 1, 4096, 14336),

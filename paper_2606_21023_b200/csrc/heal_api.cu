@@ -963,8 +963,7 @@ int presplit_impl(int64_t M, int64_t N, int64_t K, const void *A_hi, const void 
         return HEAL_OK;
     }
     const int force = forced_kernel();
-    // (the SiLU-mul epilogue pairs adjacent columns inside one thread: large-M kernels only)
-    if (((M <= 64 && force != 1) || (force == 2 && M <= 64)) && !out.silu) {
+    if ((M <= 64 && force != 1) || (force == 2 && M <= 64)) {
         bool handled = false;
         const SmallIn in{A_hi, A_lo, lda, A32, lda32, b_static};
         int st = b_nk ? launch_small<false>(nprod, M, N, K, in, B_hi, B_lo, ldb, out, stream, &handled)
@@ -1268,7 +1267,7 @@ int heal_gemm_ex(int64_t M, int64_t N, int64_t K, const void *A, int64_t lda, co
     static const long fused_max_m = std::getenv("HEAL_FUSED_MAX_M") ? std::atol(std::getenv("HEAL_FUSED_MAX_M")) : 0;        // tuning
     const bool fuse_small = fused_max_m > 0 ? (M <= fused_max_m && K <= 16384)
                                             : ((M <= 16 && K <= 16384) || (M <= 32 && K <= 8192 && N * K <= (static_cast<int64_t>(32) << 20)));
-    if (fuse_small && !b_f32 && !no_fused && !lo_scaled && !out.silu && forced_kernel() != 1) {
+    if (fuse_small && !b_f32 && !no_fused && !lo_scaled && forced_kernel() != 1) {
         bool handled = false;
         st = presplit_impl(M, N, K, nullptr, nullptr, 0, B, nullptr, ldb, out, nprod, b_nk, b_static, stream,
                            static_cast<const float *>(A), lda, &handled);

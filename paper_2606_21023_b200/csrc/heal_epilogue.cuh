@@ -22,7 +22,7 @@ struct OutArgs {
     int accumulate;       // C += scaled result (needs C): the residual add "A_i + GEMM(...)" of Algorithm 1 with
                           // C holding A_i (HEAL_EPI_ACCUMULATE), and the second launch of the two-GEMM scaled-lo form
     int silu;             // HEAL_EPI_SILU_MUL: the GEMM's columns are (gate, up) pairs -- column 2j = g_j, 2j+1 = u_j -- and the
-                          // outputs (C and/or planes, N/2 columns wide) receive SiLU(g_j) * u_j; large-M kernels only
+                          // outputs (C and/or planes, N/2 columns wide) receive SiLU(g_j) * u_j
 };
 
 // The output mode is uniform for the launch.  The store loops of the kernels are fully unrolled, run once per CTA (cold
@@ -140,9 +140,17 @@ __device__ __noinline__ void emit4_any(float *C, int64_t ldc, __half *hi, __half
         }
     }
 }
-__device__ __noinline__ void emit1_any(float *C, int64_t ldc, __half *hi, __half *lo, int64_t ld16, int accumulate,
+__device__ __noinline__ void emit1_any(float *C, int64_t ldc, __half *hi, __half *lo, int64_t ld16, int accumulate, int silu,
                                        int64_t row, int col, float v)
 {
+    if (silu) {
+        // small-M kernel: a warp's lanes are consecutive columns of one token, so the (gate, up) pair of output column col/2
+        // sits in lanes 2j, 2j+1 (panels start at even columns, N is even: both lanes of a pair are always active together)
+        const float other = __shfl_xor_sync(__activemask(), v, 1);
+        if (col & 1) return;
+        v = silu_mul(v, other);
+        col >>= 1;
+    }
     if (C) {
         float *c = C + row * ldc + col;
         if (accumulate) v = __fadd_rn(*c, v);
@@ -192,7 +200,7 @@ __device__ __forceinline__ void emit1(const OutArgs &o, int64_t row, int col, fl
 {
     v *= o.scale;
     if (FAST) o.C[row * o.ldc + col] = v;
-    else emit1_any(o.C, o.ldc, o.hi, o.lo, o.ld16, o.accumulate, row, col, v);
+    else emit1_any(o.C, o.ldc, o.hi, o.lo, o.ld16, o.accumulate, o.silu, row, col, v);
 }
 
 }  // namespace heal

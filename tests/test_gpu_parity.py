@@ -608,6 +608,31 @@ def test_silu_mul_and_accumulate_epilogue(hb, oracle, inputs, M, N, K, nprod):
     assert np.array_equal(rh.cpu().numpy().view(np.uint16), oh) and np.array_equal(rl.cpu().numpy().view(np.uint16), ol)
 
 
+@pytest.mark.parametrize("M,N,K", [(1, 4096, 4096), (8, 1032, 1024), (32, 520, 4096), (64, 28672, 512), (40, 264, 8192)])
+def test_silu_mul_small_m_kernel_bit_identical(hb, inputs, M, N, K):
+    """Decode-sized M: the SiLU-mul epilogue of the small-M kernel (the (gate, up) pair sits in two adjacent lanes) gives the bits
+    of the large-M kernels (pair inside one thread) -- fused-split, cluster-reduction, single-CTA and TMEM-ring variants -- for
+    the FP32 activations, the planes and the residual add."""
+    A = dev(inputs.activations(M, K, seed=64, outliers=True))
+    W = dev(inputs.weights_f16(K, N, seed=64, sigma=0.05))
+    R = dev(inputs.activations(M, N // 2, seed=65))
+    try:
+        hb.debug_force_kernel(0)
+        c0, h0, l0 = hb.heal_gemm_ex(A, W, 2 | hb.EPI_SILU_MUL)
+        ah, al = hb.heal_split(A)
+        c1, h1, l1 = hb.heal_gemm_presplit_ex(ah, al, W, None, 2 | hb.EPI_SILU_MUL)
+        r0 = R.clone()
+        hb.heal_gemm(A, W, 2 | hb.EPI_SILU_MUL | hb.EPI_ACCUMULATE, C=r0)
+        hb.debug_force_kernel(1)
+        c2, h2, l2 = hb.heal_gemm_ex(A, W, 2 | hb.EPI_SILU_MUL)
+    finally:
+        hb.debug_force_kernel(0)
+    torch.cuda.synchronize()
+    assert torch.equal(c0, c2) and torch.equal(h0, h2) and torch.equal(l0, l2)
+    assert torch.equal(c1, c2) and torch.equal(h1, h2) and torch.equal(l1, l2)
+    assert torch.equal(r0, R + c2)
+
+
 def test_silu_mul_ragged_last_pair(hb, oracle, inputs):
     """N = 522: the last group of four GEMM columns holds a single (gate, up) pair; N/2 = 261 outputs in padded buffers."""
     M, N, K = 200, 522, 1024
