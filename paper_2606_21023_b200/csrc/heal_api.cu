@@ -376,6 +376,8 @@ bool wants_split_k(int64_t tiles, int64_t n_seg, int64_t G_max, int ctas_per_til
 int64_t set_balance(GemmArgs &args, int64_t tiles, int64_t n_seg, int64_t G_max, int ctas_per_tile, int bn, bool full_kernel,
                     cudaStream_t stream)
 {
+    static const int group_m = std::getenv("HEAL_GROUP_M") ? std::atoi(std::getenv("HEAL_GROUP_M")) : kGroupM;      // tuning
+    args.group_m = group_m > 0 ? group_m : kGroupM;
     args.xfer = nullptr;
     args.flags = nullptr;
     args.part = nullptr;
@@ -443,7 +445,7 @@ int launch_sk_reduce(const GemmArgs &args, int ctas_per_tile, int64_t tiles, cud
     cfg.numAttrs = fill_attrs(attr, 1);
     cfg.attrs = attr;
     HEAL_CUDA(cudaLaunchKernelEx(&cfg, heal_splitk_reduce_kernel<BN>, static_cast<const float *>(args.part), n_seg, ctas_per_tile,
-                                 args.tiles_m, static_cast<int>(shares), args.out, args.M, args.N));
+                                 args.tiles_m, args.tiles_n, args.group_m, static_cast<int>(shares), args.out, args.M, args.N));
     g_launches.fetch_add(1);
     return HEAL_OK;
 }

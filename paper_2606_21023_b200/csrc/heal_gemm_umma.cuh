@@ -52,6 +52,7 @@ struct GemmArgs {
     OutArgs out;            // step E: FP32 C and/or hi/lo planes, optional 2^-p scale
     int M, N, K;
     int tiles_m, tiles_n;
+    int group_m;            // row tiles per rasterisation group (heal_sched.h tile_coords)
     int *diag;
     // segment-granular load balancing (0 = plain tile round-robin)
     int balance;
@@ -177,7 +178,7 @@ __device__ __forceinline__ void sk_store_partial(float *part, uint32_t taddr, in
 // `share` finishes float4 chunks [share*NC/shares, (share+1)*NC/shares) of every row of the unit's 128 x BN block.
 template <int BN>
 __global__ void __launch_bounds__(256)
-heal_splitk_reduce_kernel(const float *__restrict__ part, int n_seg, int R, int tiles_m, int shares, const OutArgs out, int M, int N)
+heal_splitk_reduce_kernel(const float *__restrict__ part, int n_seg, int R, int tiles_m, int tiles_n, int group_m, int shares, const OutArgs out, int M, int N)
 {
     pdl_wait();
     pdl_launch_dependents();
@@ -185,8 +186,10 @@ heal_splitk_reduce_kernel(const float *__restrict__ part, int n_seg, int R, int 
     const int unit = static_cast<int>(blockIdx.x) / shares, share = static_cast<int>(blockIdx.x) % shares;
     const int tile = unit / R, rank = unit % R;
     const int etid = threadIdx.x, warp = etid >> 5, lane = etid & 31, quad = warp & 3, chalf = warp >> 2;
-    const int64_t row = static_cast<int64_t>(tile % tiles_m) * (R * kBM) + rank * kBM + quad * 32 + lane;
-    const int col0 = (tile / tiles_m) * BN + chalf * CPW;
+    int tm, tn;
+    tile_coords(tile, tiles_m, tiles_n, tm, tn, group_m);
+    const int64_t row = static_cast<int64_t>(tm) * (R * kBM) + rank * kBM + quad * 32 + lane;
+    const int col0 = tn * BN + chalf * CPW;
     const float4 *src = reinterpret_cast<const float4 *>(part + static_cast<size_t>(unit) * n_seg * (kBM * BN));
     const size_t seg_stride = static_cast<size_t>(kBM) * BN / 4;               // float4 per partial
     const int c_lo = share * NC / shares, c_hi = (share + 1) * NC / shares;
@@ -279,8 +282,10 @@ heal_gemm_umma_kernel(const __grid_constant__ CUtensorMap tm_a_hi, const __grid_
             for (int ci = 0; ci < sched.n_chunks; ++ci) {
                 int tile, sb_seg, se_seg;
                 sched.get(ci, tile, sb_seg, se_seg);
-                const int m0 = (tile % args.tiles_m) * kBM;
-                const int n0 = (tile / args.tiles_m) * BN;
+                int tm, tn;
+                tile_coords(tile, args.tiles_m, args.tiles_n, tm, tn, args.group_m);
+                const int m0 = tm * kBM;
+                const int n0 = tn * BN;
                 const int kt_hi = min(k_tiles, se_seg * kTilesPerSeg);
                 for (int kt = sb_seg * kTilesPerSeg; kt < kt_hi; ++kt) {
                     mbar_wait_ool(empty_bar(stage), phase ^ 1u, args.diag, 100 + stage);
@@ -371,8 +376,10 @@ heal_gemm_umma_kernel(const __grid_constant__ CUtensorMap tm_a_hi, const __grid_
         for (int ci = 0; ci < sched.n_chunks; ++ci) {
             int tile, sb_seg, se_seg;
             sched.get(ci, tile, sb_seg, se_seg);
-            const int m0 = (tile % args.tiles_m) * kBM;
-            const int n0 = (tile / args.tiles_m) * BN;
+            int tm, tn;
+            tile_coords(tile, args.tiles_m, args.tiles_n, tm, tn, args.group_m);
+            const int m0 = tm * kBM;
+            const int n0 = tn * BN;
             if constexpr (Cfg::FULL) {
                 if (args.sk) {
                     // ordered split-K: park every segment partial in global memory; heal_splitk_reduce_kernel forms the sums

@@ -112,8 +112,10 @@ heal_gemm_umma2_kernel(const __grid_constant__ CUtensorMap tm_a_hi, const __grid
             for (int ci = 0; ci < sched.n_chunks; ++ci) {
                 int tile, sb_seg, se_seg;
                 sched.get(ci, tile, sb_seg, se_seg);
-                const int m0 = (tile % args.tiles_m) * (2 * kBM) + rank * kBM;
-                const int n0 = (tile / args.tiles_m) * BN + rank * Cfg::BH;
+                int tm, tn;
+                tile_coords(tile, args.tiles_m, args.tiles_n, tm, tn, args.group_m);
+                const int m0 = tm * (2 * kBM) + rank * kBM;
+                const int n0 = tn * BN + rank * Cfg::BH;
                 const int kt_hi = min(k_tiles, se_seg * kTilesPerSeg);
                 for (int kt = sb_seg * kTilesPerSeg; kt < kt_hi; ++kt) {
                     mbar_wait_ool(empty_bar(stage), phase ^ 1u, args.diag, 100 + stage);
@@ -218,8 +220,10 @@ heal_gemm_umma2_kernel(const __grid_constant__ CUtensorMap tm_a_hi, const __grid
         for (int ci = 0; ci < sched.n_chunks; ++ci) {
             int tile, sb_seg, se_seg;
             sched.get(ci, tile, sb_seg, se_seg);
-            const int m0 = (tile % args.tiles_m) * (2 * kBM) + rank * kBM;
-            const int n0 = (tile / args.tiles_m) * BN;
+            int tm, tn;
+            tile_coords(tile, args.tiles_m, args.tiles_n, tm, tn, args.group_m);
+            const int m0 = tm * (2 * kBM) + rank * kBM;
+            const int n0 = tn * BN;
             if constexpr (Cfg::FULL) {
                 if (args.sk) {
                     // ordered split-K (see heal_gemm_umma.cuh): park every segment partial of this CTA's 128 rows

@@ -121,8 +121,10 @@ heal_gemm_umma2f_kernel(const __grid_constant__ CUtensorMap tm_a32, const __grid
                 for (int ci = 0; ci < sched.n_chunks; ++ci) {
                     int tile, sb_seg, se_seg;
                     sched.get(ci, tile, sb_seg, se_seg);
-                    const int m0 = (tile % args.tiles_m) * (2 * kBM) + rank * kBM;
-                    const int n0 = (tile / args.tiles_m) * BN + rank * Cfg::BH;
+                    int tm, tn;
+                    tile_coords(tile, args.tiles_m, args.tiles_n, tm, tn, args.group_m);
+                    const int m0 = tm * (2 * kBM) + rank * kBM;
+                    const int n0 = tn * BN + rank * Cfg::BH;
                     const int kt_hi = min(k_tiles, se_seg * kTilesPerSeg);
                     for (int kt = sb_seg * kTilesPerSeg; kt < kt_hi; ++kt) {
                         mbar_wait(empty_bar(stage), phase ^ 1u, args.diag, 100 + stage);
@@ -277,8 +279,10 @@ heal_gemm_umma2f_kernel(const __grid_constant__ CUtensorMap tm_a32, const __grid
         for (int ci = 0; ci < sched.n_chunks; ++ci) {
             int tile, sb_seg, se_seg;
             sched.get(ci, tile, sb_seg, se_seg);
-            const int m0 = (tile % args.tiles_m) * (2 * kBM) + rank * kBM;
-            const int n0 = (tile / args.tiles_m) * BN;
+            int tm, tn;
+            tile_coords(tile, args.tiles_m, args.tiles_n, tm, tn, args.group_m);
+            const int m0 = tm * (2 * kBM) + rank * kBM;
+            const int n0 = tn * BN;
             if constexpr (Cfg::FULL) {
                 if (args.sk) {
                     for (int seg = sb_seg; seg < se_seg; ++seg) {

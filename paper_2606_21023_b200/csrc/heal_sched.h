@@ -10,6 +10,23 @@
 
 namespace heal {
 
+// Tile index -> (row tile, column tile).  Tiles are numbered in groups of kGroupM row tiles: inside a group the row tile runs fastest,
+// then the column tile; a group is finished before the next one starts.  A wave of consecutive tiles therefore covers a roughly square
+// patch (about 8 row tiles x G/8 column tiles), so per k-step the wave reads few distinct activation AND weight slabs and they stay
+// shared in L2 -- with plain row-fastest numbering every wave of a tall problem (8192^3: 32 row tiles) re-read all of A from HBM.
+// With at most kGroupM row tiles (all the LLM shapes at M <= 2048) this IS the row-fastest order.  Scheduling only: no bits change.
+constexpr int kGroupM = 8;
+HEAL_HD void tile_coords(int tile, int tiles_m, int tiles_n, int &tm, int &tn, int group_m = kGroupM)
+{
+    const int per_group = group_m * tiles_n;
+    const int g = tile / per_group;
+    const int first_m = g * group_m;
+    const int gm = (tiles_m - first_m < group_m) ? tiles_m - first_m : group_m;
+    const int r = tile - g * per_group;
+    tm = first_m + r % gm;
+    tn = r / gm;
+}
+
 // Work distribution.  The unit of work is (tile, K segment).  The first `dp_tiles` tiles (a multiple of
 // gridDim.x) are dealt round-robin, whole tiles, so the CTAs of a wave walk K in lockstep and share W / A
 // panels in L2.  With `balance`, the remaining tiles (the ragged last wave) are cut at segment granularity

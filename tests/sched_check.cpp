@@ -52,9 +52,27 @@ static int check(int tiles, int n_seg, int G, int balance, int dp_tiles)
     return 0;
 }
 
+// tile_coords is a bijection tile <-> (row tile, column tile)
+static int check_coords(int tiles_m, int tiles_n)
+{
+    std::vector<int> seen(static_cast<size_t>(tiles_m) * tiles_n, 0);
+    for (int t = 0; t < tiles_m * tiles_n; ++t) {
+        int tm = -1, tn = -1;
+        heal::tile_coords(t, tiles_m, tiles_n, tm, tn);
+        if (tm < 0 || tm >= tiles_m || tn < 0 || tn >= tiles_n) return 1;
+        if (seen[static_cast<size_t>(tm) * tiles_n + tn]++) return 2;
+    }
+    return 0;
+}
+
 int main()
 {
     long n = 0, bad = 0;
+    for (int tm = 1; tm <= 40; ++tm)
+        for (int tn = 1; tn <= 70; tn += (tn < 10 ? 1 : 7)) {
+            ++n;
+            if (check_coords(tm, tn)) { ++bad; std::printf("coords FAIL tiles_m %d tiles_n %d\n", tm, tn); }
+        }
     const int Gs[] = {1, 2, 3, 7, 74, 148};
     for (int G : Gs)
         for (int tiles = 1; tiles <= 700; tiles += (tiles < 40 ? 1 : 37))
