@@ -1070,15 +1070,15 @@ def test_segment_order_is_fp32_rn_ascending(hb):
 def test_soak_random_shapes_streams_and_flags(hb):
     """Short soak (a longer run of the same loop found two real bugs in round 1: hi/lo planes shared between streams,
     and HEAL_B_STATIC prefetching weight planes the library itself had just written): random shapes of every kernel
-    family on three streams, random HEAL_B_STATIC / extended-epilogue use, every result compared bit for bit with the
-    large-M kernels' result for the same inputs."""
+    family on three streams, random HEAL_B_STATIC / HEAL_FUSE_SPLIT / extended-epilogue use, every result compared bit for bit
+    with the large-M kernels' result for the same inputs."""
     import random
     import time
     rnd = random.Random(1)
     torch.manual_seed(1)
     shapes = [(1, 4096, 4096, 2), (8, 4096, 4096, 2), (16, 1032, 8192, 2), (32, 4096, 4096, 2), (64, 4096, 4096, 2), (40, 520, 14336, 2),
               (64, 32064, 4096, 2), (5, 26624, 2048, 2), (128, 4096, 4096, 2), (256, 1032, 4096, 2), (300, 520, 2056, 3), (700, 4104, 1032, 2),
-              (2048, 2048, 512, 2), (64, 256, 256, 3), (33, 264, 30000 // 8 * 8, 2)]
+              (2048, 2048, 512, 2), (64, 256, 256, 3), (33, 264, 30000 // 8 * 8, 2), (1300, 4104, 2056, 2), (4500, 1032, 520, 3)]
     cases = []
     try:
         hb.debug_force_kernel(1)
@@ -1097,7 +1097,7 @@ def test_soak_random_shapes_streams_and_flags(hb):
         outs = []
         for _ in range(12):
             A, B, nprod, ref = rnd.choice(cases)
-            flag = rnd.choice([0, hb.B_STATIC])
+            flag = rnd.choice([0, hb.B_STATIC, hb.FUSE_SPLIT, hb.FUSE_SPLIT | hb.B_STATIC])
             with torch.cuda.stream(rnd.choice(streams)):
                 if rnd.random() < 0.3:
                     C, _, _ = hb.heal_gemm_ex(A, B, nprod | flag, scale_exp=1)
