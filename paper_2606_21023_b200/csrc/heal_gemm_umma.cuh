@@ -40,8 +40,13 @@ struct GemmCfg {
     static constexpr int BAR_BYTES = 256;
     static constexpr int STAGES_RAW = (kSmemLimit - 1024 - BAR_BYTES) / STAGE_BYTES;
     static constexpr int STAGES = STAGES_RAW > 8 ? 8 : STAGES_RAW;
-    static constexpr int SMEM_BYTES = 1024 + STAGES * STAGE_BYTES + BAR_BYTES;
     static constexpr int TMEM_COLS = (2 * BN <= 32) ? 32 : (2 * BN <= 64) ? 64 : (2 * BN <= 128) ? 128 : (2 * BN <= 256) ? 256 : 512;
+    // TMEM can never be oversubscribed: a kernel takes at least the same fraction of an SM's shared memory (228 KB, 1 KB
+    // reserved per CTA) as of its 512 TMEM columns, so whatever mix of the library's CTAs fits an SM's shared memory also fits its TMEM --
+    // a CTA blocked in tcgen05.alloc while cluster peers hold TMEM elsewhere could otherwise close a wait cycle across streams.
+    static constexpr int SMEM_USED = 1024 + STAGES * STAGE_BYTES + BAR_BYTES;
+    static constexpr int SMEM_TMEM = TMEM_COLS * (228 * 1024 / 512) - 1024;
+    static constexpr int SMEM_BYTES = SMEM_USED > SMEM_TMEM ? SMEM_USED : SMEM_TMEM;
     static constexpr int COLS_PER_WARP = BN / 2;
     static_assert(BN % 32 == 0 && BN >= 32 && BN <= 256, "BN");
     static_assert(!B_MN || BN % 64 == 0, "MN-major B tiles are built from 64-column swizzle atoms");
