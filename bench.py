@@ -413,6 +413,15 @@ def run_ours(args):
     h2d = sum(A.numel() * 4 + W.numel() * 2 for _, A, W in host)
     d2h = sum(C.numel() * 4 for C in outs)
 
+    # ... and the inference form: weights resident on the device, only the step's activations travel in and the results out
+    def step_host_act():
+        for (_, A, W), (_, _, Wd, _), C in zip(host, devs, outs):
+            hb.heal_gemm_host_act(A, Wd, hb.MODE_2P, C=C)
+
+    step_host_act()
+    ms_e2e_act = timed(step_host_act, e2e_steps) / e2e_steps
+    h2d_act = sum(A.numel() * 4 for _, A, W in host)
+
     if rank == 0:
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
@@ -432,6 +441,9 @@ def run_ours(args):
                                      "source": "profiles/probes_r01.md, DESIGN.md section 7"}},
             "e2e": {"value": world * FLOP_STEP / (ms_e2e * 1e-3) / 1e12, "unit": UNIT, "h2d_bytes_per_step": h2d,
                     "d2h_bytes_per_step": d2h, "ms_per_step": ms_e2e},
+            "e2e_weights_resident": {"value": world * FLOP_STEP / (ms_e2e_act * 1e-3) / 1e12, "unit": UNIT, "h2d_bytes_per_step": h2d_act,
+                                     "d2h_bytes_per_step": d2h, "ms_per_step": ms_e2e_act,
+                                     "what": "heal_gemm_host_act: FP16 weights stay on the device (the inference case), activations and results cross PCIe every step"},
             "gpu_launches": int(launches),
             "clocks": sampler.summary(),
         }

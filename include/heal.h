@@ -201,6 +201,18 @@ int heal_gemm_host(int64_t M, int64_t N, int64_t K,
                    void *C_host, int64_t ldc,
                    uint32_t mode, void *stream);
 
+/*
+ * The inference form of the host variant: activations in, results out, WEIGHTS RESIDENT on the device.  A and C are HOST pointers
+ * (ideally pinned), B is a DEVICE pointer with the layout and alignment rules of heal_gemm.  Pipelined over blocks of 512 token rows
+ * on the library's two copy streams (activations in, compute, results out overlap); bit-identical to heal_gemm over all rows (the
+ * reduction order does not depend on M).  Synchronises `stream` before returning; calls are serialised inside the library.
+ */
+int heal_gemm_host_act(int64_t M, int64_t N, int64_t K,
+                       const void *A_host, int64_t lda,
+                       const void *B, int64_t ldb,
+                       void *C_host, int64_t ldc,
+                       uint32_t mode, void *stream);
+
 /* Bytes of workspace heal_gemm needs for this problem (hi/lo planes of A, and of B in 3P/4P). */
 size_t heal_workspace_size(int64_t M, int64_t N, int64_t K, uint32_t mode);
 

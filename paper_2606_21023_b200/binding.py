@@ -43,6 +43,8 @@ def lib():
         L.heal_gemm.argtypes = [i64, i64, i64, vp, i64, vp, i64, vp, i64, u32, vp]
         L.heal_gemm_host.restype = ci
         L.heal_gemm_host.argtypes = [i64, i64, i64, vp, i64, vp, i64, vp, i64, u32, vp]
+        L.heal_gemm_host_act.restype = ci
+        L.heal_gemm_host_act.argtypes = [i64, i64, i64, vp, i64, vp, i64, vp, i64, u32, vp]
         L.heal_split.restype = ci
         L.heal_split.argtypes = [i64, i64, vp, i64, vp, vp, i64, vp]
         L.heal_split_scaled.restype = ci
@@ -233,4 +235,16 @@ def heal_gemm_host(A: torch.Tensor, B: torch.Tensor, mode: int = MODE_2P, C: tor
         C = torch.empty((M, N), dtype=torch.float32).pin_memory()
     _check(lib().heal_gemm_host(M, N, K, A.data_ptr(), _ld(A), B.data_ptr(), _ld(B), C.data_ptr(), _ld(C), mode,
                                 _stream(stream)))
+    return C
+
+
+def heal_gemm_host_act(A: torch.Tensor, B: torch.Tensor, mode: int = MODE_2P, C: torch.Tensor | None = None, stream=None):
+    """Inference form of the host variant: pinned CPU activations in, CPU result out, weights resident on the device."""
+    assert not A.is_cuda and B.is_cuda and A.dtype == torch.float32
+    M, K = A.shape
+    N = B.shape[0] if mode & B_NK else B.shape[1]
+    if C is None:
+        C = torch.empty((M, N), dtype=torch.float32).pin_memory()
+    _check(lib().heal_gemm_host_act(M, N, K, A.data_ptr(), _ld(A), B.data_ptr(), _ld(B), C.data_ptr(), _ld(C), mode,
+                                    _stream(stream)))
     return C

@@ -1475,4 +1475,80 @@ int heal_gemm_host(int64_t M, int64_t N, int64_t K, const void *A_host, int64_t 
     return HEAL_OK;
 }
 
+int heal_gemm_host_act(int64_t M, int64_t N, int64_t K, const void *A_host, int64_t lda, const void *B, int64_t ldb,
+                       void *C_host, int64_t ldc, uint32_t mode, void *stream_)
+{
+    int nprod;
+    bool b_nk;
+    int st = validate_mode(mode, &nprod, &b_nk);
+    if (st) return st;
+    if (M < 0 || N < 0 || K < 0) return HEAL_ERR_INVALID_VALUE;
+    if (mode & (HEAL_EPI_SILU_MUL | HEAL_EPI_ACCUMULATE)) return HEAL_ERR_UNSUPPORTED_MODE;     // device entry points only
+    if (lda < K || ldc < N || ldb < (b_nk ? K : N)) return HEAL_ERR_INVALID_VALUE;
+    if (M == 0 || N == 0) return HEAL_OK;
+    if (!C_host || (K > 0 && (!A_host || !B))) return HEAL_ERR_NULL_POINTER;
+    if (K > 0 && (!aligned16(B) || (ldb & (nprod >= 3 ? 3 : 7)))) return HEAL_ERR_MISALIGNED;
+    st = ensure_init();
+    if (st) return st;
+    cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+    const int64_t dlda = round_up(K > 0 ? K : 1, 8), dldc = round_up(N, 4);
+    const size_t a_bytes = static_cast<size_t>(round_up(M * dlda * 4, 256));
+    const size_t c_bytes = static_cast<size_t>(round_up(M * dldc * 4, 256));
+    std::lock_guard<std::mutex> host_lk(g_host_mu);
+    struct Drain {
+        cudaStream_t s;
+        bool armed = true;
+        ~Drain()
+        {
+            if (!armed) return;
+            cudaStreamSynchronize(s);
+            if (g.copy_in) cudaStreamSynchronize(g.copy_in);
+            if (g.copy_out) cudaStreamSynchronize(g.copy_out);
+        }
+    } drain{stream};
+    if (a_bytes + c_bytes > g.stage_bytes) {
+        HEAL_CUDA(cudaStreamSynchronize(stream));
+        if (g.stage) HEAL_CUDA(cudaFree(g.stage));
+        g.stage = nullptr;
+        g.stage_bytes = 0;
+        HEAL_CUDA(cudaMalloc(&g.stage, a_bytes + c_bytes));
+        g.stage_bytes = a_bytes + c_bytes;
+    }
+    char *dA = static_cast<char *>(g.stage), *dC = dA + a_bytes;
+    if (!g.copy_in) {
+        HEAL_CUDA(cudaStreamCreateWithFlags(&g.copy_in, cudaStreamNonBlocking));
+        HEAL_CUDA(cudaStreamCreateWithFlags(&g.copy_out, cudaStreamNonBlocking));
+        for (auto &e : g.ev_in) HEAL_CUDA(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+        for (auto &e : g.ev_done) HEAL_CUDA(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+        HEAL_CUDA(cudaEventCreateWithFlags(&g.ev_start, cudaEventDisableTiming));
+    }
+    // Blocks of token rows: block b's activations travel in while block b-1 is computed and block b-2's results travel out.  Rows are
+    // independent and the reduction order does not depend on M, so the result is bit-identical to one heal_gemm over all rows.
+    const int64_t kBlockRows = 512;
+    const int64_t nb = (M + kBlockRows - 1) / kBlockRows;
+    constexpr int kEv = 8;
+    HEAL_CUDA(cudaEventRecord(g.ev_start, stream));
+    HEAL_CUDA(cudaStreamWaitEvent(g.copy_in, g.ev_start, 0));
+    HEAL_CUDA(cudaStreamWaitEvent(g.copy_out, g.ev_start, 0));
+    for (int64_t b = 0; b < nb; ++b) {
+        const int64_t r0 = b * kBlockRows, rows = (M - r0 < kBlockRows) ? M - r0 : kBlockRows;
+        if (b >= kEv) HEAL_CUDA(cudaEventSynchronize(g.ev_done[b % kEv]));
+        if (K > 0)
+            HEAL_CUDA(cudaMemcpy2DAsync(dA + r0 * dlda * 4, dlda * 4, static_cast<const char *>(A_host) + r0 * lda * 4, lda * 4, K * 4, rows,
+                                        cudaMemcpyHostToDevice, g.copy_in));
+        HEAL_CUDA(cudaEventRecord(g.ev_in[b % kEv], g.copy_in));
+        HEAL_CUDA(cudaStreamWaitEvent(stream, g.ev_in[b % kEv], 0));
+        st = heal_gemm(rows, N, K, dA + r0 * dlda * 4, dlda, B, ldb, dC + r0 * dldc * 4, dldc, mode, stream_);
+        if (st) return st;
+        HEAL_CUDA(cudaEventRecord(g.ev_done[b % kEv], stream));
+        HEAL_CUDA(cudaStreamWaitEvent(g.copy_out, g.ev_done[b % kEv], 0));
+        HEAL_CUDA(cudaMemcpy2DAsync(static_cast<char *>(C_host) + r0 * ldc * 4, ldc * 4, dC + r0 * dldc * 4, dldc * 4, N * 4, rows,
+                                    cudaMemcpyDeviceToHost, g.copy_out));
+    }
+    HEAL_CUDA(cudaStreamSynchronize(g.copy_out));
+    HEAL_CUDA(cudaStreamSynchronize(stream));
+    drain.armed = false;
+    return HEAL_OK;
+}
+
 }  // extern "C"

@@ -972,6 +972,20 @@ def test_host_variant_pipelined_blocks(hb, inputs, b_nk):
         assert torch.all(Ch[:, N:] == 7.0)
 
 
+@pytest.mark.parametrize("M,N,K,nprod", [(1300, 1032, 2056, 2), (40, 520, 1024, 2), (1025, 264, 520, 3)])
+def test_host_variant_with_resident_weights(hb, inputs, M, N, K, nprod):
+    """heal_gemm_host_act (host activations and results, device weights, pipelined over 512-row blocks with a ragged last block):
+    the bits of heal_gemm over all rows."""
+    A = inputs.activations(M, K, seed=91, outliers=True)
+    B = inputs.weights_f32(K, N, seed=91) if nprod >= 3 else inputs.weights_f16(K, N, seed=91)
+    Bd = dev(B)
+    ref = hb.heal_gemm(dev(A), Bd, nprod).cpu()
+    Ah = torch.from_numpy(A).pin_memory()
+    for _ in range(2):
+        C = hb.heal_gemm_host_act(Ah, Bd, nprod)
+        assert torch.equal(C, ref)
+
+
 def test_empty_and_k0(hb):
     A = torch.zeros((0, 64), device="cuda")
     W = torch.zeros((64, 16), dtype=torch.float16, device="cuda")
