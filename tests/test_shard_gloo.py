@@ -37,6 +37,20 @@ def _worker(rank, world, port, q):
     # M-sharding ranges
     rows = [None] * world
     dist.all_gather_object(rows, shard_rows(M, world, rank))
+    # M-sharding as bench.py does it: rank r GENERATES exactly its rows of the global activation matrix (rows are regenerable from
+    # (seed, row index)), runs the path on them, and the row blocks concatenate to the product over the global batch
+    from paper_2606_21023_b200.shard import aggregate_throughput
+    Mg = world * 16
+    r0, r1 = shard_rows(Mg, world, rank)
+    A_mine = inputs.activations(r1 - r0, K, seed=3, outliers=True, row0=r0)
+    A_glob = inputs.activations(Mg, K, seed=3, outliers=True)
+    mine_ok = np.array_equal(A_mine, A_glob[r0:r1])
+    mparts = [None] * world
+    dist.all_gather_object(mparts, (r0, oracle.gemm_f64(A_mine, W), mine_ok))
+    if rank == 0:
+        catm = np.concatenate([p[1] for p in sorted(mparts, key=lambda p: p[0])], axis=0)
+        assert all(p[2] for p in mparts) and np.array_equal(catm, oracle.gemm_f64(A_glob, W))
+        assert aggregate_throughput([5.0] * world, [1000.0, 2000.0][:world]) == 5.0 * world / max([1.0, 2.0][:world])
     # timing: max over ranks
     t = torch.tensor([10.0 + rank])
     dist.all_reduce(t, op=dist.ReduceOp.MAX)
