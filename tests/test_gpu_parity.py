@@ -108,6 +108,37 @@ def test_integer_exact(hb, inputs, M, N, K, nprod, b_nk):
     assert np.array_equal(got, want)
 
 
+def test_edge_dimension_sweep_integer_exact(hb):
+    """Ragged and minimal dimensions through every dispatch branch (fused small-M, cluster sizes, single-CTA tile widths 64/128/256,
+    CTA pairs, ordered split-K, HEAL_FUSE_SPLIT), both weight layouts, two and three products: 120 seeded (M, N, K) combinations of
+    tile-edge values, integer inputs with lo != 0 (entries up to +-4100 in A), so the result must equal the int64 GEMM bit for bit."""
+    import random
+    rnd = random.Random(7)
+    Ms = [1, 2, 15, 16, 17, 31, 32, 33, 63, 64, 65, 127, 128, 129, 255, 256, 257, 513]
+    Ns = [8, 24, 64, 72, 128, 136, 256, 264, 520]
+    Ks = [8, 24, 64, 72, 504, 512, 520, 1032]
+    g = torch.Generator(device="cpu")
+    g.manual_seed(11)
+    for it in range(120):
+        M, N, K = rnd.choice(Ms), rnd.choice(Ns), rnd.choice(Ks)
+        nprod = rnd.choice([2, 2, 3])
+        b_nk = rnd.random() < 0.4
+        # A: integers that need the lo plane (|a| up to 4100, not all representable in FP16); B in {-2..2}: sums < 2^24 for K <= 1032
+        Ai = torch.randint(-4100, 4101, (M, K), generator=g)
+        Bi = torch.randint(-2, 3, (K, N), generator=g)
+        ref = (Ai @ Bi).to(torch.float32)
+        A = Ai.to(torch.float32).cuda()
+        Bh = Bi.to(torch.float32 if nprod == 3 else torch.float16)
+        B = (Bh.t().contiguous() if b_nk else Bh).cuda()
+        mode = nprod | (hb.B_NK if b_nk else 0)
+        if M > 128 and N > 128 and rnd.random() < 0.5:
+            mode |= hb.FUSE_SPLIT
+        # pitches: N x K storage needs K % 8 (FP16) / % 4 (FP32); K x N storage needs N % 8 / % 4 -- all values above are multiples of 8
+        C = hb.heal_gemm(A, B, mode)
+        torch.cuda.synchronize()
+        assert torch.equal(C.cpu(), ref), (M, N, K, nprod, b_nk, hex(mode), it)
+
+
 @pytest.mark.parametrize("b_nk", [False, True])
 def test_lo_plane_exact(hb, inputs, b_nk):
     """Integers in [2049, 8191] are not FP16 numbers: lo != 0 and hi + lo = a exactly; with B in
