@@ -84,16 +84,16 @@ typedef enum {
                                      takes this path by itself when a captured call finds no workspace.  Ignored elsewhere. */
 
 #define HEAL_LO_SHIFT 10
-#define HEAL_LO_SCALED 0x40u   /* the paper's scaled residual, Eq. 10 as printed: h = h_hi +
-                                  h_lo / 2^10 with h_lo = r16((h - h_hi) * 2^10), C = GEMM(h_hi, W) +
-                                  GEMM(h_lo / 2^10, W).  Two-product mode only.  Computed the way the paper
-                                  computes it -- two FP16 tensor-core GEMMs summed into one FP32 output
-                                  (PAPER.md:571): the h_lo GEMM stores 2^-10 times its sum (exact), the h_hi GEMM
-                                  adds its own on top in FP32 RN; each keeps the reduction order above.  Differs
-                                  from the default (s = 0, one accumulator) only where h_lo would leave FP16's
-                                  normal range, i.e. for |h| < 2^-3 (reading A1); needs the FP32 output
-                                  C (not planes only) and costs two GEMM launches.  With heal_gemm_presplit(_ex)
-                                  A_lo must hold the scaled residual (heal_split_scaled with lo_shift = 10). */
+#define HEAL_LO_SCALED 0x40u   /* the paper's scaled residual, Eq. 10 as printed: h = h_hi + h_lo / 2^10 with
+                                  h_lo = r16((h - h_hi) * 2^10), C = GEMM(h_hi, W) + GEMM(h_lo / 2^10, W).  Two-product mode only.  One
+                                  kernel, one accumulator: inside every 512-long K segment the tensor core first accumulates the h_lo.W
+                                  products (k ascending), then scales that sum by 2^-10 (tcgen05.mma scale_input_d, an exact power of two)
+                                  as it adds the first h_hi.W product, then accumulates the remaining h_hi.W products; segment sums are
+                                  added in FP32 RN in ascending order as always.  Differs from the default (s = 0) only where h_lo would
+                                  leave FP16's normal range, i.e. for |h| < 2^-3 (reading A1).  The weight tile travels twice per
+                                  segment: about 8 % slower than the default on prefill shapes; every M runs the large-M kernels (same
+                                  bits for every M), so decode-sized M is about 2x slower than the default.  With
+                                  heal_gemm_presplit(_ex) A_lo must hold the scaled residual (heal_split_scaled with lo_shift = 10). */
 
 /*
  * C[M x N] (FP32) = A[M x K] (FP32) . B          one pass of the whole path: split, MMAs, epilogue.

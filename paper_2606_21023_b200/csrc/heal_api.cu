@@ -619,12 +619,13 @@ int launch_gemm2_np(int nprod, int64_t M, int64_t N, int64_t K, const void *A_hi
                     const void *B_hi, const void *B_lo, int64_t ldb, const OutArgs &out, cudaStream_t s)
 {
     const int64_t tiles = ((M + 2 * kBM - 1) / (2 * kBM)) * ((N + 255) / 256);
-    if (needs_ext(out) || wants_split_k(tiles, (K + kKSeg - 1) / kKSeg, g.num_sms / 2, 2, 256)) {
+    if (nprod == kScaledLo || needs_ext(out) || wants_split_k(tiles, (K + kKSeg - 1) / kKSeg, g.num_sms / 2, 2, 256)) {
         switch (nprod) {
         case 1: return launch_gemm2_cfg<Gemm2Cfg<256, 1, B_MN, true>>(M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, out, s);
         case 2: return launch_gemm2_cfg<Gemm2Cfg<256, 2, B_MN, true>>(M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, out, s);
         case 3: return launch_gemm2_cfg<Gemm2Cfg<256, 3, B_MN, true>>(M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, out, s);
         case 4: return launch_gemm2_cfg<Gemm2Cfg<256, 4, B_MN, true>>(M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, out, s);
+        case kScaledLo: return launch_gemm2_cfg<Gemm2Cfg<256, kScaledLo, B_MN, true>>(M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, out, s);
         }
         return HEAL_ERR_UNSUPPORTED_MODE;
     }
@@ -655,12 +656,13 @@ int launch_gemm_np(int nprod, int64_t M, int64_t N, int64_t K, const void *A_hi,
                    const void *B_hi, const void *B_lo, int64_t ldb, const OutArgs &out, cudaStream_t s)
 {
     const int64_t tiles = ((M + kBM - 1) / kBM) * ((N + BN - 1) / BN);
-    if (needs_ext(out) || wants_split_k(tiles, (K + kKSeg - 1) / kKSeg, g.num_sms, 1, BN)) {
+    if (nprod == kScaledLo || needs_ext(out) || wants_split_k(tiles, (K + kKSeg - 1) / kKSeg, g.num_sms, 1, BN)) {
         switch (nprod) {
         case 1: return launch_gemm_cfg<GemmCfg<BN, 1, B_MN, true>>(M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, out, s);
         case 2: return launch_gemm_cfg<GemmCfg<BN, 2, B_MN, true>>(M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, out, s);
         case 3: return launch_gemm_cfg<GemmCfg<BN, 3, B_MN, true>>(M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, out, s);
         case 4: return launch_gemm_cfg<GemmCfg<BN, 4, B_MN, true>>(M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, out, s);
+        case kScaledLo: return launch_gemm_cfg<GemmCfg<BN, kScaledLo, B_MN, true>>(M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, out, s);
         }
         return HEAL_ERR_UNSUPPORTED_MODE;
     }
@@ -1032,25 +1034,19 @@ int get_ws(size_t bytes, cudaStream_t stream, void **out)
     return HEAL_OK;
 }
 
-// Scaled-lo variant (HEAL_LO_SCALED; the paper's h = h_hi + h_lo / 2^10 and Eq. 10 as printed):
-// C = 2^-p (hi.W) + 2^-(p+10) (lo'.W), formed the way the paper forms it -- two FP16 tensor-core GEMMs summed into one
-// FP32 output: the lo' GEMM stores its exactly scaled sum, the hi GEMM adds its own on top (FP32 RN).
-// Each GEMM has the usual fixed reduction order, so the result is as reproducible as the one-accumulator form.
-int scaled_two_gemms(int64_t M, int64_t N, int64_t K, const void *A_hi, const void *A_lo, int64_t lda, const void *B,
-                     int64_t ldb, const OutArgs &out, int scale_exp, bool b_nk, bool b_static, cudaStream_t stream)
+// Scaled-lo variant (HEAL_LO_SCALED; the paper's h = h_hi + h_lo / 2^10 and Eq. 10 as printed): one kernel, one
+// accumulator, two passes per K segment with tcgen05's scale_input_d (GemmCfg::SCALED in heal_gemm_umma.cuh).  All M take the large-M
+// kernels (the small-M kernel has no such form), so the bits do not depend on M.
+int scaled_impl(int64_t M, int64_t N, int64_t K, const void *A_hi, const void *A_lo, int64_t lda, const void *B, int64_t ldb,
+                const OutArgs &out, bool b_nk, cudaStream_t stream)
 {
-    if (!out.C) return HEAL_ERR_NULL_POINTER;                         // the FP32 matrix carries the first GEMM
-    if (scale_exp + HEAL_LO_SHIFT > 126) return HEAL_ERR_INVALID_VALUE;
-    OutArgs first = out;
-    first.hi = first.lo = nullptr;
-    const uint32_t bits = static_cast<uint32_t>(127 - scale_exp - HEAL_LO_SHIFT) << 23;
-    memcpy(&first.scale, &bits, 4);
-    // (with HEAL_EPI_ACCUMULATE the first GEMM already adds onto the residual held in C)
-    int st = presplit_impl(M, N, K, A_lo, nullptr, lda, B, nullptr, ldb, first, 1, b_nk, b_static, stream);
-    if (st) return st;
-    OutArgs second = out;
-    second.accumulate = 1;
-    return presplit_impl(M, N, K, A_hi, nullptr, lda, B, nullptr, ldb, second, 1, b_nk, b_static, stream);
+    static_assert(kLoShift == HEAL_LO_SHIFT, "the kernels' scale_input_d immediate is the header's HEAL_LO_SHIFT");
+    if (M > kBM && N > 128 && forced_kernel() != 3) {
+        if (b_nk) return launch_gemm2_np<false>(kScaledLo, M, N, K, A_hi, A_lo, lda, B, nullptr, ldb, out, stream);
+        return launch_gemm2_np<true>(kScaledLo, M, N, K, A_hi, A_lo, lda, B, nullptr, ldb, out, stream);
+    }
+    if (b_nk) return launch_gemm_bn<false>(kScaledLo, M, N, K, A_hi, A_lo, lda, B, nullptr, ldb, out, stream);
+    return launch_gemm_bn<true>(kScaledLo, M, N, K, A_hi, A_lo, lda, B, nullptr, ldb, out, stream);
 }
 
 }  // namespace
@@ -1172,7 +1168,6 @@ static int make_out(int64_t M, int64_t N, void *C, int64_t ldc, void *C_hi, void
     const bool silu = (mode & HEAL_EPI_SILU_MUL) != 0, acc = (mode & HEAL_EPI_ACCUMULATE) != 0;
     if (scale_exp < -126 || scale_exp > 126) return HEAL_ERR_INVALID_VALUE;
     if (silu && (N & 1)) return HEAL_ERR_INVALID_VALUE;                    // (gate, up) column pairs
-    if (silu && (mode & HEAL_LO_SCALED)) return HEAL_ERR_UNSUPPORTED_MODE; // the two-GEMM form sums raw GEMM outputs
     const int64_t n_out = silu ? N / 2 : N;
     if ((C || !C_hi) && ldc < n_out) return HEAL_ERR_INVALID_VALUE;
     if ((C_hi || C_lo) && ldc16 < n_out) return HEAL_ERR_INVALID_VALUE;
@@ -1222,8 +1217,7 @@ int heal_gemm_presplit_ex(int64_t M, int64_t N, int64_t K, const void *A_hi, con
     st = ensure_init();
     if (st) return st;
     if ((mode & HEAL_LO_SCALED) && K > 0)          // A_lo holds r16((x - hi) * 2^10), e.g. from heal_split_scaled(.., 10, ..)
-        return scaled_two_gemms(M, N, K, A_hi, A_lo, lda, B_hi, ldb, out, scale_exp, b_nk, (mode & HEAL_B_STATIC) != 0,
-                                static_cast<cudaStream_t>(stream));
+        return scaled_impl(M, N, K, A_hi, A_lo, lda, B_hi, ldb, out, b_nk, static_cast<cudaStream_t>(stream));
     return presplit_impl(M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, out, nprod, b_nk, (mode & HEAL_B_STATIC) != 0,
                          static_cast<cudaStream_t>(stream));
 }
@@ -1318,7 +1312,7 @@ int heal_gemm_ex(int64_t M, int64_t N, int64_t K, const void *A, int64_t lda, co
     // step S on the activations; in 1P only the hi plane is consumed
     st = launch_split(M, K, static_cast<const float *>(A), lda, a_hi, a_lo, p.lda_p, stream, lo_scaled ? HEAL_LO_SHIFT : 0);
     if (st) return st;
-    if (lo_scaled) return scaled_two_gemms(M, N, K, a_hi, a_lo, p.lda_p, B, ldb, out, scale_exp, b_nk, b_static, stream);
+    if (lo_scaled) return scaled_impl(M, N, K, a_hi, a_lo, p.lda_p, B, ldb, out, b_nk, stream);
     const void *b_hi = B, *b_lo = nullptr;
     int64_t ldb_eff = ldb;
     if (b_f32) {

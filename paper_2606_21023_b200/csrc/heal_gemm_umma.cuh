@@ -30,13 +30,21 @@ struct GemmCfg {
                                                         // ordered split-K schedule; the default instantiation has neither, so the
                                                         // headline path carries no extra registers or code (measured: 2.5 % otherwise)
     static constexpr int BN = BN_;
-    static constexpr int NPROD = NPROD_;
+    // NPROD_ == kScaledLo: the paper's scaled residual (HEAL_LO_SCALED, Eq. 10 as printed) in ONE kernel and ONE
+    // accumulator.  Every K segment is walked twice: first all lo'.W products (lo' = r16((x - hi) 2^10)), then the hi.W products, the
+    // first of which is issued with scale_input_d = 10, i.e. D = hi_0.W_0 + D * 2^-10 inside the tensor core (an exact power-of-two
+    // scaling of the residual sum).  Segment sums are then added in FP32 RN as always.  The weight tile travels twice (64 instead of
+    // 48 KB per k-tile and product pair), which is why this is a variant and not the default; it still replaces two launches, a
+    // read-modify-write of C and a second epilogue.
+    static constexpr bool SCALED = NPROD_ == kScaledLo;
+    static constexpr int NPROD = SCALED ? 2 : NPROD_;
     static constexpr bool B_MN = B_MN_;                 // B stored K x N (N contiguous): MN-major operand
     static constexpr int A_PLANES = NPROD >= 2 ? 2 : 1;
     static constexpr int B_PLANES = NPROD >= 3 ? 2 : 1;
     static constexpr int A_TILE = kBM * kBK * 2;
     static constexpr int B_TILE = BN * kBK * 2;
-    static constexpr int STAGE_BYTES = A_PLANES * A_TILE + B_PLANES * B_TILE;
+    static constexpr int A_SLOTS = SCALED ? 1 : A_PLANES;   // SCALED: one activation plane per pass shares the slot
+    static constexpr int STAGE_BYTES = A_SLOTS * A_TILE + B_PLANES * B_TILE;
     static constexpr int BAR_BYTES = 256;
     static constexpr int STAGES_RAW = (kSmemLimit - 1024 - BAR_BYTES) / STAGE_BYTES;
     static constexpr int STAGES = STAGES_RAW > 8 ? 8 : STAGES_RAW;
@@ -292,15 +300,28 @@ heal_gemm_umma_kernel(const __grid_constant__ CUtensorMap tm_a_hi, const __grid_
                 const int m0 = tm * kBM;
                 const int n0 = tn * BN;
                 const int kt_hi = min(k_tiles, se_seg * kTilesPerSeg);
-                for (int kt = sb_seg * kTilesPerSeg; kt < kt_hi; ++kt) {
+                const int n_steps = Cfg::SCALED ? 2 * (kt_hi - sb_seg * kTilesPerSeg) : kt_hi - sb_seg * kTilesPerSeg;
+                for (int step = 0; step < n_steps; ++step) {
+                    int kt = sb_seg * kTilesPerSeg + step;
+                    bool lo_pass = false;
+                    if (Cfg::SCALED) {                       // segment by segment: the residual pass, then the hi pass
+                        const int seg = sb_seg + step / (2 * kTilesPerSeg), r = step % (2 * kTilesPerSeg);
+                        const int len = min(k_tiles, (seg + 1) * kTilesPerSeg) - seg * kTilesPerSeg;
+                        lo_pass = r < len;
+                        kt = seg * kTilesPerSeg + (lo_pass ? r : r - len);
+                    }
                     mbar_wait_ool(empty_bar(stage), phase ^ 1u, args.diag, 100 + stage);
                     const uint32_t sb = smem_base + stage * Cfg::STAGE_BYTES;
                     const uint32_t fb = full_bar(stage);
                     mbar_arrive_expect_tx(fb, Cfg::STAGE_BYTES);
                     const int k0 = kt * kBK;
-                    tma_load_2d(sb, &tm_a_hi, fb, k0, m0);
-                    if (Cfg::A_PLANES == 2) tma_load_2d(sb + Cfg::A_TILE, &tm_a_lo, fb, k0, m0);
-                    const uint32_t sbB = sb + Cfg::A_PLANES * Cfg::A_TILE;
+                    if (Cfg::SCALED) {
+                        tma_load_2d(sb, lo_pass ? &tm_a_lo : &tm_a_hi, fb, k0, m0);
+                    } else {
+                        tma_load_2d(sb, &tm_a_hi, fb, k0, m0);
+                        if (Cfg::A_PLANES == 2) tma_load_2d(sb + Cfg::A_TILE, &tm_a_lo, fb, k0, m0);
+                    }
+                    const uint32_t sbB = sb + Cfg::A_SLOTS * Cfg::A_TILE;
                     if (Cfg::B_MN) {
 #pragma unroll
                         for (int c = 0; c < BN / 64; ++c) {
@@ -340,6 +361,27 @@ heal_gemm_umma_kernel(const __grid_constant__ CUtensorMap tm_a_hi, const __grid_
                     const uint32_t d_tmem = tmem_base + static_cast<uint32_t>(buf * BN);
                     const int kt_end = min(k_tiles, (seg + 1) * kTilesPerSeg);
                     uint32_t accumulate = 0;
+                    if constexpr (Cfg::SCALED) {
+                        for (int pass = 0; pass < 2; ++pass)
+                            for (int kt = seg * kTilesPerSeg; kt < kt_end; ++kt) {
+                                mbar_wait_ool(full_bar(stage), phase, args.diag, 200 + stage);
+                                tc_fence_after();
+                                const uint32_t sb = smem_base + stage * Cfg::STAGE_BYTES;
+                                const uint64_t a_d = adesc0 | desc_addr(sb);
+                                const uint64_t b_d = bdesc0 | desc_addr(sb + Cfg::A_TILE);
+#pragma unroll
+                                for (int j = 0; j < kBK / 16; ++j) {
+                                    const uint64_t ao = static_cast<uint64_t>(j * a_step), bo = static_cast<uint64_t>(j * b_step);
+                                    if (pass == 1 && kt == seg * kTilesPerSeg && j == 0)
+                                        umma_f16_scale_d<kLoShift>(d_tmem, a_d + ao, b_d + bo, idesc);
+                                    else
+                                        umma_f16(d_tmem, a_d + ao, b_d + bo, idesc, accumulate);
+                                    accumulate = 1;
+                                }
+                                umma_commit(empty_bar(stage));
+                                if (++stage == STAGES) { stage = 0; phase ^= 1u; }
+                            }
+                    } else
                     for (int kt = seg * kTilesPerSeg; kt < kt_end; ++kt) {
                         mbar_wait_ool(full_bar(stage), phase, args.diag, 200 + stage);
                         tc_fence_after();

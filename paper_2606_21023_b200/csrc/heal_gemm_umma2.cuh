@@ -32,14 +32,16 @@ struct Gemm2Cfg {
                                                         // ordered split-K schedule; the default instantiation has neither, so the
                                                         // headline path carries no extra registers or code (measured: 2.5 % otherwise)
     static constexpr int BN = BN_;                       // pair-tile width; each CTA stages BN/2 columns of B
-    static constexpr int NPROD = NPROD_;
+    static constexpr bool SCALED = NPROD_ == kScaledLo;  // HEAL_LO_SCALED in one kernel (see heal_gemm_umma.cuh): two passes per K segment
+    static constexpr int NPROD = SCALED ? 2 : NPROD_;
     static constexpr bool B_MN = B_MN_;
     static constexpr int A_PLANES = NPROD >= 2 ? 2 : 1;
     static constexpr int B_PLANES = NPROD >= 3 ? 2 : 1;
     static constexpr int A_TILE = kBM * kBK * 2;
     static constexpr int BH = BN / 2;
     static constexpr int B_TILE = BH * kBK * 2;
-    static constexpr int STAGE_BYTES = A_PLANES * A_TILE + B_PLANES * B_TILE;
+    static constexpr int A_SLOTS = SCALED ? 1 : A_PLANES;   // SCALED: one activation plane per pass shares the slot
+    static constexpr int STAGE_BYTES = A_SLOTS * A_TILE + B_PLANES * B_TILE;
     static constexpr int BAR_BYTES = 256;
     static constexpr int STAGES_RAW = (kSmemLimit - 1024 - BAR_BYTES) / STAGE_BYTES;
     static constexpr int STAGES = STAGES_RAW > 8 ? 8 : STAGES_RAW;
@@ -120,15 +122,29 @@ heal_gemm_umma2_kernel(const __grid_constant__ CUtensorMap tm_a_hi, const __grid
                 const int m0 = tm * (2 * kBM) + rank * kBM;
                 const int n0 = tn * BN + rank * Cfg::BH;
                 const int kt_hi = min(k_tiles, se_seg * kTilesPerSeg);
-                for (int kt = sb_seg * kTilesPerSeg; kt < kt_hi; ++kt) {
+                // SCALED: every K segment is walked twice -- first the scaled residual plane, then the hi plane (each with the weight tile)
+                const int n_steps = Cfg::SCALED ? 2 * (kt_hi - sb_seg * kTilesPerSeg) : kt_hi - sb_seg * kTilesPerSeg;
+                for (int step = 0; step < n_steps; ++step) {
+                    int kt = sb_seg * kTilesPerSeg + step;
+                    bool lo_pass = false;
+                    if (Cfg::SCALED) {
+                        const int seg = sb_seg + step / (2 * kTilesPerSeg), r = step % (2 * kTilesPerSeg);
+                        const int len = min(k_tiles, (seg + 1) * kTilesPerSeg) - seg * kTilesPerSeg;     // (only the last segment of K is short,
+                        lo_pass = r < len;                                                                //  and it is the last one of the chunk)
+                        kt = seg * kTilesPerSeg + (lo_pass ? r : r - len);
+                    }
                     mbar_wait_ool(empty_bar(stage), phase ^ 1u, args.diag, 100 + stage);
                     const uint32_t sb = smem_base + stage * Cfg::STAGE_BYTES;
                     const uint32_t fb = leader_addr(full_bar(stage));
                     mbar_arrive_expect_tx_cluster(fb, Cfg::STAGE_BYTES);
                     const int k0 = kt * kBK;
-                    tma_load_2d_2cta(sb, &tm_a_hi, fb, k0, m0);
-                    if (Cfg::A_PLANES == 2) tma_load_2d_2cta(sb + Cfg::A_TILE, &tm_a_lo, fb, k0, m0);
-                    const uint32_t sbB = sb + Cfg::A_PLANES * Cfg::A_TILE;
+                    if (Cfg::SCALED) {
+                        tma_load_2d_2cta(sb, lo_pass ? &tm_a_lo : &tm_a_hi, fb, k0, m0);
+                    } else {
+                        tma_load_2d_2cta(sb, &tm_a_hi, fb, k0, m0);
+                        if (Cfg::A_PLANES == 2) tma_load_2d_2cta(sb + Cfg::A_TILE, &tm_a_lo, fb, k0, m0);
+                    }
+                    const uint32_t sbB = sb + Cfg::A_SLOTS * Cfg::A_TILE;
                     if (Cfg::B_MN) {
 #pragma unroll
                         for (int c = 0; c < Cfg::BH / 64; ++c) {
@@ -169,6 +185,30 @@ heal_gemm_umma2_kernel(const __grid_constant__ CUtensorMap tm_a_hi, const __grid
                     const uint32_t d_tmem = tmem_base + static_cast<uint32_t>(buf * BN);
                     const int kt_end = min(k_tiles, (seg + 1) * kTilesPerSeg);
                     uint32_t accumulate = 0;
+                    if constexpr (Cfg::SCALED) {
+                        // D = sum_k lo'_k . W_k (k ascending), then D = hi_0 . W_0 + D * 2^-10, then D += hi_k . W_k: Eq. 10 as printed
+                        // in one accumulator -- the tensor core scales the residual sum by an exact power of two
+                        // before the first hi product is added (scale_input_d)
+                        for (int pass = 0; pass < 2; ++pass)
+                            for (int kt = seg * kTilesPerSeg; kt < kt_end; ++kt) {
+                                mbar_wait_ool(full_bar(stage), phase, args.diag, 200 + stage);
+                                tc_fence_after();
+                                const uint32_t sb = smem_base + stage * Cfg::STAGE_BYTES;
+                                const uint64_t a_d = adesc0 | desc_addr(sb);
+                                const uint64_t b_d = bdesc0 | desc_addr(sb + Cfg::A_TILE);
+#pragma unroll
+                                for (int j = 0; j < kBK / 16; ++j) {
+                                    const uint64_t ao = static_cast<uint64_t>(j * a_step), bo = static_cast<uint64_t>(j * b_step);
+                                    if (pass == 1 && kt == seg * kTilesPerSeg && j == 0)
+                                        umma_f16_2cta_scale_d<kLoShift>(d_tmem, a_d + ao, b_d + bo, idesc);
+                                    else
+                                        umma_f16_2cta(d_tmem, a_d + ao, b_d + bo, idesc, accumulate);
+                                    accumulate = 1;
+                                }
+                                umma_commit_2cta(empty_bar(stage), 3);
+                                if (++stage == STAGES) { stage = 0; phase ^= 1u; }
+                            }
+                    } else
                     for (int kt = seg * kTilesPerSeg; kt < kt_end; ++kt) {
                         const long long t1 = HEAL_TCLK();
                         mbar_wait_ool(full_bar(stage), phase, args.diag, 200 + stage);

@@ -12,6 +12,8 @@ constexpr int kBK = 64;                     // k-tile: 64 FP16 = 128 bytes = one
 constexpr int kKSeg = 512;                  // HEAL_K_SEGMENT (include/heal.h): the reduction-order contract
 constexpr int kTilesPerSeg = kKSeg / kBK;
 constexpr int kSmemLimit = 227 * 1024;      // dynamic shared memory per CTA on sm_100
+constexpr int kLoShift = 10;                // HEAL_LO_SHIFT: the paper's residual scale 2^10
+constexpr int kScaledLo = 5;                // template value of NPROD that selects the one-kernel scaled-residual form (two products)
 
 __device__ __forceinline__ uint32_t smem_u32(const void *p)
 {
@@ -183,6 +185,28 @@ __device__ __forceinline__ void umma_f16(uint32_t d_tmem, uint64_t a_desc, uint6
         "setp.ne.b32 p, %4, 0;\n\t"
         "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}"
         ::"r"(d_tmem), "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(accumulate)
+        : "memory");
+}
+// D[tmem] = A . B + D * 2^-SHIFT (the optional scale_input_d immediate of kind::f16, PTX ISA 8.6): the accumulator is scaled down by an
+// exact power of two before the products of this instruction are added.  Used by the scaled-residual variant (HEAL_LO_SCALED).
+template <int SHIFT>
+__device__ __forceinline__ void umma_f16_scale_d(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc)
+{
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "setp.ne.b32 p, 1, 0;\n\t"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p, %4;\n\t}"
+        ::"r"(d_tmem), "l"(a_desc), "l"(b_desc), "r"(idesc), "n"(SHIFT)
+        : "memory");
+}
+template <int SHIFT>
+__device__ __forceinline__ void umma_f16_2cta_scale_d(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc)
+{
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "setp.ne.b32 p, 1, 0;\n\t"
+        "tcgen05.mma.cta_group::2.kind::f16 [%0], %1, %2, %3, p, %4;\n\t}"
+        ::"r"(d_tmem), "l"(a_desc), "l"(b_desc), "r"(idesc), "n"(SHIFT)
         : "memory");
 }
 // Arrive on an mbarrier once all previously issued tcgen05.mma of this thread have completed

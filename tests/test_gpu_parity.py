@@ -691,7 +691,7 @@ def test_fused_epilogue_errors(hb):
     st = lambda mode, N=66, ldc=72, Cp=C.data_ptr(): L.heal_gemm(8, N, 64, A.data_ptr(), 64, W.data_ptr(), 72 if N > 66 else 66 + 6, Cp, ldc, mode, None)
     assert L.heal_gemm(8, 65, 64, A.data_ptr(), 64, W.data_ptr(), 72, C.data_ptr(), 72, 2 | hb.EPI_SILU_MUL, None) == 1      # odd N
     assert L.heal_gemm(8, 64, 64, A.data_ptr(), 64, W.data_ptr(), 72, C.data_ptr(), 28, 2 | hb.EPI_SILU_MUL, None) == 1      # ldc < N/2
-    assert L.heal_gemm(8, 64, 64, A.data_ptr(), 64, W.data_ptr(), 72, C.data_ptr(), 32, 2 | hb.EPI_SILU_MUL | hb.LO_SCALED, None) == 4
+    assert L.heal_gemm(8, 64, 64, A.data_ptr(), 64, W.data_ptr(), 72, C.data_ptr(), 32, 2 | hb.EPI_SILU_MUL | hb.LO_SCALED, None) == 0
     assert L.heal_gemm_ex(8, 64, 64, A.data_ptr(), 64, W.data_ptr(), 72, None, 0, C.data_ptr(), C.data_ptr(), 72, 0,
                           2 | hb.EPI_ACCUMULATE, None) == 2                                                               # accumulate needs C
     assert L.heal_gemm_host(8, 64, 64, A.data_ptr(), 64, W.data_ptr(), 72, C.data_ptr(), 72, 2 | hb.EPI_ACCUMULATE, None) == 4
@@ -755,11 +755,12 @@ def test_scaled_split_bit_exact(hb, oracle, inputs):
         assert np.array_equal(lo.cpu().numpy().view(np.uint16), olo)
 
 
-@pytest.mark.parametrize("M,N,K", [(8, 520, 4096), (300, 1032, 4096), (64, 264, 14336)])
+@pytest.mark.parametrize("M,N,K", [(8, 520, 4096), (300, 1032, 4096), (64, 264, 14336), (1300, 4104, 2056), (256, 1032, 4096 + 72)])
 def test_lo_scaled_variant(hb, oracle, inputs, M, N, K):
-    """HEAL_LO_SCALED (Eq. 10 as printed, s = 10; two GEMMs summed into one FP32 output): against the oracle's exact
-    evaluation of the same products, inside the gate, bit-identical across M and kernel families -- and, on
-    activations small enough for the unscaled residual to underflow FP16, far closer to FP64 than the s = 0 default."""
+    """HEAL_LO_SCALED (Eq. 10 as printed, s = 10; one kernel, one accumulator: per K segment the lo'.W products first, then the
+    hi.W products with the accumulator scaled by 2^-10 inside the tensor core): against the oracle's exact evaluation of the
+    same products, inside the gate, bit-identical across M and kernel families -- and, on activations small enough for the
+    unscaled residual to underflow FP16, far closer to FP64 than the s = 0 default."""
     A = inputs.activations(M, K, seed=22, outliers=True)
     W = inputs.weights_f16(K, N, seed=22)
     Ad, Wd = dev(A), dev(W)
@@ -770,16 +771,23 @@ def test_lo_scaled_variant(hb, oracle, inputs, M, N, K):
     assert oracle.normwise_error(got.cpu().numpy(), oracle.gemm_f64(A, W), A, W) <= GATE
     assert torch.equal(hb.heal_gemm(Ad[:5], Wd, mode), got[:5])                  # M-invariant
     try:
-        hb.debug_force_kernel(1)
-        assert torch.equal(hb.heal_gemm(Ad, Wd, mode), got)
+        for which in (1, 3):                                                     # large-M kernels only | single-CTA kernel
+            hb.debug_force_kernel(which)
+            assert torch.equal(hb.heal_gemm(Ad, Wd, mode), got)
     finally:
         hb.debug_force_kernel(0)
     ah, al = hb.heal_split(Ad, lo_shift=hb.LO_SHIFT)
     assert torch.equal(hb.heal_gemm_presplit(ah, al, Wd, None, mode), got)
+    n0 = hb.launch_count()
     C, hi, lo = hb.heal_gemm_ex(Ad, Wd, mode, scale_exp=2)                        # composes with the extended epilogue
     assert torch.equal(C, got * 0.25)
     whi, wlo = hb.heal_split(C)
     assert torch.equal(hi.view(torch.int16), whi.view(torch.int16)) and torch.equal(lo.view(torch.int16), wlo.view(torch.int16))
+    _, h2, l2 = hb.heal_gemm_presplit_ex(ah, al, Wd, None, mode, want_c=False, scale_exp=2)      # planes only: no FP32 matrix needed
+    assert torch.equal(h2, hi) and torch.equal(l2, lo)
+    R = torch.ones_like(got)
+    hb.heal_gemm_presplit_ex(ah, al, Wd, None, mode | hb.EPI_ACCUMULATE, C=R, want_planes=False)
+    assert torch.equal(R, got + 1.0)
     # tiny activations: |x| ~ 2^-12, the s = 0 residual is an FP16 subnormal with almost no bits left
     At = (A * np.float32(2.0 ** -12)).astype(np.float32)
     ref = oracle.gemm_f64(At, W)
@@ -798,8 +806,9 @@ def test_lo_scaled_errors(hb):
     raw = hb.heal_gemm_raw
     assert raw(8, 16, 64, A.data_ptr(), 64, W32.data_ptr(), 16, C.data_ptr(), 16, 3 | hb.LO_SCALED) == 4      # 2P only
     assert raw(8, 16, 64, A.data_ptr(), 64, W.data_ptr(), 16, C.data_ptr(), 16, 1 | hb.LO_SCALED) == 4
-    assert L.heal_gemm_ex(8, 16, 64, A.data_ptr(), 64, W.data_ptr(), 16, None, 0, hi.data_ptr(), hi.data_ptr(), 16, 0,
-                          2 | hb.LO_SCALED, None) == 2                                                           # needs C
+    lo = torch.zeros_like(hi)
+    assert L.heal_gemm_ex(8, 16, 64, A.data_ptr(), 64, W.data_ptr(), 16, None, 0, hi.data_ptr(), lo.data_ptr(), 16, 0,
+                          2 | hb.LO_SCALED, None) == 0                                                           # planes only is fine
     assert L.heal_split_scaled(8, 64, A.data_ptr(), 64, hi.data_ptr(), hi.data_ptr(), 64, 17, None) == 1
     torch.cuda.synchronize()
 
