@@ -20,7 +20,7 @@ struct OutArgs {
     int64_t ld16;
     float scale;          // 2^-p, exactly representable; 1.0f = none
     int accumulate;       // C += scaled result (needs C): the residual add "A_i + GEMM(...)" of Algorithm 1 with
-                          // C holding A_i (HEAL_EPI_ACCUMULATE), and the second launch of the two-GEMM scaled-lo form
+                          // C holding A_i (HEAL_EPI_ACCUMULATE)
     int silu;             // HEAL_EPI_SILU_MUL: the GEMM's columns are (gate, up) pairs -- column 2j = g_j, 2j+1 = u_j -- and the
                           // outputs (C and/or planes, N/2 columns wide) receive SiLU(g_j) * u_j
 };

@@ -34,8 +34,8 @@ struct GemmCfg {
     // accumulator.  Every K segment is walked twice: first all lo'.W products (lo' = r16((x - hi) 2^10)), then the hi.W products, the
     // first of which is issued with scale_input_d = 10, i.e. D = hi_0.W_0 + D * 2^-10 inside the tensor core (an exact power-of-two
     // scaling of the residual sum).  Segment sums are then added in FP32 RN as always.  The weight tile travels twice (64 instead of
-    // 48 KB per k-tile and product pair), which is why this is a variant and not the default; it still replaces two launches, a
-    // read-modify-write of C and a second epilogue.
+    // 48 KB per k-tile and product pair), which is why this is a variant and not the default (measured 1.08x on the MLP
+    // GEMMs; round 1 formed it from two one-product launches at 1.55x).
     static constexpr bool SCALED = NPROD_ == kScaledLo;
     static constexpr int NPROD = SCALED ? 2 : NPROD_;
     static constexpr bool B_MN = B_MN_;                 // B stored K x N (N contiguous): MN-major operand
