@@ -91,8 +91,8 @@ typedef enum {
                                   as it adds the first h_hi.W product, then accumulates the remaining h_hi.W products; segment sums are
                                   added in FP32 RN in ascending order as always.  Differs from the default (s = 0) only where h_lo would
                                   leave FP16's normal range, i.e. for |h| < 2^-3 (reading A1).  The weight tile travels twice per
-                                  segment: about 8 % slower than the default on prefill shapes; every M runs the large-M kernels (same
-                                  bits for every M), so decode-sized M is about 2x slower than the default.  With
+                                  segment: about 8 % slower than the default on prefill shapes, 1.3-1.5x on decode shapes (M <= 32: the
+                                  small-M kernel's form of the same two passes, second weight read out of L2; same bits for every M).  With
                                   heal_gemm_presplit(_ex) A_lo must hold the scaled residual (heal_split_scaled with lo_shift = 10). */
 
 /*

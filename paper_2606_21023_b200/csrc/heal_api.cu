@@ -869,7 +869,9 @@ int launch_small_cfg(int64_t M, int64_t N, int64_t K, const SmallIn &in, const v
     HEAL_CUDA(cudaLaunchKernelEx(&cfg, kern, tx_hi, tx_lo, tw_hi, tw_lo, args));
     g_launches.fetch_add(1);
     static const std::string name = kernel_name("heal_gemm_smallm_kernel", Cfg::MPAD, Cfg::NPROD, Cfg::B_MN,
-                                                Cfg::FUSED ? ",fused split" : (Cfg::PAIR ? ",cta_group::2" : ""));
+                                                Cfg::FUSED ? ",fused split"
+                                                           : (Cfg::SCALED ? (Cfg::PAIR ? ",cta_group::2,scaled lo" : ",scaled lo")
+                                                                          : (Cfg::PAIR ? ",cta_group::2" : "")));
     t_last_kernel = name.c_str();
     *handled = true;
     return HEAL_OK;
@@ -898,6 +900,7 @@ int launch_small_np(int nprod, int64_t M, int64_t N, int64_t K, const SmallIn &i
             case 2: return launch_small_cfg<SmallCfg<MPAD, 2, B_MN, false, true>>(M, N, K, in, B_hi, B_lo, ldb, out, s, handled);
             case 3: return launch_small_cfg<SmallCfg<MPAD, 3, B_MN, false, true>>(M, N, K, in, B_hi, B_lo, ldb, out, s, handled);
             case 4: return launch_small_cfg<SmallCfg<MPAD, 4, B_MN, false, true>>(M, N, K, in, B_hi, B_lo, ldb, out, s, handled);
+            case kScaledLo: return launch_small_cfg<SmallCfg<MPAD, kScaledLo, B_MN, false, true>>(M, N, K, in, B_hi, B_lo, ldb, out, s, handled);
             }
         }
     }
@@ -906,6 +909,7 @@ int launch_small_np(int nprod, int64_t M, int64_t N, int64_t K, const SmallIn &i
     case 2: return launch_small_cfg<SmallCfg<MPAD, 2, B_MN, false>>(M, N, K, in, B_hi, B_lo, ldb, out, s, handled);
     case 3: return launch_small_cfg<SmallCfg<MPAD, 3, B_MN, false>>(M, N, K, in, B_hi, B_lo, ldb, out, s, handled);
     case 4: return launch_small_cfg<SmallCfg<MPAD, 4, B_MN, false>>(M, N, K, in, B_hi, B_lo, ldb, out, s, handled);
+    case kScaledLo: return launch_small_cfg<SmallCfg<MPAD, kScaledLo, B_MN, false>>(M, N, K, in, B_hi, B_lo, ldb, out, s, handled);
     }
     return HEAL_ERR_UNSUPPORTED_MODE;
 }
@@ -967,7 +971,10 @@ int presplit_impl(int64_t M, int64_t N, int64_t K, const void *A_hi, const void 
         return HEAL_OK;
     }
     const int force = forced_kernel();
-    if ((M <= 64 && force != 1) || (force == 2 && M <= 64)) {
+    // Scaled residual: the small-M kernel reads every weight tile twice (the second time out of L2), which pays up to 32 tokens
+    // (measured: 8 x 4096 x 4096 15.3 vs 24.2 us, LM head M = 1 225 vs 300 us; but M = 64 22.0 vs 21.3 and 310 vs 271 us)
+    const int64_t small_max = nprod == kScaledLo && force != 2 ? 32 : 64;
+    if (M <= small_max && force != 1) {
         bool handled = false;
         const SmallIn in{A_hi, A_lo, lda, A32, lda32, b_static};
         int st = b_nk ? launch_small<false>(nprod, M, N, K, in, B_hi, B_lo, ldb, out, stream, &handled)
@@ -1035,18 +1042,13 @@ int get_ws(size_t bytes, cudaStream_t stream, void **out)
 }
 
 // Scaled-lo variant (HEAL_LO_SCALED; the paper's h = h_hi + h_lo / 2^10 and Eq. 10 as printed): one kernel, one
-// accumulator, two passes per K segment with tcgen05's scale_input_d (GemmCfg::SCALED in heal_gemm_umma.cuh).  All M take the large-M
-// kernels (the small-M kernel has no such form), so the bits do not depend on M.
+// accumulator, two passes per K segment with tcgen05's scale_input_d (GemmCfg::SCALED in heal_gemm_umma.cuh, SmallCfg::SCALED in
+// heal_gemm_smallm.cuh).  Same kernel choice by shape as every other mode, same bits whichever kernel runs.
 int scaled_impl(int64_t M, int64_t N, int64_t K, const void *A_hi, const void *A_lo, int64_t lda, const void *B, int64_t ldb,
-                const OutArgs &out, bool b_nk, cudaStream_t stream)
+                const OutArgs &out, bool b_nk, bool b_static, cudaStream_t stream)
 {
     static_assert(kLoShift == HEAL_LO_SHIFT, "the kernels' scale_input_d immediate is the header's HEAL_LO_SHIFT");
-    if (M > kBM && N > 128 && forced_kernel() != 3) {
-        if (b_nk) return launch_gemm2_np<false>(kScaledLo, M, N, K, A_hi, A_lo, lda, B, nullptr, ldb, out, stream);
-        return launch_gemm2_np<true>(kScaledLo, M, N, K, A_hi, A_lo, lda, B, nullptr, ldb, out, stream);
-    }
-    if (b_nk) return launch_gemm_bn<false>(kScaledLo, M, N, K, A_hi, A_lo, lda, B, nullptr, ldb, out, stream);
-    return launch_gemm_bn<true>(kScaledLo, M, N, K, A_hi, A_lo, lda, B, nullptr, ldb, out, stream);
+    return presplit_impl(M, N, K, A_hi, A_lo, lda, B, nullptr, ldb, out, kScaledLo, b_nk, b_static, stream);
 }
 
 }  // namespace
@@ -1217,7 +1219,7 @@ int heal_gemm_presplit_ex(int64_t M, int64_t N, int64_t K, const void *A_hi, con
     st = ensure_init();
     if (st) return st;
     if ((mode & HEAL_LO_SCALED) && K > 0)          // A_lo holds r16((x - hi) * 2^10), e.g. from heal_split_scaled(.., 10, ..)
-        return scaled_impl(M, N, K, A_hi, A_lo, lda, B_hi, ldb, out, b_nk, static_cast<cudaStream_t>(stream));
+        return scaled_impl(M, N, K, A_hi, A_lo, lda, B_hi, ldb, out, b_nk, (mode & HEAL_B_STATIC) != 0, static_cast<cudaStream_t>(stream));
     return presplit_impl(M, N, K, A_hi, A_lo, lda, B_hi, B_lo, ldb, out, nprod, b_nk, (mode & HEAL_B_STATIC) != 0,
                          static_cast<cudaStream_t>(stream));
 }
@@ -1312,7 +1314,7 @@ int heal_gemm_ex(int64_t M, int64_t N, int64_t K, const void *A, int64_t lda, co
     // step S on the activations; in 1P only the hi plane is consumed
     st = launch_split(M, K, static_cast<const float *>(A), lda, a_hi, a_lo, p.lda_p, stream, lo_scaled ? HEAL_LO_SHIFT : 0);
     if (st) return st;
-    if (lo_scaled) return scaled_impl(M, N, K, a_hi, a_lo, p.lda_p, B, ldb, out, b_nk, stream);
+    if (lo_scaled) return scaled_impl(M, N, K, a_hi, a_lo, p.lda_p, B, ldb, out, b_nk, (mode & HEAL_B_STATIC) != 0, stream);
     const void *b_hi = B, *b_lo = nullptr;
     int64_t ldb_eff = ldb;
     if (b_f32) {

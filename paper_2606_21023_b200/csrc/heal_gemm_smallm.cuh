@@ -43,7 +43,11 @@ constexpr int kSmallMaxStages = 8;
 template <int MPAD_, int NPROD_, bool B_MN_, bool FUSED_, bool PAIR_ = false>
 struct SmallCfg {
     static constexpr int MPAD = MPAD_;                  // UMMA N: padded token count
-    static constexpr int NPROD = NPROD_;
+    // NPROD_ == kScaledLo (HEAL_LO_SCALED, Eq. 10 as printed): as in heal_gemm_umma.cuh every local K segment is walked twice,
+    // first the lo'.W products, then the hi.W products whose first MMA scales the accumulator by 2^-10 (scale_input_d); one
+    // activation plane per step shares the stage's X slot, the weight tile of the second pass comes out of L2
+    static constexpr bool SCALED = NPROD_ == kScaledLo;
+    static constexpr int NPROD = SCALED ? 2 : NPROD_;
     static constexpr bool B_MN = B_MN_;                 // weights stored K x N (N contiguous)
     static constexpr bool FUSED = FUSED_;               // split the FP32 activations in the kernel
     static constexpr bool PAIR = PAIR_;                 // large N, no K split, many tokens: two adjacent panels share one
@@ -56,16 +60,47 @@ struct SmallCfg {
     static constexpr int W_TILE = kSmallBNW * kBK * 2;  // 16 KB
     static constexpr int X_TILE = XROWS * kBK * 2;
     static constexpr int X_TILE_AL = (X_TILE + 1023) / 1024 * 1024;
-    static constexpr int STAGE_BYTES = B_PLANES * W_TILE + A_PLANES * X_TILE_AL;
+    static constexpr int X_SLOTS = SCALED ? 1 : A_PLANES;
+    static constexpr int STAGE_BYTES = B_PLANES * W_TILE + X_SLOTS * X_TILE_AL;
     static constexpr int W_BYTES = B_PLANES * W_TILE;
-    static constexpr int TX_BYTES = W_BYTES + (FUSED ? 0 : A_PLANES * X_TILE);
+    static constexpr int TX_BYTES = W_BYTES + (FUSED ? 0 : X_SLOTS * X_TILE);
     static constexpr int BAR_BYTES = 512;
     static constexpr int TASKS = MPAD / 16;             // FUSED: 8-float chunks per converter thread per k-tile
     static constexpr int PF = MPAD <= 32 ? 4 : 2;       // FUSED: k-tiles of activations kept in flight in registers
     static_assert(MPAD % 16 == 0 && MPAD >= 16 && MPAD <= 64, "MPAD");
     static_assert(!FUSED || NPROD <= 2, "the fused split needs FP16 weights");
+    static_assert(!FUSED || !SCALED, "scaled residual: planes only");
     static_assert(!PAIR || (!FUSED && MPAD >= 32), "pairs: planes only, UMMA N >= 32 across the pair");
 };
+
+// One pipeline step of a rank: which local segment (TMEM slot) and k-tile of it, and whether the step opens / closes the
+// segment.  Plain: step t -> segment t / 8, k-tile t % 8.  SCALED: a segment of len k-tiles takes 2 len steps, the residual
+// pass first.  Only a rank's last local segment can be short (len < 8).
+struct SmallStep {
+    int seg_j, kk;
+    bool lo_pass, first, last;
+};
+template <bool SCALED>
+__device__ __forceinline__ SmallStep small_step(int s, int n_t, int n_local)
+{
+    SmallStep r;
+    if (SCALED) {
+        r.seg_j = s / (2 * kTilesPerSeg);
+        const int q = s % (2 * kTilesPerSeg);
+        const int len = r.seg_j == n_local - 1 ? n_t - (n_local - 1) * kTilesPerSeg : kTilesPerSeg;
+        r.lo_pass = q < len;
+        r.kk = r.lo_pass ? q : q - len;
+        r.first = q == 0;
+        r.last = q == 2 * len - 1;
+    } else {
+        r.seg_j = s >> 3;
+        r.kk = s & 7;
+        r.lo_pass = false;
+        r.first = r.kk == 0;
+        r.last = r.kk == 7 || s == n_t - 1;
+    }
+    return r;
+}
 
 struct SmallArgs {
     OutArgs out;          // step E: FP32 C and/or hi/lo planes, optional 2^-p scale
@@ -145,6 +180,7 @@ heal_gemm_smallm_kernel(const __grid_constant__ CUtensorMap tm_x_hi, const __gri
         const int last_seg = static_cast<int>(rank) + (n_local - 1) * static_cast<int>(cs);
         n_t = (n_local - 1) * kTilesPerSeg + (min(k_tiles, (last_seg + 1) * kTilesPerSeg) - last_seg * kTilesPerSeg);
     }
+    const int n_steps = Cfg::SCALED ? 2 * n_t : n_t;     // pipeline steps (SCALED: every k-tile of W travels twice)
     // ranks that finish at least one token row (rank r owns rows [r * rows_per_rank, (r + 1) * rows_per_rank))
     const int owners = cs > 1 ? (args.M + args.rows_per_rank - 1) / args.rows_per_rank : 1;
 
@@ -231,7 +267,8 @@ heal_gemm_smallm_kernel(const __grid_constant__ CUtensorMap tm_x_hi, const __gri
             };
             auto fbar = [&](int st) { return PAIR ? leader_addr(full_bar(st)) : full_bar(st); };
             auto load_w = [&](int t, uint32_t sb, uint32_t fb) {
-                const int k0 = ((static_cast<int>(rank) + (t >> 3) * static_cast<int>(cs)) * kTilesPerSeg + (t & 7)) * kBK;
+                const SmallStep sp = small_step<Cfg::SCALED>(t, n_t, n_local);
+                const int k0 = ((static_cast<int>(rank) + sp.seg_j * static_cast<int>(cs)) * kTilesPerSeg + sp.kk) * kBK;
                 if (Cfg::B_MN) {
 #pragma unroll
                     for (int c = 0; c < 2; ++c) {
@@ -244,18 +281,23 @@ heal_gemm_smallm_kernel(const __grid_constant__ CUtensorMap tm_x_hi, const __gri
                 }
             };
             auto load_x = [&](int t, uint32_t sb, uint32_t fb) {
-                const int k0 = ((static_cast<int>(rank) + (t >> 3) * static_cast<int>(cs)) * kTilesPerSeg + (t & 7)) * kBK;
+                const SmallStep sp = small_step<Cfg::SCALED>(t, n_t, n_local);
+                const int k0 = ((static_cast<int>(rank) + sp.seg_j * static_cast<int>(cs)) * kTilesPerSeg + sp.kk) * kBK;
                 const uint32_t sx = sb + Cfg::W_BYTES;
                 const int m_first = static_cast<int>(prank) * Cfg::XROWS;          // PAIR: this CTA's half of the tokens
-                ld_x(sx, &tm_x_hi, fb, k0, m_first);
-                if (Cfg::A_PLANES == 2) ld_x(sx + Cfg::X_TILE_AL, &tm_x_lo, fb, k0, m_first);
+                if (Cfg::SCALED) {
+                    ld_x(sx, sp.lo_pass ? &tm_x_lo : &tm_x_hi, fb, k0, m_first);
+                } else {
+                    ld_x(sx, &tm_x_hi, fb, k0, m_first);
+                    if (Cfg::A_PLANES == 2) ld_x(sx + Cfg::X_TILE_AL, &tm_x_lo, fb, k0, m_first);
+                }
             };
             int stage = 0, t = 0;
             uint32_t phase = 0;
             if (early_w && !FUSED) {
                 // static weights: fill the pipeline with W tiles now, add the activation tiles once the
                 // stream predecessor (which may have produced them) has completed
-                const int pre = min(STAGES, n_t);
+                const int pre = min(STAGES, n_steps);
                 for (int s = 0; s < pre; ++s) {
                     expect(fbar(s));
                     load_w(s, smem_base + s * Cfg::STAGE_BYTES, fbar(s));
@@ -266,7 +308,7 @@ heal_gemm_smallm_kernel(const __grid_constant__ CUtensorMap tm_x_hi, const __gri
                 t = pre;
                 if (pre == STAGES) phase = 1u; else stage = pre;
             }
-            for (; t < n_t; ++t) {
+            for (; t < n_steps; ++t) {
                 mbar_wait_ool(empty_bar(stage), phase ^ 1u, args.diag, 500 + stage);
                 const uint32_t sb = smem_base + stage * Cfg::STAGE_BYTES;
                 const uint32_t fb = fbar(stage);
@@ -293,6 +335,10 @@ heal_gemm_smallm_kernel(const __grid_constant__ CUtensorMap tm_x_hi, const __gri
                 if (PAIR) umma_f16_2cta(d, a, b, idesc, acc);
                 else      umma_f16(d, a, b, idesc, acc);
             };
+            auto mma_scale_d = [&](uint32_t d, uint64_t a, uint64_t b) {      // D = a.b + D * 2^-kLoShift
+                if (PAIR) umma_f16_2cta_scale_d<kLoShift>(d, a, b, idesc);
+                else      umma_f16_scale_d<kLoShift>(d, a, b, idesc);
+            };
             auto commit = [&](uint32_t bar) {                  // PAIR: the barrier at this offset in both CTAs
                 if (PAIR) umma_commit_2cta(bar, 3);
                 else      umma_commit(bar);
@@ -304,10 +350,11 @@ heal_gemm_smallm_kernel(const __grid_constant__ CUtensorMap tm_x_hi, const __gri
             int stage = 0;
             uint32_t phase = 0;
             uint32_t accumulate = 0;
-            for (int t = 0; t < n_t; ++t) {
-                const int seg_j = t >> 3;
+            for (int t = 0; t < n_steps; ++t) {
+                const SmallStep sp = small_step<Cfg::SCALED>(t, n_t, n_local);
+                const int seg_j = sp.seg_j;
                 const int slot = ring ? seg_j % ring : seg_j;
-                if ((t & 7) == 0) {                               // new segment -> next TMEM slot
+                if (sp.first) {                                   // new segment -> next TMEM slot
                     accumulate = 0;
                     if (ring && seg_j >= ring) {                  // the slot's previous segment must have been drained
                         mbar_wait_ool(tempty_bar(slot), static_cast<uint32_t>((seg_j / ring - 1) & 1), args.diag, 640 + slot);
@@ -319,7 +366,7 @@ heal_gemm_smallm_kernel(const __grid_constant__ CUtensorMap tm_x_hi, const __gri
                 if (FUSED) mbar_wait_ool(xfull_bar(stage), phase, args.diag, 620 + stage);
                 tc_fence_after();
                 if (t == 0) HEAL_STAMP(args.trace, 4);
-                if (t == n_t - 1) HEAL_STAMP(args.trace, 5);
+                if (t == n_steps - 1) HEAL_STAMP(args.trace, 5);
                 const uint32_t sb = smem_base + stage * Cfg::STAGE_BYTES;
                 const uint64_t w_hi = wdesc0 | desc_addr(sb);
                 const uint64_t w_lo = wdesc0 | desc_addr(sb + Cfg::W_TILE);
@@ -329,6 +376,12 @@ heal_gemm_smallm_kernel(const __grid_constant__ CUtensorMap tm_x_hi, const __gri
 #pragma unroll
                 for (int q = 0; q < kBK / 16; ++q) {
                     const uint64_t wo = static_cast<uint64_t>(q * w_step), xo = static_cast<uint64_t>(q * x_step);
+                    if (Cfg::SCALED) {                     // x_hi is the step's plane: the residual in the first pass
+                        if (!sp.lo_pass && sp.kk == 0 && q == 0) mma_scale_d(d_tmem, w_hi + wo, x_hi + xo);
+                        else                                     mma(d_tmem, w_hi + wo, x_hi + xo, accumulate);
+                        accumulate = 1;
+                        continue;
+                    }
                     // product order as in the large-M kernel: a_hi.b_hi, a_hi.b_lo, a_lo.b_hi, a_lo.b_lo
                     mma(d_tmem, w_hi + wo, x_hi + xo, accumulate);
                     accumulate = 1;
@@ -340,7 +393,7 @@ heal_gemm_smallm_kernel(const __grid_constant__ CUtensorMap tm_x_hi, const __gri
                     if (NPROD == 4) mma(d_tmem, w_lo + wo, x_lo + xo, 1);
                 }
                 commit(empty_bar(stage));
-                if (ring && ((t & 7) == 7 || t == n_t - 1)) commit(tfull_bar(slot));           // segment complete
+                if (ring && sp.last) commit(tfull_bar(slot));                                  // segment complete
                 if (++stage == STAGES) { stage = 0; phase ^= 1u; }
             }
             commit(done_bar);                              // all local segments complete in TMEM

@@ -755,7 +755,8 @@ def test_scaled_split_bit_exact(hb, oracle, inputs):
         assert np.array_equal(lo.cpu().numpy().view(np.uint16), olo)
 
 
-@pytest.mark.parametrize("M,N,K", [(8, 520, 4096), (300, 1032, 4096), (64, 264, 14336), (1300, 4104, 2056), (256, 1032, 4096 + 72)])
+@pytest.mark.parametrize("M,N,K", [(8, 520, 4096), (300, 1032, 4096), (64, 264, 14336), (1300, 4104, 2056), (256, 1032, 4096 + 72),
+                                   (16, 1032, 4096 + 72), (33, 26632, 2600), (1, 4096, 512), (24, 136, 328)])
 def test_lo_scaled_variant(hb, oracle, inputs, M, N, K):
     """HEAL_LO_SCALED (Eq. 10 as printed, s = 10; one kernel, one accumulator: per K segment the lo'.W products first, then the
     hi.W products with the accumulator scaled by 2^-10 inside the tensor core): against the oracle's exact evaluation of the
@@ -794,6 +795,30 @@ def test_lo_scaled_variant(hb, oracle, inputs, M, N, K):
     e0 = oracle.normwise_error(hb.heal_gemm(dev(At), Wd, 2).cpu().numpy(), ref, At, W)
     e10 = oracle.normwise_error(hb.heal_gemm(dev(At), Wd, mode).cpu().numpy(), ref, At, W)
     assert e10 <= GATE and e10 * 16 < e0, (e0, e10)
+
+
+@pytest.mark.parametrize("M,N,K", [(5, 1032, 6144 + 40), (48, 27000, 1104), (64, 2056, 7168)])
+def test_lo_scaled_small_m_weights_n_by_k(hb, oracle, inputs, M, N, K):
+    """HEAL_LO_SCALED on the small-M kernel (cluster K split, cta_group::2 pairs, TMEM ring) with weights stored N x K: same
+    bits as the large-M kernels and as the K x N layout, and the oracle's evaluation of the same products."""
+    A = inputs.activations(M, K, seed=26, outliers=True)
+    W = inputs.weights_f16(K, N, seed=26)
+    Ad, Wd = dev(A), dev(W)
+    Wt = Wd.t().contiguous()
+    mode = 2 | hb.LO_SCALED
+    try:
+        hb.debug_force_kernel(2 if M > 32 else 0)             # this mode leaves M > 32 to the large-M kernels by itself
+        got = hb.heal_gemm(Ad, Wt, mode | hb.B_NK)
+        assert "smallm" in hb.last_kernel() and "scaled lo" in hb.last_kernel()
+        assert torch.equal(hb.heal_gemm(Ad, Wd, mode), got)
+        hb.debug_force_kernel(1)
+        assert torch.equal(hb.heal_gemm(Ad, Wt, mode | hb.B_NK), got)
+        assert "smallm" not in hb.last_kernel()
+    finally:
+        hb.debug_force_kernel(0)
+    rows = np.array(sorted({0, M // 2, M - 1}))
+    o3 = oracle.gemm_split(A[rows], W, 2, s=10)
+    assert np.all(np.abs(got.cpu().numpy()[rows] - o3) <= 2 * elementwise_bound(A[rows], W, K, 2) + 1e-30)
 
 
 def test_lo_scaled_errors(hb):
