@@ -704,7 +704,11 @@ struct SmallIn {
 // st.async pushes (lowest latency) pay off while a thread sends few values: up to 8 of any width, or up to 32 8-byte
 // vectors (the plain path has no 8-byte form and falls back to 4-byte remote stores, which are slow; measured: M = 16,
 // K = 6144 21.7 -> 15.7 us, K = 14336 36.9 -> 26.9 us).
-inline bool async_push_ok(int64_t pushes, int64_t vw) { return pushes <= 8 || (vw == 2 && pushes <= 32); }
+inline bool async_push_ok(int64_t pushes, int64_t vw)
+{
+    static const long lim = std::getenv("HEAL_ASYNC_MAX") ? std::atol(std::getenv("HEAL_ASYNC_MAX")) : 8;      // tuning
+    return pushes <= lim || (vw == 2 && pushes <= 32);
+}
 
 template <class Cfg>
 int launch_small_cfg(int64_t M, int64_t N, int64_t K, const SmallIn &in, const void *B_hi, const void *B_lo, int64_t ldb,
@@ -732,6 +736,14 @@ int launch_small_cfg(int64_t M, int64_t N, int64_t K, const SmallIn &in, const v
                 break;
             }
         }
+    }
+    // All CTAs of the grid should be resident at once (a small second wave costs a whole first-tile latency and its stream runs
+    // on a fraction of the SMs): two CTAs fit an SM when a stage exceeds 24 KB, else three (the smem budgets below).  Measured:
+    // 64 x 6144 x 4096 (48 panels) 28.9 -> 25.2 us and 40 x 6144 x 4096 25.4 -> 20.4 us with clusters of 4 instead of 8.
+    {
+        static const bool no_cap = std::getenv("HEAL_NO_WAVE_CAP") != nullptr;      // debug only
+        const int64_t capacity = static_cast<int64_t>(Cfg::STAGE_BYTES > 24 * 1024 ? 2 : 3) * g.num_sms;
+        while (!no_cap && cs > 1 && panels * cs > capacity) cs /= 2;
     }
     if (const char *e = std::getenv("HEAL_SMALL_CS")) {                          // debug only
         const int want = std::atoi(e);

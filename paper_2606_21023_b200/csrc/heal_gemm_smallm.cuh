@@ -562,8 +562,8 @@ heal_gemm_smallm_kernel(const __grid_constant__ CUtensorMap tm_x_hi, const __gri
                 cluster_arrive_relaxed();
                 cluster_wait();
             }
-            // push this rank's partials: token m -> rank m / rpr, float (seg * 128 + nl) * rpr + m % rpr of its
-            // red area (the rpr values a thread sends for one segment are contiguous: vector stores)
+            // push this rank's partials: token m -> rank m / rpr; its red area holds, per segment, [nl][rpr] floats, or for
+            // rpr % 4 == 0 [rpr / 4][nl] 16-byte vectors of four consecutive rows
             const int rpr = args.rows_per_rank;
             for (int j = 0; j < n_local; ++j) {
                 const int seg = static_cast<int>(rank) + j * static_cast<int>(cs);
@@ -586,7 +586,8 @@ heal_gemm_smallm_kernel(const __grid_constant__ CUtensorMap tm_x_hi, const __gri
 #pragma unroll
                             for (int i = 0; i < 16; i += 4) {
                                 if (c * 16 + i < Mr) {    // rpr % 4 == 0: rows m..m+3 have one owner (rows >= M: unused zeros)
-                                    const uint32_t a = map_to_cta(red_base + row_off + ml * 4u, dst);
+                                    // groups of four rows are the slow index: a warp's vector stores land on 512 contiguous bytes
+                                    const uint32_t a = map_to_cta(red_base + ((static_cast<uint32_t>(seg * (rpr >> 2)) + (ml >> 2)) * kSmallBNW + nl) * 16u, dst);
                                     if (async) st_async_v4(a, v[i], v[i + 1], v[i + 2], v[i + 3], map_to_cta(red_bar, dst));
                                     else       st_dsmem_v4(a, v[i], v[i + 1], v[i + 2], v[i + 3]);
                                 }
@@ -636,7 +637,7 @@ heal_gemm_smallm_kernel(const __grid_constant__ CUtensorMap tm_x_hi, const __gri
                 const int seg_stride = kSmallBNW * rpr;
                 if ((rpr & 3) == 0) {
                     for (int r4 = 0; r4 < rows; r4 += 4) {
-                        const float4 *src = reinterpret_cast<const float4 *>(red + nl * rpr + r4);
+                        const float4 *src = reinterpret_cast<const float4 *>(red) + (r4 >> 2) * kSmallBNW + nl;
                         float4 acc = src[0];
 #pragma unroll 4
                         for (int s = 1; s < args.n_seg; ++s) {
