@@ -737,26 +737,32 @@ int launch_small_cfg(int64_t M, int64_t N, int64_t K, const SmallIn &in, const v
             }
         }
     }
-    // All CTAs of the grid should be resident at once (a small second wave costs a whole first-tile latency and its stream runs
-    // on a fraction of the SMs): two CTAs fit an SM when a stage exceeds 24 KB, else three (the smem budgets below).  Measured:
-    // 64 x 6144 x 4096 (48 panels) 28.9 -> 25.2 us and 40 x 6144 x 4096 25.4 -> 20.4 us with clusters of 4 instead of 8.
-    {
-        static const bool no_cap = std::getenv("HEAL_NO_WAVE_CAP") != nullptr;      // debug only
-        const int64_t capacity = static_cast<int64_t>(Cfg::STAGE_BYTES > 24 * 1024 ? 2 : 3) * g.num_sms;
-        while (!no_cap && cs > 1 && panels * cs > capacity) cs /= 2;
-    }
+    bool forced_cs = false, no_fit_possible = false;
     if (const char *e = std::getenv("HEAL_SMALL_CS")) {                          // debug only
         const int want = std::atoi(e);
         if (!Cfg::PAIR && want >= 1 && want <= 8) cs = want <= n_seg ? want : cs;
+        forced_cs = true;
     }
-    int max_local = (n_seg + cs - 1) / cs;
+    // Everything below depends on the cluster size.  It is planned in a loop because all CTAs of the grid should be resident at
+    // once: a small second wave pays a whole first-tile latency and streams on a fraction of the SMs (measured: 32 x 6144 x 4096,
+    // 384 CTAs of 88 KB, 19.1 us with 88 CTAs in a second wave; 64 x 6144 x 4096 28.9 -> 19.7 us with clusters of 4 instead of 8).
+    // If the grid does not fit, in this order: two pipeline stages, the pushed partial sums overlaid on the pipeline, both, and
+    // finally half the cluster size.
+    static const bool no_wave_fit = std::getenv("HEAL_NO_WAVE_CAP") != nullptr;      // debug only
+    int max_local = 0, ring = 0, tmem_cols = 32, rpr = 0, stages = 0;
+    size_t red = 0, smem = 0;
+    bool use_ring = false, red_alias = false;
+    for (int remedy = 0;; ++remedy) {
+    const int stage_cap = (remedy == 1 || remedy == 3) ? 2 : kSmallMaxStages;
+    const bool force_alias = remedy == 2 || remedy == 3;
+    max_local = (n_seg + cs - 1) / cs;
     // One CTA per panel reading planes, and the segments would need more than 256 TMEM columns (one CTA per SM):
     // they cycle through a ring of TMEM slots instead (256 columns, so two CTAs fit per SM and one's epilogue
     // overlaps the other's stream) and the epilogue keeps the running sum.  Measured: LM head M = 64 227 -> 202 us;
     // where everything fits in 256 columns anyway the plain "drain at the end" epilogue is faster (LM head M = 1
     // 161 vs 168 us), so the ring is used only when needed.
-    const bool use_ring = cs == 1 && !Cfg::FUSED && n_seg * Cfg::MPAD > 256;
-    int ring = 0;
+    use_ring = cs == 1 && !Cfg::FUSED && n_seg * Cfg::MPAD > 256;
+    ring = 0;
     if (use_ring) {
         ring = 256 / Cfg::MPAD;
         if (ring > n_seg) ring = n_seg;
@@ -766,14 +772,14 @@ int launch_small_cfg(int64_t M, int64_t N, int64_t K, const SmallIn &in, const v
         cs *= 2;
         max_local = (n_seg + cs - 1) / cs;
     }
-    int tmem_cols = 32;
+    tmem_cols = 32;
     while (tmem_cols < (use_ring ? ring : max_local) * Cfg::MPAD) tmem_cols *= 2;
     if (tmem_cols > 512) return HEAL_OK;                        // leave to the large-M kernel
     // token rows finished by one rank; 3 or more are rounded up to a multiple of 4 so that the pushes are 16-byte vectors
     // (fewer ranks then own rows; measured: M = 24 decode 16.5 us with 4-byte pushes vs 9.9 us at M = 32)
-    int rpr = cs > 1 ? static_cast<int>((M + cs - 1) / cs) : 0;
+    rpr = cs > 1 ? static_cast<int>((M + cs - 1) / cs) : 0;
     if (rpr >= 3) rpr = (rpr + 3) / 4 * 4;
-    const size_t red = cs > 1 ? static_cast<size_t>(n_seg) * rpr * kSmallBNW * 4 : 0;
+    red = cs > 1 ? static_cast<size_t>(n_seg) * rpr * kSmallBNW * 4 : 0;
     // Shared memory.  Measured on B200 (decode 4096 x 4096, LM head): what matters is how many CTAs are resident
     // -- the next kernel's CTAs run their prologue (and with HEAL_B_STATIC prefetch W) beside this kernel's --
     // rather than the depth of one CTA's pipeline: aim for three CTAs per SM (two when a stage exceeds 24 KB,
@@ -781,22 +787,23 @@ int launch_small_cfg(int64_t M, int64_t N, int64_t K, const SmallIn &in, const v
     // has k-tiles.
     // Partial sums pushed by the cluster: a dedicated area when small (decode), else overlaid on the pipeline.
     static const size_t alias_min = std::getenv("HEAL_RED_ALIAS_MIN") ? static_cast<size_t>(std::atol(std::getenv("HEAL_RED_ALIAS_MIN"))) : 16 * 1024;   // debug only
-    const bool red_alias = red > alias_min;
+    red_alias = red > alias_min || (force_alias && red > 0);
     const size_t fixed = (red_alias ? 0 : red) + Cfg::BAR_BYTES;          // no alignment slack: see the kernel
     size_t budget = tmem_cols > 256 ? static_cast<size_t>(kSmemLimit)
                     : (Cfg::STAGE_BYTES <= 24 * 1024 && cs > 1 ? static_cast<size_t>(74 * 1024) : static_cast<size_t>(112 * 1024));
-    if (budget < fixed + 3 * static_cast<size_t>(Cfg::STAGE_BYTES) && budget < static_cast<size_t>(112 * 1024)) budget = static_cast<size_t>(112 * 1024);
-    if (budget < fixed + 3 * static_cast<size_t>(Cfg::STAGE_BYTES)) budget = static_cast<size_t>(kSmemLimit);
+    const size_t min_stages = stage_cap < 3 ? 2 : 3;
+    if (budget < fixed + min_stages * static_cast<size_t>(Cfg::STAGE_BYTES) && budget < static_cast<size_t>(112 * 1024)) budget = static_cast<size_t>(112 * 1024);
+    if (budget < fixed + min_stages * static_cast<size_t>(Cfg::STAGE_BYTES)) budget = static_cast<size_t>(kSmemLimit);
     if (budget < fixed + 2 * static_cast<size_t>(Cfg::STAGE_BYTES)) return HEAL_OK;      // large-M kernel
     if (red_alias && fixed + red > static_cast<size_t>(kSmemLimit)) return HEAL_OK;
-    int stages = static_cast<int>((budget - fixed) / Cfg::STAGE_BYTES);
-    if (stages > kSmallMaxStages) stages = kSmallMaxStages;
-    if (stages > max_local * kTilesPerSeg) stages = max_local * kTilesPerSeg;
+    stages = static_cast<int>((budget - fixed) / Cfg::STAGE_BYTES);
+    if (stages > stage_cap) stages = stage_cap;
+    if (stages > max_local * kTilesPerSeg * (Cfg::SCALED ? 2 : 1)) stages = max_local * kTilesPerSeg * (Cfg::SCALED ? 2 : 1);
     if (const char *e = std::getenv("HEAL_SMALL_STAGES")) {                      // debug only
         const int want = std::atoi(e);
         if (want >= 2 && want <= kSmallMaxStages && fixed + static_cast<size_t>(want) * Cfg::STAGE_BYTES <= static_cast<size_t>(kSmemLimit)) stages = want;
     }
-    size_t smem = fixed + static_cast<size_t>(stages) * Cfg::STAGE_BYTES;
+    smem = fixed + static_cast<size_t>(stages) * Cfg::STAGE_BYTES;
     if (red_alias && smem < fixed + red) smem = fixed + red;
     // TMEM must never be oversubscribed by the CTAs an SM can hold: a CTA blocked in tcgen05.alloc has not yet arrived at
     // its cluster barrier, its peers hold TMEM elsewhere while they wait for it, and a cycle of such waits across clusters
@@ -807,6 +814,31 @@ int launch_small_cfg(int64_t M, int64_t N, int64_t K, const SmallIn &in, const v
         const size_t need = (static_cast<size_t>(tmem_cols) * (228 * 1024) + 511) / 512;
         if (smem + 1024 < need) smem = need - 1024;
         if (smem > static_cast<size_t>(kSmemLimit)) smem = static_cast<size_t>(kSmemLimit);
+    }
+    static const int reg_limit = [] {                    // CTAs per SM the register file allows (64 K registers, 256 per warp at a time)
+        cudaFuncAttributes fa;
+        if (cudaFuncGetAttributes(&fa, heal_gemm_smallm_kernel<Cfg>) != cudaSuccess || fa.numRegs <= 0) return 1;
+        const int per_warp = (fa.numRegs * 32 + 255) / 256 * 256;
+        return 65536 / (per_warp * (kSmallThreads / 32));
+    }();
+    int64_t per_sm = static_cast<int64_t>((228 * 1024) / (smem + 1024));
+    if (per_sm > reg_limit) per_sm = reg_limit;
+    const int64_t grid = Cfg::PAIR ? (panels + 1) / 2 * 2 : panels * cs;
+    // fused split with more than 16 tokens: the converter warps only keep up while at most two CTAs share an SM; past that the
+    // caller splits first and comes back with planes (measured, M = 32: 5120 x 5120 32.2 fused vs 19.5 us, 6144 x 4096 21.1 vs 15.6 us)
+    if (Cfg::FUSED && M > 16 && grid > 2 * static_cast<int64_t>(g.num_sms) && !forced_cs) return HEAL_OK;
+    if (no_wave_fit || forced_cs || no_fit_possible || cs == 1 || grid <= per_sm * g.num_sms) break;
+    if (remedy == 3) {                  // nothing made the grid fit at this cluster size: halve it, unless TMEM then overflows
+        const int half_local = (n_seg + cs / 2 - 1) / (cs / 2);
+        const bool ring_ok = cs / 2 == 1 && !Cfg::FUSED;
+        if (half_local * Cfg::MPAD > 512 && !ring_ok) {
+            remedy = -1;                // keep the plan of the first attempt at this size
+            no_fit_possible = true;
+            continue;
+        }
+        cs /= 2;
+        remedy = -1;
+    }
     }
     auto kern = heal_gemm_smallm_kernel<Cfg>;
     static std::atomic<size_t> attr_smem{0};           // only ever raised: a concurrent smaller request cannot lower it
