@@ -737,109 +737,144 @@ int launch_small_cfg(int64_t M, int64_t N, int64_t K, const SmallIn &in, const v
             }
         }
     }
-    bool forced_cs = false, no_fit_possible = false;
+    bool forced_cs = false;
     if (const char *e = std::getenv("HEAL_SMALL_CS")) {                          // debug only
         const int want = std::atoi(e);
         if (!Cfg::PAIR && want >= 1 && want <= 8) cs = want <= n_seg ? want : cs;
         forced_cs = true;
     }
-    // Everything below depends on the cluster size.  It is planned in a loop because all CTAs of the grid should be resident at
-    // once: a small second wave pays a whole first-tile latency and streams on a fraction of the SMs (measured: 32 x 6144 x 4096,
-    // 384 CTAs of 88 KB, 19.1 us with 88 CTAs in a second wave; 64 x 6144 x 4096 28.9 -> 19.7 us with clusters of 4 instead of 8).
-    // If the grid does not fit, in this order: two pipeline stages, the pushed partial sums overlaid on the pipeline, both, and
-    // finally half the cluster size.
-    static const bool no_wave_fit = std::getenv("HEAL_NO_WAVE_CAP") != nullptr;      // debug only
-    int max_local = 0, ring = 0, tmem_cols = 32, rpr = 0, stages = 0;
-    size_t red = 0, smem = 0;
-    bool use_ring = false, red_alias = false;
-    for (int remedy = 0;; ++remedy) {
-    const int stage_cap = (remedy == 1 || remedy == 3) ? 2 : kSmallMaxStages;
-    const bool force_alias = remedy == 2 || remedy == 3;
-    max_local = (n_seg + cs - 1) / cs;
-    // One CTA per panel reading planes, and the segments would need more than 256 TMEM columns (one CTA per SM):
-    // they cycle through a ring of TMEM slots instead (256 columns, so two CTAs fit per SM and one's epilogue
-    // overlaps the other's stream) and the epilogue keeps the running sum.  Measured: LM head M = 64 227 -> 202 us;
-    // where everything fits in 256 columns anyway the plain "drain at the end" epilogue is faster (LM head M = 1
-    // 161 vs 168 us), so the ring is used only when needed.
-    use_ring = cs == 1 && !Cfg::FUSED && n_seg * Cfg::MPAD > 256;
-    ring = 0;
-    if (use_ring) {
-        ring = 256 / Cfg::MPAD;
-        if (ring > n_seg) ring = n_seg;
-        if (ring > 16) ring = 16;
-    }
-    while (!use_ring && max_local * Cfg::MPAD > 512 && cs * 2 <= 8 && cs * 2 <= n_seg) {
-        cs *= 2;
-        max_local = (n_seg + cs - 1) / cs;
-    }
-    tmem_cols = 32;
-    while (tmem_cols < (use_ring ? ring : max_local) * Cfg::MPAD) tmem_cols *= 2;
-    if (tmem_cols > 512) return HEAL_OK;                        // leave to the large-M kernel
-    // token rows finished by one rank; 3 or more are rounded up to a multiple of 4 so that the pushes are 16-byte vectors
-    // (fewer ranks then own rows; measured: M = 24 decode 16.5 us with 4-byte pushes vs 9.9 us at M = 32)
-    rpr = cs > 1 ? static_cast<int>((M + cs - 1) / cs) : 0;
-    if (rpr >= 3) rpr = (rpr + 3) / 4 * 4;
-    red = cs > 1 ? static_cast<size_t>(n_seg) * rpr * kSmallBNW * 4 : 0;
-    // Shared memory.  Measured on B200 (decode 4096 x 4096, LM head): what matters is how many CTAs are resident
-    // -- the next kernel's CTAs run their prologue (and with HEAL_B_STATIC prefetch W) beside this kernel's --
-    // rather than the depth of one CTA's pipeline: aim for three CTAs per SM (two when a stage exceeds 24 KB,
-    // one when the CTA needs more than half of TMEM), at least 2 stages, at most 8 and no more than the CTA
-    // has k-tiles.
-    // Partial sums pushed by the cluster: a dedicated area when small (decode), else overlaid on the pipeline.
-    static const size_t alias_min = std::getenv("HEAL_RED_ALIAS_MIN") ? static_cast<size_t>(std::atol(std::getenv("HEAL_RED_ALIAS_MIN"))) : 16 * 1024;   // debug only
-    red_alias = red > alias_min || (force_alias && red > 0);
-    const size_t fixed = (red_alias ? 0 : red) + Cfg::BAR_BYTES;          // no alignment slack: see the kernel
-    size_t budget = tmem_cols > 256 ? static_cast<size_t>(kSmemLimit)
-                    : (Cfg::STAGE_BYTES <= 24 * 1024 && cs > 1 ? static_cast<size_t>(74 * 1024) : static_cast<size_t>(112 * 1024));
-    const size_t min_stages = stage_cap < 3 ? 2 : 3;
-    if (budget < fixed + min_stages * static_cast<size_t>(Cfg::STAGE_BYTES) && budget < static_cast<size_t>(112 * 1024)) budget = static_cast<size_t>(112 * 1024);
-    if (budget < fixed + min_stages * static_cast<size_t>(Cfg::STAGE_BYTES)) budget = static_cast<size_t>(kSmemLimit);
-    if (budget < fixed + 2 * static_cast<size_t>(Cfg::STAGE_BYTES)) return HEAL_OK;      // large-M kernel
-    if (red_alias && fixed + red > static_cast<size_t>(kSmemLimit)) return HEAL_OK;
-    stages = static_cast<int>((budget - fixed) / Cfg::STAGE_BYTES);
-    if (stages > stage_cap) stages = stage_cap;
-    if (stages > max_local * kTilesPerSeg * (Cfg::SCALED ? 2 : 1)) stages = max_local * kTilesPerSeg * (Cfg::SCALED ? 2 : 1);
-    if (const char *e = std::getenv("HEAL_SMALL_STAGES")) {                      // debug only
-        const int want = std::atoi(e);
-        if (want >= 2 && want <= kSmallMaxStages && fixed + static_cast<size_t>(want) * Cfg::STAGE_BYTES <= static_cast<size_t>(kSmemLimit)) stages = want;
-    }
-    smem = fixed + static_cast<size_t>(stages) * Cfg::STAGE_BYTES;
-    if (red_alias && smem < fixed + red) smem = fixed + red;
-    // TMEM must never be oversubscribed by the CTAs an SM can hold: a CTA blocked in tcgen05.alloc has not yet arrived at
-    // its cluster barrier, its peers hold TMEM elsewhere while they wait for it, and a cycle of such waits across clusters
-    // (or across kernels on concurrent streams) would hang.  Every kernel of the library therefore takes at least the
-    // same fraction of an SM's shared memory (228 KB, 1 KB reserved per CTA) as of its 512 TMEM columns, so whatever mix
-    // of the library's CTAs fits into an SM's shared memory also fits into its TMEM.
-    {
-        const size_t need = (static_cast<size_t>(tmem_cols) * (228 * 1024) + 511) / 512;
-        if (smem + 1024 < need) smem = need - 1024;
-        if (smem > static_cast<size_t>(kSmemLimit)) smem = static_cast<size_t>(kSmemLimit);
-    }
+    // CTAs of this kernel the GPU holds at once for a cluster size and a shared-memory size.  The driver's occupancy calls answer
+    // "one CTA per SM" for every kernel that allocates tensor memory, whatever its size (the hardware does co-locate them: phase
+    // stamps show up to three of these CTAs per SM), so the estimate is made here: CTAs per SM by shared memory and registers, and
+    // for clusters the driver's own cudaOccupancyMaxActiveClusters table of a plain 192-thread kernel on this 148-SM part (a cluster
+    // has to fit into one GPC, and the GPCs have different sizes: e.g. 37 clusters of 7 at two CTAs per SM, not 42).
     static const int reg_limit = [] {                    // CTAs per SM the register file allows (64 K registers, 256 per warp at a time)
         cudaFuncAttributes fa;
         if (cudaFuncGetAttributes(&fa, heal_gemm_smallm_kernel<Cfg>) != cudaSuccess || fa.numRegs <= 0) return 1;
         const int per_warp = (fa.numRegs * 32 + 255) / 256 * 256;
         return 65536 / (per_warp * (kSmallThreads / 32));
     }();
-    int64_t per_sm = static_cast<int64_t>((228 * 1024) / (smem + 1024));
-    if (per_sm > reg_limit) per_sm = reg_limit;
-    const int64_t grid = Cfg::PAIR ? (panels + 1) / 2 * 2 : panels * cs;
+    auto resident = [&](int c, size_t smem_bytes) -> int64_t {
+        static const int kClusters148[3][8] = {{148, 74, 45, 33, 26, 22, 15, 15},          // one CTA per SM, cluster size 1..8
+                                               {296, 148, 93, 71, 56, 45, 37, 33},         // two
+                                               {444, 222, 142, 104, 82, 71, 56, 48}};      // three
+        int64_t per_sm = static_cast<int64_t>((228 * 1024) / (smem_bytes + 1024));
+        if (per_sm > reg_limit) per_sm = reg_limit;
+        if (per_sm < 1) per_sm = 1;
+        const int cx = Cfg::PAIR ? 2 : c;
+        if (g.num_sms == 148 && per_sm <= 3) return static_cast<int64_t>(kClusters148[per_sm - 1][cx - 1]) * cx;
+        if (g.num_sms == 148) return static_cast<int64_t>(kClusters148[2][cx - 1]) * cx * per_sm / 3;
+        return per_sm * g.num_sms / cx * cx * (cx > 2 ? 9 : 10) / 10;                      // other parts: a tenth lost to GPC boundaries
+    };
+    // Everything else follows from the cluster size c and two options (at most two pipeline stages; partial sums overlaid on the
+    // pipeline even when small).  status: 0 = launchable, 1 = leave to the large-M kernel.
+    struct Plan {
+        int status, cs, max_local, ring, tmem_cols, rpr, stages;
+        size_t red, smem;
+        bool red_alias;
+        int64_t grid, slots;               // CTAs of the launch; CTAs the GPU holds at once
+        int64_t cost() const { return (grid + slots - 1) / slots * max_local; }     // waves x segments per CTA
+        bool fits() const { return grid <= slots; }
+    };
+    auto plan = [&](int c, bool two_stages, bool force_alias) {
+        Plan q = {};
+        q.status = 1;
+        q.cs = c;
+        q.max_local = (n_seg + c - 1) / c;
+        // One CTA per panel reading planes, and the segments would need more than 256 TMEM columns (one CTA per SM):
+        // they cycle through a ring of TMEM slots instead (256 columns, so two CTAs fit per SM and one's epilogue
+        // overlaps the other's stream) and the epilogue keeps the running sum.  Measured: LM head M = 64 227 -> 202 us;
+        // where everything fits in 256 columns anyway the plain "drain at the end" epilogue is faster (LM head M = 1
+        // 161 vs 168 us), so the ring is used only when needed.
+        const bool use_ring = c == 1 && !Cfg::FUSED && n_seg * Cfg::MPAD > 256;
+        if (use_ring) {
+            q.ring = 256 / Cfg::MPAD;
+            if (q.ring > n_seg) q.ring = n_seg;
+            if (q.ring > 16) q.ring = 16;
+        }
+        q.tmem_cols = 32;
+        while (q.tmem_cols < (use_ring ? q.ring : q.max_local) * Cfg::MPAD) q.tmem_cols *= 2;
+        if (q.tmem_cols > 512) return q;
+        // token rows finished by one rank; 3 or more are rounded up to a multiple of 4 so that the pushes are 16-byte vectors
+        // (fewer ranks then own rows; measured: M = 24 decode 16.5 us with 4-byte pushes vs 9.9 us at M = 32)
+        q.rpr = c > 1 ? static_cast<int>((M + c - 1) / c) : 0;
+        if (q.rpr >= 3) q.rpr = (q.rpr + 3) / 4 * 4;
+        q.red = c > 1 ? static_cast<size_t>(n_seg) * q.rpr * kSmallBNW * 4 : 0;
+        // Shared memory.  Measured on B200 (decode 4096 x 4096, LM head): what matters is how many CTAs are resident
+        // -- the next kernel's CTAs run their prologue (and with HEAL_B_STATIC prefetch W) beside this kernel's --
+        // rather than the depth of one CTA's pipeline: aim for three CTAs per SM (two when a stage exceeds 24 KB,
+        // one when the CTA needs more than half of TMEM), at least 2 stages, at most 8 and no more than the CTA
+        // has k-tiles.
+        // Partial sums pushed by the cluster: a dedicated area when small (decode), else overlaid on the pipeline.
+        static const size_t alias_min = std::getenv("HEAL_RED_ALIAS_MIN") ? static_cast<size_t>(std::atol(std::getenv("HEAL_RED_ALIAS_MIN"))) : 16 * 1024;   // debug only
+        q.red_alias = q.red > alias_min || (force_alias && q.red > 0);
+        const size_t fixed = (q.red_alias ? 0 : q.red) + Cfg::BAR_BYTES;          // no alignment slack: see the kernel
+        size_t budget = q.tmem_cols > 256 ? static_cast<size_t>(kSmemLimit)
+                        : (Cfg::STAGE_BYTES <= 24 * 1024 && c > 1 ? static_cast<size_t>(74 * 1024) : static_cast<size_t>(112 * 1024));
+        const size_t min_stages = two_stages ? 2 : 3;
+        if (budget < fixed + min_stages * static_cast<size_t>(Cfg::STAGE_BYTES) && budget < static_cast<size_t>(112 * 1024)) budget = static_cast<size_t>(112 * 1024);
+        if (budget < fixed + min_stages * static_cast<size_t>(Cfg::STAGE_BYTES)) budget = static_cast<size_t>(kSmemLimit);
+        if (budget < fixed + 2 * static_cast<size_t>(Cfg::STAGE_BYTES)) return q;            // large-M kernel
+        if (q.red_alias && fixed + q.red > static_cast<size_t>(kSmemLimit)) return q;
+        q.stages = static_cast<int>((budget - fixed) / Cfg::STAGE_BYTES);
+        if (q.stages > (two_stages ? 2 : kSmallMaxStages)) q.stages = two_stages ? 2 : kSmallMaxStages;
+        const int steps = q.max_local * kTilesPerSeg * (Cfg::SCALED ? 2 : 1);
+        if (q.stages > steps) q.stages = steps;
+        if (const char *e = std::getenv("HEAL_SMALL_STAGES")) {                      // debug only
+            const int want = std::atoi(e);
+            if (want >= 2 && want <= kSmallMaxStages && fixed + static_cast<size_t>(want) * Cfg::STAGE_BYTES <= static_cast<size_t>(kSmemLimit)) q.stages = want;
+        }
+        q.smem = fixed + static_cast<size_t>(q.stages) * Cfg::STAGE_BYTES;
+        if (q.red_alias && q.smem < fixed + q.red) q.smem = fixed + q.red;
+        // TMEM must never be oversubscribed by the CTAs an SM can hold: a CTA blocked in tcgen05.alloc has not yet arrived at
+        // its cluster barrier, its peers hold TMEM elsewhere while they wait for it, and a cycle of such waits across clusters
+        // (or across kernels on concurrent streams) would hang.  Every kernel of the library therefore takes at least the
+        // same fraction of an SM's shared memory (228 KB, 1 KB reserved per CTA) as of its 512 TMEM columns, so whatever mix
+        // of the library's CTAs fits into an SM's shared memory also fits into its TMEM.
+        const size_t need = (static_cast<size_t>(q.tmem_cols) * (228 * 1024) + 511) / 512;
+        if (q.smem + 1024 < need) q.smem = need - 1024;
+        if (q.smem > static_cast<size_t>(kSmemLimit)) q.smem = static_cast<size_t>(kSmemLimit);
+        q.slots = resident(c, q.smem);
+        q.grid = Cfg::PAIR ? (panels + 1) / 2 * 2 : panels * c;
+        q.status = 0;
+        return q;
+    };
+    // TMEM: a cluster too small for its segments grows (as long as K allows)
+    while (!(cs == 1 && !Cfg::FUSED) && ((n_seg + cs - 1) / cs) * Cfg::MPAD > 512 && cs * 2 <= 8 && cs * 2 <= n_seg) cs *= 2;
+    Plan pl = plan(cs, false, false);
+    if (pl.status) return HEAL_OK;                              // leave to the large-M kernel
     // fused split with more than 16 tokens: the converter warps only keep up while at most two CTAs share an SM; past that the
     // caller splits first and comes back with planes (measured, M = 32: 5120 x 5120 32.2 fused vs 19.5 us, 6144 x 4096 21.1 vs 15.6 us)
-    if (Cfg::FUSED && M > 16 && grid > 2 * static_cast<int64_t>(g.num_sms) && !forced_cs) return HEAL_OK;
-    if (no_wave_fit || forced_cs || no_fit_possible || cs == 1 || grid <= per_sm * g.num_sms) break;
-    if (remedy == 3) {                  // nothing made the grid fit at this cluster size: halve it, unless TMEM then overflows
-        const int half_local = (n_seg + cs / 2 - 1) / (cs / 2);
-        const bool ring_ok = cs / 2 == 1 && !Cfg::FUSED;
-        if (half_local * Cfg::MPAD > 512 && !ring_ok) {
-            remedy = -1;                // keep the plan of the first attempt at this size
-            no_fit_possible = true;
-            continue;
+    if (Cfg::FUSED && M > 16 && pl.grid > 2 * static_cast<int64_t>(g.num_sms) && !forced_cs) return HEAL_OK;
+    // All CTAs of the grid should be resident at once: a small second wave pays a whole first-tile latency and streams on a
+    // fraction of the SMs (measured: 32 x 6144 x 4096, 384 CTAs of 88 KB, 19.1 us with 88 CTAs in a second wave, 13.7 us in one).
+    // If the plan does not fit: two pipeline stages, then the partial sums overlaid on the pipeline, then both; failing that, the
+    // cluster size (and options) with the fewest waves x segments per CTA, the smallest such cluster first (measured:
+    // 24 x 5120 x 17408 90 -> 40 us with clusters of 6 instead of 8, 64 x 10240 x 8192 80 -> 53 us, 32 x 8192 x 28672 138 -> 99 us).
+    static const bool no_wave_fit = std::getenv("HEAL_NO_WAVE_CAP") != nullptr;      // debug only
+    if (!pl.fits() && cs > 1 && !forced_cs && !no_wave_fit) {
+        bool found = false;
+        for (int opt = 1; opt < 4 && !found; ++opt) {
+            const Plan q = plan(cs, (opt & 1) != 0, (opt & 2) != 0);
+            if (q.status == 0 && q.fits()) { pl = q; found = true; }
         }
-        cs /= 2;
-        remedy = -1;
+        for (int c = 1; c <= 8 && !found; ++c) {
+            if (c > n_seg || c == cs) continue;
+            for (int opt = 0; opt < 4; ++opt) {
+                const Plan q = plan(c, (opt & 1) != 0, (opt & 2) != 0);
+                if (q.status == 0 && q.cost() < pl.cost()) pl = q;
+            }
+        }
     }
-    }
+    static const bool plan_debug = std::getenv("HEAL_PLAN_DEBUG") != nullptr;      // debug only
+    if (plan_debug)
+        std::fprintf(stderr, "[heal plan] M=%lld N=%lld K=%lld MPAD=%d fused=%d: cs %d -> %d, grid %lld slots %lld, max_local %d, tmem %d, stages %d, smem %zu, red %zu alias %d\n",
+                     (long long)M, (long long)N, (long long)K, Cfg::MPAD, (int)Cfg::FUSED, cs, pl.cs, (long long)pl.grid, (long long)pl.slots, pl.max_local, pl.tmem_cols,
+                     pl.stages, pl.smem, pl.red, (int)pl.red_alias);
+    cs = pl.cs;
+    const int max_local = pl.max_local, ring = pl.ring, tmem_cols = pl.tmem_cols, rpr = pl.rpr, stages = pl.stages;
+    const size_t red = pl.red, smem = pl.smem;
+    const bool red_alias = pl.red_alias;
     auto kern = heal_gemm_smallm_kernel<Cfg>;
     static std::atomic<size_t> attr_smem{0};           // only ever raised: a concurrent smaller request cannot lower it
     if (smem > attr_smem.load(std::memory_order_acquire)) {
