@@ -213,6 +213,31 @@ int heal_gemm_host_act(int64_t M, int64_t N, int64_t K,
                        void *C_host, int64_t ldc,
                        uint32_t mode, void *stream);
 
+/*
+ * heal_gemm for callers that must not allocate: code under CUDA graph capture, tight serving loops, harnesses that forbid
+ * cudaMalloc.  Same operation and same bits as heal_gemm (split, two-product MMA, FP32 epilogue), restricted to
+ * decode-sized problems, with every byte of scratch -- the hi/lo FP16 planes of A (step S) and the kernels' diagnostic words -- in
+ * ONE file-scope device array of HEAL_STATIC_SCRATCH_BYTES (+ 256 B) inside the library.  Every GPU that loads the library holds
+ * that array until the process exits.  The call makes no cudaMalloc / cudaFree and calls no allocating library routine, also when
+ * it is the first call into the library; it launches the split kernel and the small-M GEMM kernel on `stream` and returns.
+ *   A, B, C, lda, ldb, ldc, stream: as for heal_gemm (DEVICE pointers, same alignment rules); B is FP16.
+ *   mode: HEAL_MODE_1P or HEAL_MODE_2P, optionally | HEAL_B_NK | HEAL_B_STATIC; anything else: HEAL_ERR_UNSUPPORTED_MODE.
+ *   Limits: M <= HEAL_STATIC_MAX_M and 2 * roundup(M * roundup(K, 8) * 2, 256) <= HEAL_STATIC_SCRATCH_BYTES (every M <= 64 up to
+ *   K = 32768); beyond either, and for the few shapes the small-M kernel leaves to the large-M kernels, HEAL_ERR_WORKSPACE and
+ *   nothing is launched.
+ *   Sharing: all calls, on all streams, use the same array.  Calls that overlap on the GPU (different streams without an ordering
+ *   between them, or graphs replayed concurrently) RACE on the planes and give wrong results; calls on one stream, or otherwise
+ *   ordered, are safe.  The array keeps the previous call's planes; nothing in it needs clearing between calls (each call rewrites
+ *   the part it reads; the diagnostic words are zero from module load and change only when a kernel traps).
+ */
+#define HEAL_STATIC_SCRATCH_BYTES (8u << 20)
+#define HEAL_STATIC_MAX_M 64
+int heal_gemm_static(int64_t M, int64_t N, int64_t K,
+                     const void *A, int64_t lda,
+                     const void *B, int64_t ldb,
+                     void *C, int64_t ldc,
+                     uint32_t mode, void *stream);
+
 /* Bytes of workspace heal_gemm needs for this problem (hi/lo planes of A, and of B in 3P/4P). */
 size_t heal_workspace_size(int64_t M, int64_t N, int64_t K, uint32_t mode);
 

@@ -41,6 +41,8 @@ def lib():
         i64, vp, u32, ci = ctypes.c_int64, ctypes.c_void_p, ctypes.c_uint32, ctypes.c_int
         L.heal_gemm.restype = ci
         L.heal_gemm.argtypes = [i64, i64, i64, vp, i64, vp, i64, vp, i64, u32, vp]
+        L.heal_gemm_static.restype = ci
+        L.heal_gemm_static.argtypes = [i64, i64, i64, vp, i64, vp, i64, vp, i64, u32, vp]
         L.heal_gemm_host.restype = ci
         L.heal_gemm_host.argtypes = [i64, i64, i64, vp, i64, vp, i64, vp, i64, u32, vp]
         L.heal_gemm_host_act.restype = ci
@@ -135,6 +137,29 @@ def heal_gemm(A: torch.Tensor, B: torch.Tensor, mode: int = MODE_2P, C: torch.Te
         C = torch.empty((M, _n_out(N, mode)), dtype=torch.float32, device=A.device)
     _check(lib().heal_gemm(M, N, K, A.data_ptr(), _ld(A), B.data_ptr(), _ld(B), C.data_ptr(), _ld(C), mode,
                            _stream(stream)))
+    return C
+
+
+STATIC_SCRATCH_BYTES = 8 << 20
+STATIC_MAX_M = 64
+
+
+def heal_gemm_static_raw(M, N, K, A_ptr, lda, B_ptr, ldb, C_ptr, ldc, mode, stream=None) -> int:
+    """Status code of heal_gemm_static, no exception (for error-path tests)."""
+    return lib().heal_gemm_static(M, N, K, A_ptr, lda, B_ptr, ldb, C_ptr, ldc, mode, _stream(stream))
+
+
+def heal_gemm_static(A: torch.Tensor, B: torch.Tensor, mode: int = MODE_2P, C: torch.Tensor | None = None, stream=None):
+    """C = A.B through heal_gemm_static: the entry point that allocates nothing (scratch in a static device array of
+    STATIC_SCRATCH_BYTES inside the library; M <= STATIC_MAX_M, FP16 weights, 1P/2P).  Calls that overlap on the GPU race."""
+    assert A.is_cuda and B.is_cuda and A.dtype == torch.float32 and B.dtype == torch.float16
+    M, K = A.shape
+    N = B.shape[0] if mode & B_NK else B.shape[1]
+    assert (B.shape[1] if mode & B_NK else B.shape[0]) == K
+    if C is None:
+        C = torch.empty((M, N), dtype=torch.float32, device=A.device)
+    _check(lib().heal_gemm_static(M, N, K, A.data_ptr(), _ld(A), B.data_ptr(), _ld(B), C.data_ptr(), _ld(C), mode,
+                                  _stream(stream)))
     return C
 
 

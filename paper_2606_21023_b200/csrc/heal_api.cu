@@ -1130,6 +1130,65 @@ int scaled_impl(int64_t M, int64_t N, int64_t K, const void *A_hi, const void *A
     return presplit_impl(M, N, K, A_hi, A_lo, lda, B, nullptr, ldb, out, kScaledLo, b_nk, b_static, stream);
 }
 
+// ---- heal_gemm_static: the allocation-free entry point --------------------------------------------------------------------------
+// Scratch of heal_gemm_static (include/heal.h): [0, 256) the kernels' diagnostic words, then the hi and lo FP16 planes of the
+// activations.  File-scope device memory: every GPU that loads the library holds these 8 MiB + 256 B until the process exits.  In
+// host code the NAME of the array is only a stand-in for the symbol; the device address comes from cudaGetSymbolAddress, taken
+// once per device with that device current (static_scratch()).  Zero-initialised at module load, which is all the diagnostic words
+// need; the planes are rewritten by step S of every call (rows >= M and columns >= K are never read: the tensor maps end at M and K).
+constexpr size_t kStaticDiagBytes = 256;
+constexpr size_t kStaticScratchBytes = HEAL_STATIC_SCRATCH_BYTES;
+static __device__ __align__(256) unsigned char g_static_scratch[kStaticDiagBytes + kStaticScratchBytes];
+
+int static_scratch(unsigned char **out)
+{
+    constexpr int kMaxDev = 64;
+    static std::mutex mu;
+    static unsigned char *ptrs[kMaxDev] = {};
+    int dev = -1;
+    HEAL_CUDA(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= kMaxDev) return HEAL_ERR_UNSUPPORTED_DEVICE;
+    std::lock_guard<std::mutex> lk(mu);
+    if (!ptrs[dev]) {
+        void *p = nullptr;
+        HEAL_CUDA(cudaGetSymbolAddress(&p, g_static_scratch));
+        if (!p) return HEAL_ERR_CUDA;
+        ptrs[dev] = static_cast<unsigned char *>(p);
+    }
+    *out = ptrs[dev];
+    return HEAL_OK;
+}
+
+// ensure_init() without its cudaMalloc: if the library has not been initialised yet, the diagnostic words live in the static array
+int ensure_init_static(unsigned char *scratch)
+{
+    {
+        std::lock_guard<std::mutex> lk(g_mu);
+        if (!g.init) {
+            g.init = true;
+            auto fail = [&](int st) { g.init_status = st; return st; };
+            int dev = 0;
+            cudaError_t e = cudaGetDevice(&dev);
+            if (e != cudaSuccess) return fail(cuda_fail(e));
+            cudaDeviceProp prop;
+            e = cudaGetDeviceProperties(&prop, dev);
+            if (e != cudaSuccess) return fail(cuda_fail(e));
+            if (prop.major != 10) return fail(HEAL_ERR_UNSUPPORTED_DEVICE);
+            g.device = dev;
+            g.num_sms = prop.multiProcessorCount;
+            void *fn = nullptr;
+            cudaDriverEntryPointQueryResult qres;
+            e = cudaGetDriverEntryPointByVersion("cuTensorMapEncodeTiled", &fn, 12000, cudaEnableDefault, &qres);
+            if (e != cudaSuccess || qres != cudaDriverEntryPointSuccess || !fn)
+                return fail(cuda_fail(e != cudaSuccess ? e : cudaErrorUnknown));
+            g.encode = reinterpret_cast<PFN_cuTensorMapEncodeTiled_v12000>(fn);
+            g.diag = reinterpret_cast<int *>(scratch);
+            return HEAL_OK;
+        }
+    }
+    return ensure_init();                  // already initialised: only the status / device check
+}
+
 }  // namespace
 
 // =============================================== C ABI ===========================================
@@ -1415,6 +1474,53 @@ int heal_gemm(int64_t M, int64_t N, int64_t K, const void *A, int64_t lda, const
               int64_t ldc, uint32_t mode, void *stream_)
 {
     return heal_gemm_ex(M, N, K, A, lda, B, ldb, C, ldc, nullptr, nullptr, 0, 0, mode, stream_);
+}
+
+int heal_gemm_static(int64_t M, int64_t N, int64_t K, const void *A, int64_t lda, const void *B, int64_t ldb, void *C,
+                     int64_t ldc, uint32_t mode, void *stream_)
+{
+    int nprod;
+    bool b_nk;
+    int st = validate_mode(mode, &nprod, &b_nk);
+    if (st) return st;
+    if (nprod > 2 || (mode & ~(HEAL_MODE_PRODUCTS_MASK | HEAL_B_NK | HEAL_B_STATIC))) return HEAL_ERR_UNSUPPORTED_MODE;
+    if (M < 0 || N < 0 || K < 0) return HEAL_ERR_INVALID_VALUE;
+    if (N > 0x7fffff00 || K > 0x7fffff00) return HEAL_ERR_INVALID_VALUE;
+    if (lda < K || ldb < (b_nk ? K : N) || ldc < N) return HEAL_ERR_INVALID_VALUE;
+    if (M > HEAL_STATIC_MAX_M) return HEAL_ERR_WORKSPACE;                        // the decode kernel's range
+    const int64_t lda_p = round_up(K > 0 ? K : 1, 8);
+    const size_t a_plane = static_cast<size_t>(round_up(M * lda_p * 2, 256));
+    if (2 * a_plane > kStaticScratchBytes) return HEAL_ERR_WORKSPACE;            // the planes do not fit the static scratch
+    if (M == 0 || N == 0) return HEAL_OK;
+    if (!C) return HEAL_ERR_NULL_POINTER;
+    if (!aligned16(C) || (ldc & 3)) return HEAL_ERR_MISALIGNED;
+    if (K > 0) {
+        if (!A || !B) return HEAL_ERR_NULL_POINTER;
+        if (!aligned16(A) || !aligned16(B) || (lda & 3) || (ldb & 7)) return HEAL_ERR_MISALIGNED;
+    }
+    unsigned char *scratch = nullptr;
+    st = static_scratch(&scratch);
+    if (st) return st;
+    st = ensure_init_static(scratch);
+    if (st) return st;
+    cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+    heal::OutArgs out = {};
+    out.C = static_cast<float *>(C);
+    out.ldc = ldc;
+    out.scale = 1.0f;
+    const bool b_static = (mode & HEAL_B_STATIC) != 0;
+    if (K == 0) return presplit_impl(M, N, K, nullptr, nullptr, lda, nullptr, nullptr, ldb, out, nprod, b_nk, b_static, stream);
+    __half *a_hi = reinterpret_cast<__half *>(scratch + kStaticDiagBytes);
+    __half *a_lo = reinterpret_cast<__half *>(scratch + kStaticDiagBytes + a_plane);
+    st = launch_split(M, K, static_cast<const float *>(A), lda, a_hi, a_lo, lda_p, stream);      // step S into the static planes
+    if (st) return st;
+    // steps G + E: the small-M kernel only (it needs no further scratch; the large-M kernels' schedules may allocate hand-off buffers)
+    bool handled = false;
+    const SmallIn in{a_hi, a_lo, lda_p, nullptr, 0, b_static};
+    st = b_nk ? launch_small<false>(nprod, M, N, K, in, B, nullptr, ldb, out, stream, &handled)
+              : launch_small<true>(nprod, M, N, K, in, B, nullptr, ldb, out, stream, &handled);
+    if (st) return st;
+    return handled ? HEAL_OK : HEAL_ERR_WORKSPACE;         // (K beyond what 512 TMEM columns and a cluster of 8 hold at this M)
 }
 
 int heal_gemm_host(int64_t M, int64_t N, int64_t K, const void *A_host, int64_t lda, const void *B_host, int64_t ldb,
