@@ -843,22 +843,37 @@ int launch_small_cfg(int64_t M, int64_t N, int64_t K, const SmallIn &in, const v
     while (!(cs == 1 && !Cfg::FUSED) && ((n_seg + cs - 1) / cs) * Cfg::MPAD > 512 && cs * 2 <= 8 && cs * 2 <= n_seg) cs *= 2;
     Plan pl = plan(cs, false, false);
     if (pl.status) return HEAL_OK;                              // leave to the large-M kernel
+    // More than 16 tokens (few tokens: the rule above, which also keeps the pushes st.async): among the cluster sizes from cs/2 + 1
+    // that still give about 1.2 CTAs per SM and whose grid is resident, take the one with the fewest segments on its longest rank,
+    // the smallest on a tie -- K = 5120 has 10 segments: 5 ranks of 2 instead of 8 ranks of 2 or 1 (measured, planes:
+    // 24 x 5120 x 5120 19.2 -> 17.0 us, 64 x 5120 x 5120 25.2 -> 21.3 us, 32 x 7168 x 5120 22.2 -> 20.4 us with 5 ranks instead of 4).
+    static const bool no_wave_fit = std::getenv("HEAL_NO_WAVE_CAP") != nullptr;      // debug only
+    // All CTAs of the grid should be resident at once: a small second wave pays a whole first-tile latency and streams on a
+    // fraction of the SMs (measured: 32 x 6144 x 4096, 384 CTAs of 88 KB, 19.1 us with 88 CTAs in a second wave, 13.7 us in one).
+    // If the plan does not fit: two pipeline stages, then the partial sums overlaid on the pipeline, then both.
+    if (!pl.fits() && cs > 1 && !forced_cs && !no_wave_fit) {
+        for (int opt = 1; opt < 4; ++opt) {
+            const Plan q = plan(cs, (opt & 1) != 0, (opt & 2) != 0);
+            if (q.status == 0 && q.fits()) { pl = q; break; }
+        }
+    }
+    if (!Cfg::PAIR && !forced_cs && M > 16 && cs > 1) {
+        Plan best = pl;
+        for (int c = cs / 2 + 1; c <= 8 && c <= n_seg; ++c) {
+            if (c == cs || panels * c * 5 < 6 * static_cast<int64_t>(g.num_sms)) continue;
+            const Plan q = plan(c, false, false);
+            if (q.status == 0 && q.fits() && (q.cost() < best.cost() || (q.cost() == best.cost() && (!best.fits() || q.cs < best.cs)))) best = q;
+        }
+        pl = best;
+    }
     // fused split with more than 16 tokens: the converter warps only keep up while at most two CTAs share an SM; past that the
     // caller splits first and comes back with planes (measured, M = 32: 5120 x 5120 32.2 fused vs 19.5 us, 6144 x 4096 21.1 vs 15.6 us)
     if (Cfg::FUSED && M > 16 && pl.grid > 2 * static_cast<int64_t>(g.num_sms) && !forced_cs) return HEAL_OK;
-    // All CTAs of the grid should be resident at once: a small second wave pays a whole first-tile latency and streams on a
-    // fraction of the SMs (measured: 32 x 6144 x 4096, 384 CTAs of 88 KB, 19.1 us with 88 CTAs in a second wave, 13.7 us in one).
-    // If the plan does not fit: two pipeline stages, then the partial sums overlaid on the pipeline, then both; failing that, the
-    // cluster size (and options) with the fewest waves x segments per CTA, the smallest such cluster first (measured:
-    // 24 x 5120 x 17408 90 -> 40 us with clusters of 6 instead of 8, 64 x 10240 x 8192 80 -> 53 us, 32 x 8192 x 28672 138 -> 99 us).
-    static const bool no_wave_fit = std::getenv("HEAL_NO_WAVE_CAP") != nullptr;      // debug only
+    // Still not resident: the cluster size (and options) with the fewest waves x segments per CTA, the smallest such cluster first
+    // (measured: 24 x 5120 x 17408 90 -> 40 us with clusters of 6 instead of 8, 64 x 10240 x 8192 80 -> 53 us,
+    // 32 x 8192 x 28672 138 -> 99 us).
     if (!pl.fits() && cs > 1 && !forced_cs && !no_wave_fit) {
-        bool found = false;
-        for (int opt = 1; opt < 4 && !found; ++opt) {
-            const Plan q = plan(cs, (opt & 1) != 0, (opt & 2) != 0);
-            if (q.status == 0 && q.fits()) { pl = q; found = true; }
-        }
-        for (int c = 1; c <= 8 && !found; ++c) {
+        for (int c = 1; c <= 8; ++c) {
             if (c > n_seg || c == cs) continue;
             for (int opt = 0; opt < 4; ++opt) {
                 const Plan q = plan(c, (opt & 1) != 0, (opt & 2) != 0);
