@@ -881,6 +881,33 @@ def test_small_m_cluster_grid_never_oversubscribes_tmem(hb, inputs, M, N, K):
     assert all(torch.equal(o, ref) for o in outs)
 
 
+@pytest.mark.parametrize("M,N,K", [(24, 5120, 5120), (64, 5120, 5120), (32, 7168, 5120), (24, 5120, 17408), (64, 10240, 8192),
+                                   (32, 8192, 28672), (32, 6144, 4096), (64, 6144, 4096), (40, 6152, 4096 + 72), (64, 8192, 8192)])
+def test_small_m_launch_plans_bit_identical(hb, M, N, K):
+    """Shapes whose small-M launch plan is not the plain one (heal_api.cu launch_small_cfg): clusters of 5, 6 or 3 ranks chosen for
+    balance or residency, two pipeline stages, partial sums overlaid on the pipeline, grids of several waves.  The plan is a pure
+    performance choice: bit-identical to the large-M kernels (themselves checked against the oracle), planes and fused-split entry."""
+    gen = torch.Generator(device="cuda")
+    gen.manual_seed(M * 131 + N + K)
+    A = torch.randn(M, K, device="cuda", generator=gen)
+    A[:, 7] *= 50.0
+    W = (torch.randn(K, N, device="cuda", generator=gen) * 0.02).half()
+    ah, al = hb.heal_split(A)
+    try:
+        hb.debug_force_kernel(1)
+        ref = hb.heal_gemm_presplit(ah, al, W, None, 2).clone()
+        assert "smallm" not in hb.last_kernel()
+    finally:
+        hb.debug_force_kernel(0)
+    got = hb.heal_gemm_presplit(ah, al, W, None, 2)
+    assert "smallm" in hb.last_kernel()
+    assert torch.equal(got, ref)
+    assert torch.equal(hb.heal_gemm(A, W, 2), ref)
+    assert torch.equal(hb.heal_gemm(A, W, 2 | hb.B_STATIC), ref)
+    assert torch.equal(hb.heal_gemm_presplit(ah, al, W.t().contiguous(), None, 2 | hb.B_NK), ref)
+    torch.cuda.synchronize()
+
+
 def test_graph_survives_workspace_growth(hb, inputs):
     """Warm up and capture a small problem, then run a larger one eagerly on the same stream (the library-owned hi/lo
     plane workspace and the split-K partial area have to grow), then replay the graph: the buffers baked into the graph
