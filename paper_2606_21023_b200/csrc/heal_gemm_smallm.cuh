@@ -575,40 +575,38 @@ heal_gemm_smallm_kernel(const __grid_constant__ CUtensorMap tm_x_hi, const __gri
                         tmem_ld_32x32b_x16(tmem_base + (static_cast<uint32_t>(quad * 32) << 16) + static_cast<uint32_t>(j * MPAD + c * 16), v);
                         tmem_ld_wait();
                         const bool async = args.red_async != 0;
-                        // owner rank and row inside its block of the first token of this chunk, then stepped along
-                        // (one division per chunk instead of one per element of the unrolled loops)
-                        uint32_t dst = static_cast<uint32_t>((c * 16) / rpr), ml = static_cast<uint32_t>((c * 16) % rpr);
-                        auto step = [&](uint32_t n) {
-                            ml += n;
-                            while (ml >= static_cast<uint32_t>(rpr)) { ml -= static_cast<uint32_t>(rpr); ++dst; }
-                        };
+                        // rows_per_rank is 1, 2 or a multiple of 4 (host): the owner rank and the row inside its block follow from
+                        // shifts, or are stepped along from one division per chunk.  The loops stop at the last token: this code runs once,
+                        // on the latency-critical tail, with one warp per scheduler -- 16 predicated-off iterations with a division-free
+                        // but branchy step cost 1100 cycles per segment at M = 1 (clock stamps), the same loop cut at M costs 100.
                         if ((rpr & 3) == 0) {
+                            uint32_t dst = static_cast<uint32_t>((c * 16) / rpr), ml = static_cast<uint32_t>((c * 16) % rpr);
 #pragma unroll
                             for (int i = 0; i < 16; i += 4) {
-                                if (c * 16 + i < Mr) {    // rpr % 4 == 0: rows m..m+3 have one owner (rows >= M: unused zeros)
-                                    // groups of four rows are the slow index: a warp's vector stores land on 512 contiguous bytes
-                                    const uint32_t a = map_to_cta(red_base + ((static_cast<uint32_t>(seg * (rpr >> 2)) + (ml >> 2)) * kSmallBNW + nl) * 16u, dst);
-                                    if (async) st_async_v4(a, v[i], v[i + 1], v[i + 2], v[i + 3], map_to_cta(red_bar, dst));
-                                    else       st_dsmem_v4(a, v[i], v[i + 1], v[i + 2], v[i + 3]);
-                                }
-                                step(4);
+                                if (c * 16 + i >= Mr) break;      // rows m..m+3 have one owner (rows >= M: unused zeros)
+                                // groups of four rows are the slow index: a warp's vector stores land on 512 contiguous bytes
+                                const uint32_t a = map_to_cta(red_base + ((static_cast<uint32_t>(seg * (rpr >> 2)) + (ml >> 2)) * kSmallBNW + nl) * 16u, dst);
+                                if (async) st_async_v4(a, v[i], v[i + 1], v[i + 2], v[i + 3], map_to_cta(red_bar, dst));
+                                else       st_dsmem_v4(a, v[i], v[i + 1], v[i + 2], v[i + 3]);
+                                ml += 4;
+                                if (ml == static_cast<uint32_t>(rpr)) { ml = 0; ++dst; }
                             }
-                        } else if ((rpr & 1) == 0 && async) {
+                        } else if (rpr == 2 && async) {
 #pragma unroll
                             for (int i = 0; i < 16; i += 2) {
-                                if (c * 16 + i < Mr)
-                                    st_async_v2(map_to_cta(red_base + row_off + ml * 4u, dst), v[i], v[i + 1], map_to_cta(red_bar, dst));
-                                step(2);
+                                if (c * 16 + i >= Mr) break;
+                                const uint32_t dst = static_cast<uint32_t>(c * 16 + i) >> 1;
+                                st_async_v2(map_to_cta(red_base + row_off, dst), v[i], v[i + 1], map_to_cta(red_bar, dst));
                             }
-                        } else {
+                        } else {                                  // one row per rank (or two, plain stores)
+                            const uint32_t sh = static_cast<uint32_t>(rpr) - 1u;            // 0 or 1
 #pragma unroll
                             for (int i = 0; i < 16; ++i) {
-                                if (c * 16 + i < Mr) {
-                                    const uint32_t a = map_to_cta(red_base + row_off + ml * 4u, dst);
-                                    if (async) st_async_b32(a, v[i], map_to_cta(red_bar, dst));
-                                    else       st_dsmem_b32(a, v[i]);
-                                }
-                                step(1);
+                                if (c * 16 + i >= Mr) break;
+                                const uint32_t m = static_cast<uint32_t>(c * 16 + i), dst = m >> sh, ml = m & sh;
+                                const uint32_t a = map_to_cta(red_base + row_off + ml * 4u, dst);
+                                if (async) st_async_b32(a, v[i], map_to_cta(red_bar, dst));
+                                else       st_dsmem_b32(a, v[i]);
                             }
                         }
                     }
