@@ -866,6 +866,11 @@ int launch_small_cfg(int64_t M, int64_t N, int64_t K, const SmallIn &in, const v
         }
         pl = best;
     }
+    // fused split on one CTA per panel (large N: every CTA walks the whole of K): the per-k-tile hand-over between the converter warps
+    // and the MMA thread costs more over 64+ k-tiles than the split launch it saves (measured, M = 1 / 16: 28672 x 4096 41.0 / 43.9 us
+    // fused vs 38.0 / 38.4 us on planes, LM head 175 / 186 vs 170 / 175 us, 65536 x 5120 110 / 116 vs 107 / 110 us)
+    static const bool fused_long = std::getenv("HEAL_FUSED_LONG") != nullptr;      // debug only
+    if (Cfg::FUSED && pl.cs == 1 && n_seg >= 4 && !forced_cs && !fused_long) return HEAL_OK;
     // fused split with more than 16 tokens: the converter warps only keep up while at most two CTAs share an SM; past that the
     // caller splits first and comes back with planes (measured, M = 32: 5120 x 5120 32.2 fused vs 19.5 us, 6144 x 4096 21.1 vs 15.6 us)
     if (Cfg::FUSED && M > 16 && pl.grid > 2 * static_cast<int64_t>(g.num_sms) && !forced_cs) return HEAL_OK;
