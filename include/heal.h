@@ -112,7 +112,8 @@ typedef enum {
  * then split inside the GEMM kernel.  Buffers that a captured graph may hold are never freed or handed to another stream.
  * With FP16 weights and decode-sized M (M <= 16 with K <= 16384; M <= 32 for problems of up to 32 Mi weights) the split
  * runs inside the GEMM kernel -- one launch, no workspace -- wherever that is the faster form: not for very wide weight
- * matrices (N of about 26 500 columns or more with K >= 2048, e.g. the LM head), which take split + GEMM on planes like larger M.
+ * matrices (N of about 26 500 columns or more with K >= 2048, e.g. the LM head), which take split + GEMM on planes like larger M
+ * (unless the call is being captured on a stream without a workspace: then the fused kernel, not HEAL_ERR_WORKSPACE).
  * Numerical contract: finite inputs with |x| <= 65504 (activations observed
  * < 1024); anything larger, Inf or NaN propagates to Inf/NaN in the affected rows/columns.
  */

@@ -699,6 +699,7 @@ struct SmallIn {
     const float *A32;
     int64_t lda32;
     bool b_static;
+    bool fused_any = false;    // FUSED: take the fused kernel also where planes would be faster (the caller cannot have planes)
 };
 
 // st.async pushes (lowest latency) pay off while a thread sends few values: up to 8 of any width, or up to 32 8-byte
@@ -870,10 +871,10 @@ int launch_small_cfg(int64_t M, int64_t N, int64_t K, const SmallIn &in, const v
     // and the MMA thread costs more over 64+ k-tiles than the split launch it saves (measured, M = 1 / 16: 28672 x 4096 41.0 / 43.9 us
     // fused vs 38.0 / 38.4 us on planes, LM head 175 / 186 vs 170 / 175 us, 65536 x 5120 110 / 116 vs 107 / 110 us)
     static const bool fused_long = std::getenv("HEAL_FUSED_LONG") != nullptr;      // debug only
-    if (Cfg::FUSED && pl.cs == 1 && n_seg >= 4 && !forced_cs && !fused_long) return HEAL_OK;
+    if (Cfg::FUSED && pl.cs == 1 && n_seg >= 4 && !forced_cs && !fused_long && !in.fused_any) return HEAL_OK;
     // fused split with more than 16 tokens: the converter warps only keep up while at most two CTAs share an SM; past that the
     // caller splits first and comes back with planes (measured, M = 32: 5120 x 5120 32.2 fused vs 19.5 us, 6144 x 4096 21.1 vs 15.6 us)
-    if (Cfg::FUSED && M > 16 && pl.grid > 2 * static_cast<int64_t>(g.num_sms) && !forced_cs) return HEAL_OK;
+    if (Cfg::FUSED && M > 16 && pl.grid > 2 * static_cast<int64_t>(g.num_sms) && !forced_cs && !in.fused_any) return HEAL_OK;
     // Still not resident: the cluster size (and options) with the fewest waves x segments per CTA, the smallest such cluster first
     // (measured: 24 x 5120 x 17408 90 -> 40 us with clusters of 6 instead of 8, 64 x 10240 x 8192 80 -> 53 us,
     // 32 x 8192 x 28672 138 -> 99 us).
@@ -1051,7 +1052,7 @@ int validate_mode(uint32_t mode, int *nprod, bool *b_nk)
 // A32 != nullptr: FP32 activations for the fused small-M kernel (M <= 64, FP16 weights) instead of planes
 int presplit_impl(int64_t M, int64_t N, int64_t K, const void *A_hi, const void *A_lo, int64_t lda, const void *B_hi,
                   const void *B_lo, int64_t ldb, const OutArgs &out, int nprod, bool b_nk, bool b_static,
-                  cudaStream_t stream, const float *A32 = nullptr, int64_t lda32 = 0, bool *handled_out = nullptr)
+                  cudaStream_t stream, const float *A32 = nullptr, int64_t lda32 = 0, bool *handled_out = nullptr, bool fused_any = false)
 {
     if (handled_out) *handled_out = true;
     if (K == 0) {                                       // empty sum: zeros in every requested output (SiLU(0) * 0 = 0 as well)
@@ -1075,7 +1076,7 @@ int presplit_impl(int64_t M, int64_t N, int64_t K, const void *A_hi, const void 
     const int64_t small_max = nprod == kScaledLo && force != 2 ? 32 : 64;
     if (M <= small_max && force != 1) {
         bool handled = false;
-        const SmallIn in{A_hi, A_lo, lda, A32, lda32, b_static};
+        const SmallIn in{A_hi, A_lo, lda, A32, lda32, b_static, fused_any};
         int st = b_nk ? launch_small<false>(nprod, M, N, K, in, B_hi, B_lo, ldb, out, stream, &handled)
                       : launch_small<true>(nprod, M, N, K, in, B_hi, B_lo, ldb, out, stream, &handled);
         if (st || handled) return st;
@@ -1428,6 +1429,16 @@ int heal_gemm_ex(int64_t M, int64_t N, int64_t K, const void *A, int64_t lda, co
         st = presplit_impl(M, N, K, nullptr, nullptr, 0, B, nullptr, ldb, out, nprod, b_nk, b_static, stream,
                            static_cast<const float *>(A), lda, &handled);
         if (st || handled) return st;
+        // left to split + planes because that is faster -- but a captured call on a stream without a workspace cannot have planes:
+        // the fused kernel then, rather than HEAL_ERR_WORKSPACE
+        if (stream_capturing(stream)) {
+            void *probe = nullptr;
+            if (get_ws(plan_ws(M, N, K, nprod, b_nk).total, stream, &probe) == HEAL_ERR_WORKSPACE) {
+                st = presplit_impl(M, N, K, nullptr, nullptr, 0, B, nullptr, ldb, out, nprod, b_nk, b_static, stream,
+                                   static_cast<const float *>(A), lda, &handled, true);
+                if (st || handled) return st;
+            }
+        }
     }
 
     // Prefill shapes served by the CTA-pair kernel (M > 128, N > 128), two or three products: step S of the activations can run

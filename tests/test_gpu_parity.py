@@ -416,6 +416,30 @@ def test_captured_call_without_workspace_uses_fused_split(hb, inputs):
             assert torch.equal(C, ref)
 
 
+def test_captured_decode_call_on_wide_weights_without_workspace(hb):
+    """Decode-sized M on very wide weights normally takes split + planes (faster there); captured on a stream the library has never
+    seen, with no workspace to put planes in, it takes the fused-split kernel instead of failing.  Same bits either way."""
+    gen = torch.Generator(device="cuda")
+    gen.manual_seed(5)
+    A = torch.randn(4, 2048, device="cuda", generator=gen)
+    W = (torch.randn(2048, 28672, device="cuda", generator=gen) * 0.02).half()
+    ref = hb.heal_gemm(A, W, 2).clone()
+    assert "fused" not in hb.last_kernel()
+    C = torch.zeros_like(ref)
+    s = torch.cuda.Stream()
+    torch.cuda.synchronize()
+    with torch.cuda.stream(s):
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=s):
+            hb.heal_gemm(A, W, 2, C=C)
+        assert "fused split" in hb.last_kernel()
+        for _ in range(2):
+            C.zero_()
+            g.replay()
+            s.synchronize()
+            assert torch.equal(C, ref)
+
+
 @pytest.mark.parametrize("M,N,K,b_nk", [(1, 4096, 4096, False), (8, 1032, 4096, False), (16, 520, 8192, False), (13, 264, 1000, True),
                                         (5, 4096, 520, True), (16, 128, 8192, False)])
 def test_fused_split_small_m_bit_identical(hb, oracle, inputs, M, N, K, b_nk):
