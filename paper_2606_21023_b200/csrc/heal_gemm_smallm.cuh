@@ -462,7 +462,7 @@ heal_gemm_smallm_kernel(const __grid_constant__ CUtensorMap tm_x_hi, const __gri
                                     asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(sx + Cfg::X_TILE_AL + off), "r"(l.x), "r"(l.y), "r"(l.z), "r"(l.w) : "memory");
                             }
                         }
-                        fence_proxy_async_smem();           // generic-proxy writes -> visible to the tensor core
+                        if (r0 < args.M) fence_proxy_async_smem();   // generic-proxy writes -> visible to the tensor core (writers only)
                         __syncwarp();
                         if (lane == 0) mbar_arrive(xfull_bar(stage));
                         if (t + PF < n_t) fetch(t + PF, buf[p]);
