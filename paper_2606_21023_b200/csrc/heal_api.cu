@@ -705,6 +705,18 @@ struct SmallIn {
 // st.async pushes (lowest latency) pay off while a thread sends few values: up to 8 of any width, or up to 32 8-byte
 // vectors (the plain path has no 8-byte form and falls back to 4-byte remote stores, which are slow; measured: M = 16,
 // K = 6144 21.7 -> 15.7 us, K = 14336 36.9 -> 26.9 us).
+// Token rows finished by one rank of a cluster of c.  A remote store costs about 300 cycles whatever its width (st.async, one warp per
+// scheduler: clock stamps), so the rows are dealt in the widest vectors the token count allows: blocks of 4 rows from 3 tokens on
+// (16-byte pushes; fewer ranks then own rows), 2 rows for 2 tokens.  Measured: 16 x 4096 x 4096 10.5 -> 9.9 us with 4 pushes of 16
+// bytes instead of 8 of 8, M = 24 decode 16.5 us with 4-byte pushes vs 9.9 us at M = 32.
+inline int64_t rows_per_rank(int64_t M, int64_t c)
+{
+    if (c <= 1) return 0;
+    const int64_t r = (M + c - 1) / c;
+    if (M >= 3) return (r + 3) / 4 * 4;
+    return M == 2 ? 2 : r;
+}
+
 inline bool async_push_ok(int64_t pushes, int64_t vw)
 {
     static const long lim = std::getenv("HEAL_ASYNC_MAX") ? std::atol(std::getenv("HEAL_ASYNC_MAX")) : 8;      // tuning
@@ -729,8 +741,7 @@ int launch_small_cfg(int64_t M, int64_t N, int64_t K, const SmallIn &in, const v
     if (cs > 2 && M <= 16) {
         const int longest = (n_seg + cs - 1) / cs;
         for (int c = cs / 2 + 1; c < cs; ++c) {
-            int64_t r = (M + c - 1) / c;                                        // rows per rank (rounded as below), pushes per thread
-            if (r >= 3) r = (r + 3) / 4 * 4;
+            const int64_t r = rows_per_rank(M, c);                              // pushes per thread follow from it
             const int64_t vw = (r & 3) == 0 ? 4 : ((r & 1) == 0 ? 2 : 1);
             if ((n_seg + c - 1) / c == longest && panels * c * 5 >= 6 * g.num_sms && async_push_ok(longest * ((M + vw - 1) / vw), vw)) {
                 cs = c;                                                          // (only while the pushes stay st.async)
@@ -777,7 +788,7 @@ int launch_small_cfg(int64_t M, int64_t N, int64_t K, const SmallIn &in, const v
         int64_t cost() const { return (grid + slots - 1) / slots * max_local; }     // waves x segments per CTA
         bool fits() const { return grid <= slots; }
     };
-    auto plan = [&](int c, bool two_stages, bool force_alias) {
+    auto plan = [&](int c, bool two_stages, bool force_alias, bool never_alias = false) {
         Plan q = {};
         q.status = 1;
         q.cs = c;
@@ -796,10 +807,7 @@ int launch_small_cfg(int64_t M, int64_t N, int64_t K, const SmallIn &in, const v
         q.tmem_cols = 32;
         while (q.tmem_cols < (use_ring ? q.ring : q.max_local) * Cfg::MPAD) q.tmem_cols *= 2;
         if (q.tmem_cols > 512) return q;
-        // token rows finished by one rank; 3 or more are rounded up to a multiple of 4 so that the pushes are 16-byte vectors
-        // (fewer ranks then own rows; measured: M = 24 decode 16.5 us with 4-byte pushes vs 9.9 us at M = 32)
-        q.rpr = c > 1 ? static_cast<int>((M + c - 1) / c) : 0;
-        if (q.rpr >= 3) q.rpr = (q.rpr + 3) / 4 * 4;
+        q.rpr = static_cast<int>(rows_per_rank(M, c));
         q.red = c > 1 ? static_cast<size_t>(n_seg) * q.rpr * kSmallBNW * 4 : 0;
         // Shared memory.  Measured on B200 (decode 4096 x 4096, LM head): what matters is how many CTAs are resident
         // -- the next kernel's CTAs run their prologue (and with HEAL_B_STATIC prefetch W) beside this kernel's --
@@ -808,7 +816,7 @@ int launch_small_cfg(int64_t M, int64_t N, int64_t K, const SmallIn &in, const v
         // has k-tiles.
         // Partial sums pushed by the cluster: a dedicated area when small (decode), else overlaid on the pipeline.
         static const size_t alias_min = std::getenv("HEAL_RED_ALIAS_MIN") ? static_cast<size_t>(std::atol(std::getenv("HEAL_RED_ALIAS_MIN"))) : 16 * 1024;   // debug only
-        q.red_alias = q.red > alias_min || (force_alias && q.red > 0);
+        q.red_alias = !never_alias && (q.red > alias_min || (force_alias && q.red > 0));
         const size_t fixed = (q.red_alias ? 0 : q.red) + Cfg::BAR_BYTES;          // no alignment slack: see the kernel
         size_t budget = q.tmem_cols > 256 ? static_cast<size_t>(kSmemLimit)
                         : (Cfg::STAGE_BYTES <= 24 * 1024 && c > 1 ? static_cast<size_t>(74 * 1024) : static_cast<size_t>(112 * 1024));
@@ -886,6 +894,15 @@ int launch_small_cfg(int64_t M, int64_t N, int64_t K, const SmallIn &in, const v
                 if (q.status == 0 && q.cost() < pl.cost()) pl = q;
             }
         }
+    }
+    // Partial sums overlaid on the pipeline cost a second cluster barrier -- nobody may push before every rank's main loop is over, so
+    // the pushes (about 300 cycles each) no longer overlap the wait for the slowest rank.  A dedicated area is better whenever the grid
+    // stays resident with at least three stages (measured: 8 x 8192 x 8192 27.3 -> 24.6 us, 16 x 8192 x 8192 28.9 -> 25.7 us,
+    // 2 x 4096 x 14336 27.0 -> 23.1 us; with two stages it is worse: 16 x 4096 x 14336 29.2 vs 38.9 us).
+    static const bool no_dedicated = std::getenv("HEAL_NO_DEDICATED_RED") != nullptr;      // debug only
+    if (pl.red_alias && pl.cs > 1 && M <= 16 && !no_dedicated) {       // (more tokens: the larger area costs residency -- measured worse)
+        const Plan q = plan(pl.cs, false, false, true);
+        if (q.status == 0 && q.fits() && q.stages >= 3 && !q.red_alias) pl = q;
     }
     static const bool plan_debug = std::getenv("HEAL_PLAN_DEBUG") != nullptr;      // debug only
     if (plan_debug)
