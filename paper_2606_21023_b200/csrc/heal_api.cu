@@ -709,11 +709,12 @@ struct SmallIn {
 // scheduler: clock stamps), so the rows are dealt in the widest vectors the token count allows: blocks of 4 rows from 3 tokens on
 // (16-byte pushes; fewer ranks then own rows), 2 rows for 2 tokens.  Measured: 16 x 4096 x 4096 10.5 -> 9.9 us with 4 pushes of 16
 // bytes instead of 8 of 8, M = 24 decode 16.5 us with 4-byte pushes vs 9.9 us at M = 32.
-inline int64_t rows_per_rank(int64_t M, int64_t c)
+// `narrow`: one or two rows per rank stay as they are (4- and 8-byte pushes, twice as many, but a quarter or half of the partial-sum area).
+inline int64_t rows_per_rank(int64_t M, int64_t c, bool narrow = false)
 {
     if (c <= 1) return 0;
     const int64_t r = (M + c - 1) / c;
-    if (M >= 3) return (r + 3) / 4 * 4;
+    if (r >= 3 || (M >= 3 && !narrow)) return (r + 3) / 4 * 4;
     return M == 2 ? 2 : r;
 }
 
@@ -788,7 +789,7 @@ int launch_small_cfg(int64_t M, int64_t N, int64_t K, const SmallIn &in, const v
         int64_t cost() const { return (grid + slots - 1) / slots * max_local; }     // waves x segments per CTA
         bool fits() const { return grid <= slots; }
     };
-    auto plan = [&](int c, bool two_stages, bool force_alias, bool never_alias = false) {
+    auto plan = [&](int c, bool two_stages, bool force_alias, bool never_alias = false, bool narrow = false) {
         Plan q = {};
         q.status = 1;
         q.cs = c;
@@ -807,7 +808,7 @@ int launch_small_cfg(int64_t M, int64_t N, int64_t K, const SmallIn &in, const v
         q.tmem_cols = 32;
         while (q.tmem_cols < (use_ring ? q.ring : q.max_local) * Cfg::MPAD) q.tmem_cols *= 2;
         if (q.tmem_cols > 512) return q;
-        q.rpr = static_cast<int>(rows_per_rank(M, c));
+        q.rpr = static_cast<int>(rows_per_rank(M, c, narrow));
         q.red = c > 1 ? static_cast<size_t>(n_seg) * q.rpr * kSmallBNW * 4 : 0;
         // Shared memory.  Measured on B200 (decode 4096 x 4096, LM head): what matters is how many CTAs are resident
         // -- the next kernel's CTAs run their prologue (and with HEAL_B_STATIC prefetch W) beside this kernel's --
@@ -901,8 +902,10 @@ int launch_small_cfg(int64_t M, int64_t N, int64_t K, const SmallIn &in, const v
     // 2 x 4096 x 14336 27.0 -> 23.1 us; with two stages it is worse: 16 x 4096 x 14336 29.2 vs 38.9 us).
     static const bool no_dedicated = std::getenv("HEAL_NO_DEDICATED_RED") != nullptr;      // debug only
     if (pl.red_alias && pl.cs > 1 && M <= 16 && !no_dedicated) {       // (more tokens: the larger area costs residency -- measured worse)
-        const Plan q = plan(pl.cs, false, false, true);
-        if (q.status == 0 && q.fits() && q.stages >= 3 && !q.red_alias) pl = q;
+        for (int narrow = 0; narrow < 2; ++narrow) {       // (narrow rows: 8 x 4096 x 14336 28.0 us overlaid -> 25.3 us dedicated with 8-byte pushes)
+            const Plan q = plan(pl.cs, false, false, true, narrow != 0);
+            if (q.status == 0 && q.fits() && q.stages >= 3 && !q.red_alias) { pl = q; break; }
+        }
     }
     static const bool plan_debug = std::getenv("HEAL_PLAN_DEBUG") != nullptr;      // debug only
     if (plan_debug)
