@@ -901,7 +901,8 @@ int launch_small_cfg(int64_t M, int64_t N, int64_t K, const SmallIn &in, const v
     // stays resident with at least three stages (measured: 8 x 8192 x 8192 27.3 -> 24.6 us, 16 x 8192 x 8192 28.9 -> 25.7 us,
     // 2 x 4096 x 14336 27.0 -> 23.1 us; with two stages it is worse: 16 x 4096 x 14336 29.2 vs 38.9 us).
     static const bool no_dedicated = std::getenv("HEAL_NO_DEDICATED_RED") != nullptr;      // debug only
-    if (pl.red_alias && pl.cs > 1 && M <= 16 && !no_dedicated) {       // (more tokens: the larger area costs residency -- measured worse)
+    static const long dedicated_max_m = std::getenv("HEAL_DEDICATED_MAX_M") ? std::atol(std::getenv("HEAL_DEDICATED_MAX_M")) : 64;      // tuning
+    if (pl.red_alias && pl.cs > 1 && M <= dedicated_max_m && !no_dedicated) {       // (beyond 16 tokens it rarely fits: 24 x 6144 x 4096 16.3 -> 15.8 us)
         for (int narrow = 0; narrow < 2; ++narrow) {       // (narrow rows: 8 x 4096 x 14336 28.0 us overlaid -> 25.3 us dedicated with 8-byte pushes)
             const Plan q = plan(pl.cs, false, false, true, narrow != 0);
             if (q.status == 0 && q.fits() && q.stages >= 3 && !q.red_alias) { pl = q; break; }
