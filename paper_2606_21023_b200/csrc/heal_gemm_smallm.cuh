@@ -125,7 +125,7 @@ struct SmallArgs {
 };
 
 template <class Cfg>
-__global__ void __launch_bounds__(kSmallThreads)
+__global__ void __launch_bounds__(kSmallThreads, Cfg::MPAD >= 32 ? 3 : 0)
 heal_gemm_smallm_kernel(const __grid_constant__ CUtensorMap tm_x_hi, const __grid_constant__ CUtensorMap tm_x_lo,
                         const __grid_constant__ CUtensorMap tm_w_hi, const __grid_constant__ CUtensorMap tm_w_lo,
                         const SmallArgs args)
@@ -576,14 +576,16 @@ heal_gemm_smallm_kernel(const __grid_constant__ CUtensorMap tm_x_hi, const __gri
                         tmem_ld_wait();
                         const bool async = args.red_async != 0;
                         // rows_per_rank is 1, 2 or a multiple of 4 (host): the owner rank and the row inside its block follow from
-                        // shifts, or are stepped along from one division per chunk.  The loops stop at the last token: this code runs once,
-                        // on the latency-critical tail, with one warp per scheduler -- 16 predicated-off iterations with a division-free
-                        // but branchy step cost 1100 cycles per segment at M = 1 (clock stamps), the same loop cut at M costs 100.
+                        // shifts, or are stepped along from one division per chunk.  Past the last token the 16-token kernels leave the
+                        // loop; the 32- and 64-token ones skip the iteration (leaving costs them 30-70 registers, i.e. a CTA per SM).
+                        // This code runs once, on the latency-critical tail, with one warp per scheduler: 16 iterations that each stepped the
+                        // owner with a data-dependent loop cost 1100 cycles per segment at M = 1 (clock stamps), this form about 100.
+#define HEAL_PAST_LAST_TOKEN if constexpr (MPAD == 16) break; else continue
                         if ((rpr & 3) == 0) {
                             uint32_t dst = static_cast<uint32_t>((c * 16) / rpr), ml = static_cast<uint32_t>((c * 16) % rpr);
 #pragma unroll
                             for (int i = 0; i < 16; i += 4) {
-                                if (c * 16 + i >= Mr) break;      // rows m..m+3 have one owner (rows >= M: unused zeros)
+                                if (c * 16 + i >= Mr) { HEAL_PAST_LAST_TOKEN; }      // rows m..m+3 have one owner (rows >= M: unused zeros)
                                 // groups of four rows are the slow index: a warp's vector stores land on 512 contiguous bytes
                                 const uint32_t a = map_to_cta(red_base + ((static_cast<uint32_t>(seg * (rpr >> 2)) + (ml >> 2)) * kSmallBNW + nl) * 16u, dst);
                                 if (async) st_async_v4(a, v[i], v[i + 1], v[i + 2], v[i + 3], map_to_cta(red_bar, dst));
@@ -594,7 +596,7 @@ heal_gemm_smallm_kernel(const __grid_constant__ CUtensorMap tm_x_hi, const __gri
                         } else if (rpr == 2 && async) {
 #pragma unroll
                             for (int i = 0; i < 16; i += 2) {
-                                if (c * 16 + i >= Mr) break;
+                                if (c * 16 + i >= Mr) { HEAL_PAST_LAST_TOKEN; }
                                 const uint32_t dst = static_cast<uint32_t>(c * 16 + i) >> 1;
                                 st_async_v2(map_to_cta(red_base + row_off, dst), v[i], v[i + 1], map_to_cta(red_bar, dst));
                             }
@@ -602,7 +604,7 @@ heal_gemm_smallm_kernel(const __grid_constant__ CUtensorMap tm_x_hi, const __gri
                             const uint32_t sh = static_cast<uint32_t>(rpr) - 1u;            // 0 or 1
 #pragma unroll
                             for (int i = 0; i < 16; ++i) {
-                                if (c * 16 + i >= Mr) break;
+                                if (c * 16 + i >= Mr) { HEAL_PAST_LAST_TOKEN; }
                                 const uint32_t m = static_cast<uint32_t>(c * 16 + i), dst = m >> sh, ml = m & sh;
                                 const uint32_t a = map_to_cta(red_base + row_off + ml * 4u, dst);
                                 if (async) st_async_b32(a, v[i], map_to_cta(red_bar, dst));
@@ -612,6 +614,7 @@ heal_gemm_smallm_kernel(const __grid_constant__ CUtensorMap tm_x_hi, const __gri
                     }
                 }
             }
+#undef HEAL_PAST_LAST_TOKEN
             tc_fence_before();
             if (!args.red_async) {
                 __syncwarp();
