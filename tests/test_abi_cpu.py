@@ -78,3 +78,36 @@ def test_tile_schedule_covers_every_unit_once(tmp_path):
     out = subprocess.run([str(exe)], capture_output=True, text=True)
     assert out.returncode == 0, out.stdout[-2000:]
     assert ", 0 failures" in out.stdout
+
+
+def test_register_budgets_of_the_kernels(lib):
+    """Residency is part of the launch plans (heal_api.cu counts CTAs per SM): the small-M kernels must stay within three CTAs of
+    192 threads per SM (<= 112 registers), the large-M kernels within the whole register file of one CTA per SM, and nothing
+    may spill more than a few words.  cuobjdump reads the cubin; no GPU needed."""
+    import shutil
+    import subprocess
+    from paper_2606_21023_b200 import binding as hb
+    exe = shutil.which("cuobjdump") or "/usr/local/cuda/bin/cuobjdump"
+    if not os.path.exists(exe):
+        pytest.skip("cuobjdump not available")
+    out = subprocess.run([exe, "-res-usage", hb.LIB_PATH], capture_output=True, text=True).stdout
+    lines = out.splitlines()
+    seen = 0
+    for i, ln in enumerate(lines):
+        m = re.search(r"Function (\S+):", ln)
+        if not m or i + 1 >= len(lines):
+            continue
+        name = m.group(1)
+        r = re.search(r"REG:(\d+) STACK:(\d+)", lines[i + 1])
+        if not r:
+            continue
+        regs, stack = int(r.group(1)), int(r.group(2))
+        if "heal_gemm_smallm_kernel" in name:
+            seen += 1
+            assert regs <= 112, (name, regs)
+            assert stack <= 64, (name, stack)
+        elif "heal_gemm_umma2f_kernel" in name:
+            assert regs * 512 <= 65536, (name, regs)
+        elif "heal_gemm_umma2_kernel" in name or "heal_gemm_umma_kernel" in name:
+            assert regs * 384 <= 65536, (name, regs)
+    assert seen >= 40
