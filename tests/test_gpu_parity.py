@@ -906,10 +906,13 @@ def test_small_m_cluster_grid_never_oversubscribes_tmem(hb, inputs, M, N, K):
 
 
 @pytest.mark.parametrize("M,N,K", [(24, 5120, 5120), (64, 5120, 5120), (32, 7168, 5120), (24, 5120, 17408), (64, 10240, 8192),
-                                   (32, 8192, 28672), (32, 6144, 4096), (64, 6144, 4096), (40, 6152, 4096 + 72), (64, 8192, 8192)])
+                                   (32, 8192, 28672), (32, 6144, 4096), (64, 6144, 4096), (40, 6152, 4096 + 72), (64, 8192, 8192),
+                                   (2, 4096, 14336), (9, 4096, 14336), (13, 4096, 14336 + 72), (5, 1032, 14408), (3, 2056, 12800),
+                                   (16, 8192, 8192), (7, 7168, 5120), (12, 5120, 17408)])
 def test_small_m_launch_plans_bit_identical(hb, M, N, K):
     """Shapes whose small-M launch plan is not the plain one (heal_api.cu launch_small_cfg): clusters of 5, 6 or 3 ranks chosen for
-    balance or residency, two pipeline stages, partial sums overlaid on the pipeline, grids of several waves.  The plan is a pure
+    balance or residency, two pipeline stages, partial sums overlaid on the pipeline or in a dedicated area with one, two or four rows
+    per rank (odd token counts included), grids of several waves.  The plan is a pure
     performance choice: bit-identical to the large-M kernels (themselves checked against the oracle), planes and fused-split entry."""
     gen = torch.Generator(device="cuda")
     gen.manual_seed(M * 131 + N + K)
