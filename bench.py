@@ -260,14 +260,17 @@ def mlp_block_report(hb, M=2048):
 
 
 def small_m_report(hb, peaks):
-    """HBM-bound shapes of BASELINE.json configs[1] (decode 4096x4096, M = 1/8/32) and configs[4] (LM head, M = 1/64):
+    """HBM-bound shapes of BASELINE.json configs[1] (decode 4096x4096, M = 1/8/32) and configs[4] (LM head, M = 1/64), plus the
+    down and gate+up projections of a decoder layer at decode batch sizes:
     achieved GB/s = (2KN + 4MK + 4MN) / t through heal_gemm (device buffers; one fused kernel for decode-sized M), timed as a
     CUDA graph of back-to-back calls rotating over enough distinct weight copies to exceed the 126 MB L2; `eager_us` = the
     same calls issued one by one from the host (no graph): host-side launch cost included."""
     import torch
     out = {}
     for tag, M, N, K in [("decode_M1", 1, 4096, 4096), ("decode_M8", 8, 4096, 4096), ("decode_M32", 32, 4096, 4096),
-                         ("lm_head_M1", 1, 128256, 4096), ("lm_head_M64", 64, 128256, 4096)]:
+                         ("lm_head_M1", 1, 128256, 4096), ("lm_head_M64", 64, 128256, 4096),
+                         # (context beyond BASELINE.json: the two large decode GEMMs of a Llama-3-8B layer)
+                         ("layer_down_M8", 8, 4096, 14336), ("layer_gate_up_M1", 1, 28672, 4096)]:
         gen = torch.Generator(device="cuda")
         gen.manual_seed(7)
         ncopies = max(2, min(12, int(3 * L2_BYTES // (K * N * 2)) + 1))
