@@ -439,7 +439,8 @@ def run_ours(args):
                          "frac_of_nominal_2250": achieved / 2250.0, "frac_of_measured_burst": achieved / peaks["burst"],
                          "frac_of_measured_sustained": achieved / peaks["sustained"], "avg_launch_ms": ms_gemm,
                          "flops_per_launch": flop_launch,
-                         "limiter": {"what": "L2 -> SM operand delivery (48 KB per CTA and k-tile; tensor pipe ~80 % active in ncu)",
+                         "limiter": {"what": "operand movement per MMA: the SM's shared-memory port (48 KB of TMA writes + 96 KB of tcgen05.mma operand reads per CTA and "
+                                             "1024-cycle k-tile) ahead of the L2 -> SM fabric; tensor pipe ~80 % active in ncu",
                                      "achieved_GBps_per_sm": delivery, "probe_peak_GBps_per_sm": 69.4,
                                      "source": "profiles/probes_r01.md, DESIGN.md section 7"}},
             "e2e": {"value": world * FLOP_STEP / (ms_e2e * 1e-3) / 1e12, "unit": UNIT, "h2d_bytes_per_step": h2d,
