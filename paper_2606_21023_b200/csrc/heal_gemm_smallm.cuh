@@ -117,6 +117,8 @@ struct SmallArgs {
                           // no arrive); many: plain remote stores + one fence and arrive per warp (higher throughput)
     int red_alias;        // the pushed partial sums reuse the pipeline stages (large M * K): needs a second cluster
                           // barrier ("every rank's main loop is over") before anybody pushes
+    int early_push;       // CS > 1, dedicated partial-sum area, several local segments: every finished segment is committed on its own
+                          // barrier and pushed while the next ones still stream
     int ring;             // CS == 1, planes: number of TMEM slots the segments cycle through (0 = every local
                           // segment keeps its own slot until the end)
     int b_static;         // HEAL_B_STATIC: W may be read before the stream predecessor has completed
@@ -199,6 +201,8 @@ heal_gemm_smallm_kernel(const __grid_constant__ CUtensorMap tm_x_hi, const __gri
         mbar_init(done_bar, 1);
         mbar_init(red_bar, args.red_async ? 1 : cs * 4); // async: completes when every pushed byte has landed;
                                                          // else one arrival per epilogue warp of every rank
+        if (args.early_push)                                   // (no ring in a cluster: the slots' barriers are free)
+            for (int j = 0; j < min(16, args.max_local); ++j) mbar_init(tfull_bar(j), 1);
         for (int j = 0; j < ring; ++j) {
             mbar_init(tfull_bar(j), 1);
             mbar_init(tempty_bar(j), PAIR ? 8 : 4);      // PAIR: lives in the leader, 4 epilogue warps of each CTA
@@ -394,6 +398,7 @@ heal_gemm_smallm_kernel(const __grid_constant__ CUtensorMap tm_x_hi, const __gri
                 }
                 commit(empty_bar(stage));
                 if (ring && sp.last) commit(tfull_bar(slot));                                  // segment complete
+                if (args.early_push && sp.last && seg_j < 16) commit(tfull_bar(seg_j));
                 if (++stage == STAGES) { stage = 0; phase ^= 1u; }
             }
             commit(done_bar);                              // all local segments complete in TMEM
@@ -526,8 +531,10 @@ heal_gemm_smallm_kernel(const __grid_constant__ CUtensorMap tm_x_hi, const __gri
         // the cluster barrier of the prologue ("every rank's red_bar is initialised") is collected here, while the tensor core
         // is still busy, instead of between the last commit and the first push (barrier.cluster.wait.acquire costs ~0.2 us)
         if (cs > 1) cluster_wait();
-        mbar_wait_ool(done_bar, 0, args.diag, 700);
-        tc_fence_after();
+        if (!args.early_push) {
+            mbar_wait_ool(done_bar, 0, args.diag, 700);
+            tc_fence_after();
+        }
         if (et == 0) HEAL_STAMP(args.trace, 6);
         if (cs == 1) {
             // single-CTA panel: all segments are local slots; sum them in ascending order in registers
@@ -566,6 +573,10 @@ heal_gemm_smallm_kernel(const __grid_constant__ CUtensorMap tm_x_hi, const __gri
             // rpr % 4 == 0 [rpr / 4][nl] 16-byte vectors of four consecutive rows
             const int rpr = args.rows_per_rank;
             for (int j = 0; j < n_local; ++j) {
+                if (args.early_push) {                     // this segment's MMAs have retired (the later ones may still be running)
+                    mbar_wait_ool(j < 16 ? tfull_bar(j) : done_bar, 0, args.diag, 730);
+                    tc_fence_after();
+                }
                 const int seg = static_cast<int>(rank) + j * static_cast<int>(cs);
                 const uint32_t row_off = static_cast<uint32_t>((seg * kSmallBNW + nl) * rpr) * 4u;
 #pragma unroll
@@ -615,6 +626,7 @@ heal_gemm_smallm_kernel(const __grid_constant__ CUtensorMap tm_x_hi, const __gri
                 }
             }
 #undef HEAL_PAST_LAST_TOKEN
+            if (args.early_push) mbar_wait_ool(done_bar, 0, args.diag, 731);       // every MMA (and its commits) has retired
             tc_fence_before();
             if (!args.red_async) {
                 __syncwarp();
