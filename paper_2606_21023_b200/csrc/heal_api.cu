@@ -970,7 +970,7 @@ int launch_small_cfg(int64_t M, int64_t N, int64_t K, const SmallIn &in, const v
     }
     args.ring = ring;
     static const bool no_early = std::getenv("HEAL_NO_EARLY_PUSH") != nullptr;      // debug only
-    args.early_push = (cs > 1 && !red_alias && max_local >= 2 && !no_early) ? 1 : 0;
+    args.early_push = (cs > 1 && !red_alias && max_local >= 2 && max_local <= 16 && !no_early) ? 1 : 0;
     static const bool no_static = std::getenv("HEAL_NO_STATIC") != nullptr;       // debug only
     args.b_static = (in.b_static && !no_static) ? 1 : 0;
     args.diag = g.diag;

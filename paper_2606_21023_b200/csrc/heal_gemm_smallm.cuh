@@ -202,7 +202,7 @@ heal_gemm_smallm_kernel(const __grid_constant__ CUtensorMap tm_x_hi, const __gri
         mbar_init(red_bar, args.red_async ? 1 : cs * 4); // async: completes when every pushed byte has landed;
                                                          // else one arrival per epilogue warp of every rank
         if (args.early_push)                                   // (no ring in a cluster: the slots' barriers are free)
-            for (int j = 0; j < min(16, args.max_local); ++j) mbar_init(tfull_bar(j), 1);
+            for (int j = 0; j < args.max_local; ++j) mbar_init(tfull_bar(j), 1);
         for (int j = 0; j < ring; ++j) {
             mbar_init(tfull_bar(j), 1);
             mbar_init(tempty_bar(j), PAIR ? 8 : 4);      // PAIR: lives in the leader, 4 epilogue warps of each CTA
@@ -354,6 +354,7 @@ heal_gemm_smallm_kernel(const __grid_constant__ CUtensorMap tm_x_hi, const __gri
             int stage = 0;
             uint32_t phase = 0;
             uint32_t accumulate = 0;
+            const int seg_commit = ring | args.early_push;        // (early push: at most 16 local segments, slot = local segment)
             for (int t = 0; t < n_steps; ++t) {
                 const SmallStep sp = small_step<Cfg::SCALED>(t, n_t, n_local);
                 const int seg_j = sp.seg_j;
@@ -397,8 +398,7 @@ heal_gemm_smallm_kernel(const __grid_constant__ CUtensorMap tm_x_hi, const __gri
                     if (NPROD == 4) mma(d_tmem, w_lo + wo, x_lo + xo, 1);
                 }
                 commit(empty_bar(stage));
-                if (ring && sp.last) commit(tfull_bar(slot));                                  // segment complete
-                if (args.early_push && sp.last && seg_j < 16) commit(tfull_bar(seg_j));
+                if (seg_commit && sp.last) commit(tfull_bar(slot));                            // segment complete (ring / early push)
                 if (++stage == STAGES) { stage = 0; phase ^= 1u; }
             }
             commit(done_bar);                              // all local segments complete in TMEM
@@ -574,7 +574,7 @@ heal_gemm_smallm_kernel(const __grid_constant__ CUtensorMap tm_x_hi, const __gri
             const int rpr = args.rows_per_rank;
             for (int j = 0; j < n_local; ++j) {
                 if (args.early_push) {                     // this segment's MMAs have retired (the later ones may still be running)
-                    mbar_wait_ool(j < 16 ? tfull_bar(j) : done_bar, 0, args.diag, 730);
+                    mbar_wait_ool(tfull_bar(j), 0, args.diag, 730);
                     tc_fence_after();
                 }
                 const int seg = static_cast<int>(rank) + j * static_cast<int>(cs);
